@@ -1,0 +1,216 @@
+/* awr.h - C ABI of the B200-native AsyncWebRL token-loss library (libawr.so).
+ *
+ * What it computes (all citations are /root/reference/PAPER.md lines; "A<n>" / "O<n>" are
+ * the readings and oracle steps of SURVEY.md section 8(c), restated in DESIGN.md):
+ *
+ *   J(theta) = E[ 1/(G k) sum_i sum_j sum_t min( (pi_theta/pi_behave) A_i ,
+ *                 (pi_prox/pi_behave) clip(pi_theta/pi_prox, 1-eps, 1+eps) A_i ) ]   Eq. (1), :57
+ *   A_i = (r_i - mean(r)) / std(r) over the G rollouts of one task                    :61
+ *   1/k (constant, k = 10) or the standard 1/|tau_i| (steps of rollout i)             :55, :59
+ *
+ * per token t of trajectory i of group g, with z_t the logits row and y_t the sampled id:
+ *   l_t = z_t[y_t] - logsumexp(z_t)          r_t = exp(l_t - prox_lp_t)
+ *   w_t = exp(prox_lp_t - behave_lp_t), truncated at stale_cap if 0 < stale_cap < inf (A4)
+ *   u = r_t A_i ; v = clip(r_t, 1-eps, 1+eps) A_i ; trig_t = (v < u)                  (A5, A6)
+ *   scale_i = loss_scale / (NG * G_g) * (1/k_norm | 1/|tau_i|)                        (A1, O6)
+ *   term_t = scale_i w_t min(u, v)           loss = - sum_t term_t  (fixed order, fp64 sum)
+ *   c_t = trig_t ? 0 : scale_i w_t r_t A_i   dlogits[t, v] = c_t (softmax(z_t)_v - [v = y_t])
+ *   clip_count = sum_t trig_t
+ *
+ * Conventions
+ *   - Every pointer in awr_batch / awr_outputs / awr_head_* is a DEVICE pointer owned by the
+ *     caller; inputs are read-only; outputs are overwritten (never accumulated into).
+ *     Only awr_loss_fwd_bwd_host takes HOST pointers (stated there).
+ *   - Calls only enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the legacy
+ *     default stream).  No allocation, no host synchronisation, no hidden state; outputs are
+ *     valid once the stream has been synchronised.  Graph-capturable.
+ *   - Return value: AWR_OK or a negative awr_status.  Host-side checks cover scalars, null
+ *     pointers, alignment and workspace size only.  Data-dependent faults set bits in
+ *     *err_word (AWR_ERRBIT_*) and the affected token contributes nothing.
+ *   - target_ids[t] < 0 marks a masked token: zero term, zero dlogits row, token_lp = 0,
+ *     never counted (A13).  target_ids[t] >= V additionally sets AWR_ERRBIT_TARGET_RANGE.
+ *   - Rows: logits[t * ld + v], 0 <= v < V, ld >= V; every row start must be 16-byte aligned
+ *     (base pointer 16-B aligned and ld * sizeof(element) % 16 == 0).  Columns >= V are never
+ *     read or written.  dlogits has the same dtype and stride and MAY alias logits exactly
+ *     (in-place); any other overlap is undefined.
+ *   - The device must be compute capability 10.x (sm_100a code only): otherwise AWR_ERR_ARCH.
+ *     There is no CPU or other-architecture fallback.
+ */
+#ifndef AWR_H_
+#define AWR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AWR_VERSION 100
+
+#if defined(__GNUC__)
+#define AWR_API __attribute__((visibility("default")))
+#else
+#define AWR_API
+#endif
+
+typedef enum awr_status {
+    AWR_OK = 0,
+    AWR_ERR_NULL = -1,      /* a required pointer is NULL */
+    AWR_ERR_SHAPE = -2,     /* negative / inconsistent sizes, ld < V, counts overflowing int32 */
+    AWR_ERR_DTYPE = -3,     /* unknown dtype / layout enum */
+    AWR_ERR_ALIGN = -4,     /* row starts not 16-byte aligned */
+    AWR_ERR_PARAM = -5,     /* k_norm <= 0, clip_eps outside [0,1), NaN scalars, bad enum */
+    AWR_ERR_WORKSPACE = -6, /* workspace NULL, misaligned (256 B) or too small */
+    AWR_ERR_ARCH = -7,      /* current device is not sm_100 */
+    AWR_ERR_CUDA = -8       /* a CUDA runtime call / launch failed (cudaGetLastError cleared) */
+} awr_status;
+
+enum { AWR_DTYPE_BF16 = 0, AWR_DTYPE_F32 = 1 };
+enum { AWR_NORM_CONST_K = 0,   /* n_i = 1 / k_norm   (:59) */
+       AWR_NORM_PER_TRAJ = 1   /* n_i = 1 / |tau_i|  (:55) */ };
+enum { AWR_FLAG_SAMPLE_STD = 1u /* A2: std with 1/(G-1) instead of the default 1/G */ };
+enum { AWR_W_K_BY_V = 0 /* w_head[k * V + v] */, AWR_W_V_BY_K = 1 /* w_head[v * K + k] */ };
+enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
+       AWR_KERNEL_GENERIC = 1,  /* one CTA per row, second pass re-reads the row through L2 */
+       AWR_KERNEL_CLUSTER = 2   /* row resident in the shared memory of a 2-CTA cluster (bf16) */ };
+enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
+       AWR_ERRBIT_TARGET_RANGE = 8u };
+
+/* One batch of response tokens (:61 "G rollouts per task, |tau_i| steps per rollout,
+ * |tau_{i,j}| tokens per step"), as three CSR offset arrays.  Each offset array starts at 0,
+ * is non-decreasing and ends at the count of the level below (O1); violations set
+ * AWR_ERRBIT_* and give unspecified (but memory-safe) results. */
+typedef struct awr_batch {
+    int64_t n_tok;              /* rows of logits = response tokens in the batch */
+    int64_t V;                  /* vocabulary size */
+    int64_t ld;                 /* row stride in elements, >= V */
+    const void* logits;         /* [n_tok, ld], dtype logits_dtype */
+    const int32_t* target_ids;  /* [n_tok] sampled token y_t; < 0 = masked */
+    const float* behave_lp;     /* [n_tok] log pi_behave(y_t) (:53) */
+    const float* prox_lp;       /* [n_tok] log pi_prox(y_t)   (:53, :436) */
+    const int32_t* step_off;    /* [n_steps + 1] token index where each step starts */
+    const int32_t* traj_off;    /* [n_traj + 1]  step index where each trajectory starts */
+    const int32_t* group_off;   /* [n_groups + 1] trajectory index where each group starts */
+    const float* rewards;       /* [n_traj] r_i (:73 binary in the paper; any finite f32) */
+    int32_t n_steps;
+    int32_t n_traj;
+    int32_t n_groups;
+    int32_t logits_dtype;       /* AWR_DTYPE_* */
+} awr_batch;
+
+typedef struct awr_params {
+    float k_norm;       /* the constant k of 1/k (:59), > 0; used when normalizer == CONST_K */
+    float clip_eps;     /* eps of the decoupled clip (:57), in [0, 1); paper: 0.2 (:437) */
+    float stale_cap;    /* A4: w_t <- min(w_t, cap); <= 0 or +inf = off (Eq. 1 exactly) */
+    float loss_scale;   /* multiplies loss and gradient (micro-batching); 1 = Eq. 1 */
+    float dual_clip_c;  /* reserved for Eq. (2) (:270); must be <= 1 (= off) in this version */
+    int32_t normalizer; /* AWR_NORM_* */
+    uint32_t flags;     /* AWR_FLAG_*; unknown bits -> AWR_ERR_PARAM */
+    int32_t kernel;     /* AWR_KERNEL_*; CLUSTER on an unsupported shape -> AWR_ERR_PARAM */
+} awr_params;
+
+typedef struct awr_outputs {
+    float* loss;            /* [1]  -J, f32 (summed in fp64 in token order, then rounded) */
+    void* dlogits;          /* [n_tok, ld] same dtype/stride as logits; NULL in awr_loss_fwd */
+    float* token_lp;        /* [n_tok] l_t = log pi_theta(y_t); 0 for masked tokens */
+    int64_t* clip_count;    /* [1] number of tokens with trig_t */
+    /* optional (NULL = not wanted) */
+    float* adv;             /* [n_traj] A_i */
+    int32_t* tok_traj;      /* [n_tok] trajectory index of each token */
+    float* target_logit;    /* [n_tok] z_t[y_t] widened to f32 (exact); 0 for masked tokens */
+    float* tok_term;        /* [n_tok] per-token contribution to J (loss = -sum) */
+    float* tok_coef;        /* [n_tok] c_t */
+    uint32_t* err_word;     /* [1] OR of AWR_ERRBIT_* (0 = clean) */
+} awr_outputs;
+
+/* a0..a4 fused: segment expansion, group advantage (:61), online log-sum-exp + target gather,
+ * decoupled ratio / clip / normalizer (Eq. 1, :57-:59) and the gradient write.  4 launches. */
+AWR_API int awr_loss_fwd_bwd(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
+                     void* workspace, size_t workspace_bytes, void* stream);
+
+/* Forward only: loss, token_lp, clip_count (and the optional per-token outputs); out->dlogits
+ * is ignored.  Reads each row once, writes no gradient. */
+AWR_API int awr_loss_fwd(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
+                 void* workspace, size_t workspace_bytes, void* stream);
+
+/* Kernel 1 alone (:61).  One warp per group.  flags: AWR_FLAG_SAMPLE_STD. */
+AWR_API int awr_group_advantage(const float* rewards, const int32_t* group_off, int32_t n_groups,
+                        int32_t n_traj, uint32_t flags, float* adv, void* stream);
+
+/* Bytes of device workspace awr_loss_fwd_bwd / awr_loss_fwd need (256-B aligned pointer). */
+AWR_API size_t awr_workspace_bytes(int64_t n_tok, int64_t V, int32_t n_steps, int32_t n_traj,
+                           int32_t n_groups);
+
+/* Same path with HOST buffers: every pointer in `batch` and `out` is a host pointer (pinned
+ * memory gives full PCIe speed; pageable works).  Rows are staged through `dev_workspace` in
+ * panels: H2D copy, the same kernels in place on the panel, D2H copy of the gradient panel, on
+ * three internal non-blocking streams ordered after `stream`; the call returns after the
+ * results are in the host buffers (it synchronises).  dev_workspace: device pointer of at
+ * least awr_host_workspace_bytes(...) bytes. */
+AWR_API int awr_loss_fwd_bwd_host(const awr_batch* host_batch, const awr_params* params,
+                          const awr_outputs* host_out, void* dev_workspace,
+                          size_t dev_workspace_bytes, void* stream);
+AWR_API size_t awr_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t ld, int32_t logits_dtype,
+                                int32_t n_steps, int32_t n_traj, int32_t n_groups);
+
+/* a5 (BASELINE.json config 4): hidden states + LM head instead of logits.  logits = hidden
+ * [n_tok, K] x w_head, never written to memory, fp32 accumulation fed straight to the
+ * log-sum-exp (A17).  Outputs dhidden = dS W^T and dw_head = H^T dS (bf16, overwritten). */
+typedef struct awr_head_batch {
+    int64_t n_tok;
+    int64_t V;
+    int64_t K;                  /* hidden size; multiple of 64 */
+    const void* hidden;         /* bf16 [n_tok, K] row-major */
+    const void* w_head;         /* bf16, layout w_layout */
+    const int32_t* target_ids;
+    const float* behave_lp;
+    const float* prox_lp;
+    const int32_t* step_off;
+    const int32_t* traj_off;
+    const int32_t* group_off;
+    const float* rewards;
+    int32_t n_steps;
+    int32_t n_traj;
+    int32_t n_groups;
+    int32_t w_layout;           /* AWR_W_* */
+} awr_head_batch;
+
+typedef struct awr_head_outputs {
+    float* loss;
+    void* dhidden;          /* bf16 [n_tok, K] */
+    void* dw_head;          /* bf16, same layout as w_head */
+    float* token_lp;
+    int64_t* clip_count;
+    float* adv;             /* optional */
+    int32_t* tok_traj;      /* optional */
+    float* tok_term;        /* optional */
+    float* tok_coef;        /* optional */
+    uint32_t* err_word;     /* optional */
+} awr_head_outputs;
+
+AWR_API int awr_loss_fwd_bwd_fused_head(const awr_head_batch* batch, const awr_params* params,
+                                const awr_head_outputs* out, void* workspace,
+                                size_t workspace_bytes, void* stream);
+AWR_API size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
+                                int32_t n_traj, int32_t n_groups);
+
+AWR_API const char* awr_status_string(int status);
+AWR_API int awr_version(void);
+
+/* Introspection for benchmarks and tests: which row kernel AWR_KERNEL_AUTO resolves to for
+ * this shape (AWR_KERNEL_GENERIC or AWR_KERNEL_CLUSTER), and the number of kernel launches one
+ * awr_loss_fwd_bwd call enqueues. */
+AWR_API int awr_select_kernel(int64_t V, int64_t ld, int32_t logits_dtype);
+AWR_API int awr_launches_per_call(void);
+
+/* Measurement hook (bench.py "roofline"): the NEXT awr_loss_fwd_bwd / awr_loss_fwd call made by
+ * any thread records `ev_before` / `ev_after` (two cudaEvent_t created by the caller with timing
+ * enabled) on its stream immediately around the row kernel (a2 + a3 + a4), then forgets them.
+ * Pass NULL, NULL to cancel.  Not thread-safe by design: a profiling aid, not part of the path. */
+AWR_API int awr_profile_next_row_kernel(void* ev_before, void* ev_after);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AWR_H_ */

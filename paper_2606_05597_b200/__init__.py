@@ -1,0 +1,10 @@
+"""B200-native fused AsyncWebRL token loss (decoupled-PPO / multi-step GRPO, Eq. 1)
+and its gradient over the LM-head vocabulary: hand-written sm_100a CUDA kernels behind the C ABI
+of include/awr.h (libawr.so), plus this thin torch-tensor binding.  No CPU fallback exists."""
+from ._abi import (AwrError, DTYPE_BF16, DTYPE_F32, ERRBIT_GROUP_OFF, ERRBIT_STEP_OFF,
+                   ERRBIT_TARGET_RANGE, ERRBIT_TRAJ_OFF, FLAG_SAMPLE_STD, KERNEL_AUTO,
+                   KERNEL_CLUSTER, KERNEL_GENERIC, NORM_CONST_K, NORM_PER_TRAJ, W_K_BY_V,
+                   W_V_BY_K, lib_path, load)
+from .api import (HostLossCall, LossCall, OPTIONAL_OUTPUTS, awr_group_advantage, awr_loss_fwd,
+                  awr_loss_fwd_bwd, awr_loss_fwd_bwd_host, host_workspace_bytes,
+                  launches_per_call, make_params, profile_next_row_kernel, select_kernel, workspace_bytes)

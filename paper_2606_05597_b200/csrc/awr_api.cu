@@ -1,0 +1,414 @@
+// C-ABI entry points of libawr.so (include/awr.h): argument checks, workspace layout, launch
+// sequencing.  Every step of the path runs in the kernels; nothing here computes.
+#include <math.h>
+#include <string.h>
+
+#include "awr_common.cuh"
+#include "awr_kernels.h"
+
+namespace awr {
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct DeviceInfo {
+    int major = -1;
+    int num_sms = 0;
+};
+
+static cudaError_t device_info(DeviceInfo& info) {
+    static DeviceInfo cache[64];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64 && cache[dev].major >= 0) { info = cache[dev]; return cudaSuccess; }
+    DeviceInfo d;
+    e = cudaDeviceGetAttribute(&d.major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&d.num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64) cache[dev] = d;
+    info = d;
+    return cudaSuccess;
+}
+
+// Device workspace of awr_loss_fwd_bwd / awr_loss_fwd.
+struct Workspace {
+    uint32_t* err;
+    float* adv;
+    float* traj_scale;
+    int32_t* tok_traj;
+    float* tok_term;
+    uint8_t* tok_flag;
+    size_t zero_bytes;   // [err, adv, traj_scale] prefix that is memset to 0
+    size_t total;
+};
+
+static Workspace carve(void* base, int64_t n_tok, int32_t n_traj) {
+    Workspace w;
+    uint8_t* p = reinterpret_cast<uint8_t*>(base);
+    size_t off = 0;
+    w.err = reinterpret_cast<uint32_t*>(p + off); off += 256;
+    w.adv = reinterpret_cast<float*>(p + off); off += align_up((size_t)n_traj * 4, 256);
+    w.traj_scale = reinterpret_cast<float*>(p + off); off += align_up((size_t)n_traj * 4, 256);
+    w.zero_bytes = off;
+    w.tok_traj = reinterpret_cast<int32_t*>(p + off); off += align_up((size_t)n_tok * 4, 256);
+    w.tok_term = reinterpret_cast<float*>(p + off); off += align_up((size_t)n_tok * 4, 256);
+    w.tok_flag = reinterpret_cast<uint8_t*>(p + off); off += align_up((size_t)n_tok, 256);
+    w.total = off;
+    return w;
+}
+
+static int check_params(const awr_params* p) {
+    if (!(p->k_norm > 0.f) || !isfinite(p->k_norm)) return AWR_ERR_PARAM;
+    if (!(p->clip_eps >= 0.f && p->clip_eps < 1.f)) return AWR_ERR_PARAM;
+    if (isnan(p->stale_cap)) return AWR_ERR_PARAM;
+    if (!isfinite(p->loss_scale)) return AWR_ERR_PARAM;
+    if (p->dual_clip_c > 1.f) return AWR_ERR_PARAM;          // Eq. (2) reserved
+    if (p->normalizer != AWR_NORM_CONST_K && p->normalizer != AWR_NORM_PER_TRAJ) return AWR_ERR_PARAM;
+    if (p->flags & ~(uint32_t)AWR_FLAG_SAMPLE_STD) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER) return AWR_ERR_PARAM;
+    return AWR_OK;
+}
+
+static int check_segments(int64_t n_tok, int32_t n_steps, int32_t n_traj, int32_t n_groups) {
+    if (n_tok < 0 || n_steps < 0 || n_traj < 0 || n_groups < 0) return AWR_ERR_SHAPE;
+    if (n_tok > 0x7fffffffLL) return AWR_ERR_SHAPE;            // offsets are int32
+    return AWR_OK;
+}
+
+static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype) {
+    const bool ok = rows_cluster_supported(V, ld, dtype);
+    if (requested == AWR_KERNEL_CLUSTER) return ok ? AWR_KERNEL_CLUSTER : -1;
+    if (requested == AWR_KERNEL_GENERIC) return AWR_KERNEL_GENERIC;
+    // auto: the cluster kernel pays off once a row is a sizeable fraction of shared memory
+    return (ok && V * 2 >= 65536) ? AWR_KERNEL_CLUSTER : AWR_KERNEL_GENERIC;
+}
+
+static cudaEvent_t g_prof_before = nullptr, g_prof_after = nullptr;
+
+static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, void* ws_ptr,
+               size_t ws_bytes, void* stream, bool backward) {
+    if (!b || !p || !o) return AWR_ERR_NULL;
+    int rc = check_segments(b->n_tok, b->n_steps, b->n_traj, b->n_groups);
+    if (rc) return rc;
+    if (b->V <= 0 || b->ld < b->V) return AWR_ERR_SHAPE;
+    if (b->logits_dtype != AWR_DTYPE_BF16 && b->logits_dtype != AWR_DTYPE_F32) return AWR_ERR_DTYPE;
+    rc = check_params(p);
+    if (rc) return rc;
+    if (!o->loss || !o->clip_count) return AWR_ERR_NULL;
+    if (b->n_tok > 0 && (!o->token_lp || (backward && !o->dlogits))) return AWR_ERR_NULL;
+    if (!b->step_off || !b->traj_off || !b->group_off) return AWR_ERR_NULL;
+    if (b->n_tok > 0 && (!b->logits || !b->target_ids || !b->behave_lp || !b->prox_lp)) return AWR_ERR_NULL;
+    if (b->n_traj > 0 && !b->rewards) return AWR_ERR_NULL;
+    const size_t esz = b->logits_dtype == AWR_DTYPE_BF16 ? 2 : 4;
+    if ((reinterpret_cast<uintptr_t>(b->logits) & 15) || ((size_t)b->ld * esz) % 16) return AWR_ERR_ALIGN;
+    if (backward && (reinterpret_cast<uintptr_t>(o->dlogits) & 15)) return AWR_ERR_ALIGN;
+    const size_t need = awr_workspace_bytes(b->n_tok, b->V, b->n_steps, b->n_traj, b->n_groups);
+    if (!ws_ptr || (reinterpret_cast<uintptr_t>(ws_ptr) & 255) || ws_bytes < need) return AWR_ERR_WORKSPACE;
+    const int kernel = resolve_kernel(p->kernel, b->V, b->ld, b->logits_dtype);
+    if (kernel < 0) return AWR_ERR_PARAM;
+
+    DeviceInfo info;
+    if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    if (info.major != 10) return AWR_ERR_ARCH;
+
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Workspace w = carve(ws_ptr, b->n_tok, b->n_traj);
+    uint32_t* err = o->err_word ? o->err_word : w.err;
+    float* adv = o->adv ? o->adv : w.adv;
+    int32_t* tok_traj = o->tok_traj ? o->tok_traj : w.tok_traj;
+    float* tok_term = o->tok_term ? o->tok_term : w.tok_term;
+
+    cudaError_t e = cudaMemsetAsync(ws_ptr, 0, w.zero_bytes, st);
+    if (e == cudaSuccess && o->err_word) e = cudaMemsetAsync(o->err_word, 0, 4, st);
+    if (e == cudaSuccess && o->adv && b->n_traj > 0) e = cudaMemsetAsync(o->adv, 0, (size_t)b->n_traj * 4, st);
+    // a0
+    if (e == cudaSuccess)
+        e = launch_segment_expand(b->step_off, b->traj_off, b->group_off, b->n_tok, b->n_steps,
+                                  b->n_traj, b->n_groups, tok_traj, err, st);
+    // a1 (+ O6 scale)
+    if (e == cudaSuccess)
+        e = launch_group_advantage(b->rewards, b->group_off, b->traj_off, b->n_groups, b->n_traj,
+                                   p->flags, p->normalizer, p->k_norm, p->loss_scale, adv,
+                                   w.traj_scale, st);
+    // a2 + a3 + a4
+    RowArgs a;
+    a.logits = b->logits;
+    a.dlogits = backward ? o->dlogits : nullptr;
+    a.n_tok = b->n_tok; a.V = b->V; a.ld = b->ld;
+    a.target_ids = b->target_ids; a.behave_lp = b->behave_lp; a.prox_lp = b->prox_lp;
+    a.tok_traj = tok_traj; a.adv = adv; a.traj_scale = w.traj_scale;
+    a.token_lp = o->token_lp; a.tok_term = tok_term; a.tok_coef = o->tok_coef;
+    a.target_logit = o->target_logit; a.tok_flag = w.tok_flag; a.err_word = err;
+    a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap;
+    cudaEvent_t ev0 = g_prof_before, ev1 = g_prof_after;
+    g_prof_before = g_prof_after = nullptr;
+    if (e == cudaSuccess && ev0) e = cudaEventRecord(ev0, st);
+    if (e == cudaSuccess) {
+        e = kernel == AWR_KERNEL_CLUSTER ? launch_rows_cluster(a, info.num_sms, st)
+                                         : launch_rows_generic(a, b->logits_dtype, info.num_sms, st);
+    }
+    if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, st);
+    // a3 final reduction
+    if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    return AWR_OK;
+}
+
+}  // namespace awr
+
+using namespace awr;
+
+extern "C" {
+
+int awr_version(void) { return AWR_VERSION; }
+
+const char* awr_status_string(int s) {
+    switch (s) {
+        case AWR_OK: return "ok";
+        case AWR_ERR_NULL: return "required pointer is NULL";
+        case AWR_ERR_SHAPE: return "bad sizes";
+        case AWR_ERR_DTYPE: return "unknown dtype or layout";
+        case AWR_ERR_ALIGN: return "rows must start on 16-byte boundaries";
+        case AWR_ERR_PARAM: return "parameter out of range";
+        case AWR_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+        case AWR_ERR_ARCH: return "device is not sm_100 (B200); no fallback exists";
+        case AWR_ERR_CUDA: return "CUDA runtime error";
+        default: return "unknown status";
+    }
+}
+
+size_t awr_workspace_bytes(int64_t n_tok, int64_t V, int32_t n_steps, int32_t n_traj,
+                           int32_t n_groups) {
+    (void)V; (void)n_steps; (void)n_groups;
+    if (n_tok < 0 || n_traj < 0) return 0;
+    return carve(nullptr, n_tok, n_traj).total;
+}
+
+int awr_select_kernel(int64_t V, int64_t ld, int32_t logits_dtype) {
+    return resolve_kernel(AWR_KERNEL_AUTO, V, ld, logits_dtype);
+}
+
+int awr_launches_per_call(void) { return 4; }
+
+int awr_profile_next_row_kernel(void* ev_before, void* ev_after) {
+    if ((ev_before == nullptr) != (ev_after == nullptr)) return AWR_ERR_NULL;
+    g_prof_before = reinterpret_cast<cudaEvent_t>(ev_before);
+    g_prof_after = reinterpret_cast<cudaEvent_t>(ev_after);
+    return AWR_OK;
+}
+
+int awr_loss_fwd_bwd(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
+                     void* workspace, size_t workspace_bytes, void* stream) {
+    return run(batch, params, out, workspace, workspace_bytes, stream, true);
+}
+
+int awr_loss_fwd(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
+                 void* workspace, size_t workspace_bytes, void* stream) {
+    return run(batch, params, out, workspace, workspace_bytes, stream, false);
+}
+
+int awr_group_advantage(const float* rewards, const int32_t* group_off, int32_t n_groups,
+                        int32_t n_traj, uint32_t flags, float* adv, void* stream) {
+    if (n_groups < 0 || n_traj < 0) return AWR_ERR_SHAPE;
+    if (flags & ~(uint32_t)AWR_FLAG_SAMPLE_STD) return AWR_ERR_PARAM;
+    if (!group_off || (n_traj > 0 && (!rewards || !adv))) return AWR_ERR_NULL;
+    DeviceInfo info;
+    if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    if (info.major != 10) return AWR_ERR_ARCH;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaSuccess;
+    if (n_traj > 0) e = cudaMemsetAsync(adv, 0, (size_t)n_traj * 4, st);
+    if (e == cudaSuccess)
+        e = launch_group_advantage(rewards, group_off, nullptr, n_groups, n_traj, flags,
+                                   AWR_NORM_CONST_K, 1.f, 1.f, adv, nullptr, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    return AWR_OK;
+}
+
+// ------------------------------------------------------------------ host-buffer variant
+namespace {
+constexpr int kPanelBufs = 3;
+
+struct HostPlan {
+    int64_t panel_rows;
+    size_t panel_bytes;   // per buffer
+    size_t small_bytes;   // per-token / per-segment arrays
+    size_t ws_bytes;      // awr_workspace_bytes
+    size_t total;
+};
+
+HostPlan host_plan(int64_t n_tok, int64_t V, int64_t ld, int32_t dtype, int32_t n_steps,
+                   int32_t n_traj, int32_t n_groups) {
+    HostPlan h;
+    const size_t esz = dtype == AWR_DTYPE_BF16 ? 2 : 4;
+    const size_t row_bytes = (size_t)ld * esz;
+    int64_t rows = (int64_t)((256u << 20) / (row_bytes ? row_bytes : 1));
+    rows = rows / 74 * 74;                         // whole waves of the 74-cluster schedule
+    if (rows < 74) rows = 74;
+    if (rows > n_tok) rows = n_tok > 0 ? n_tok : 1;
+    h.panel_rows = rows;
+    h.panel_bytes = align_up((size_t)rows * row_bytes, 256);
+    size_t s = 0;
+    s += align_up((size_t)n_tok * 4, 256) * 4;     // target_ids, behave_lp, prox_lp, token_lp
+    s += align_up((size_t)(n_steps + 1) * 4, 256) + align_up((size_t)(n_traj + 1) * 4, 256) +
+         align_up((size_t)(n_groups + 1) * 4, 256) + align_up((size_t)n_traj * 4, 256);
+    s += 256;                                      // loss, clip_count, err
+    s += align_up((size_t)n_tok * 4, 256) * 4;     // optional tok_traj, target_logit, tok_term, tok_coef
+    s += align_up((size_t)n_traj * 4, 256);        // optional adv
+    h.small_bytes = s;
+    h.ws_bytes = awr_workspace_bytes(n_tok, V, n_steps, n_traj, n_groups);
+    h.total = h.small_bytes + h.ws_bytes + kPanelBufs * h.panel_bytes;
+    return h;
+}
+}  // namespace
+
+size_t awr_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t ld, int32_t logits_dtype,
+                                int32_t n_steps, int32_t n_traj, int32_t n_groups) {
+    if (n_tok < 0 || V <= 0 || ld < V || n_steps < 0 || n_traj < 0 || n_groups < 0) return 0;
+    return host_plan(n_tok, V, ld, logits_dtype, n_steps, n_traj, n_groups).total;
+}
+
+int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_outputs* ho,
+                          void* dev_ws, size_t dev_ws_bytes, void* stream) {
+    if (!hb || !p || !ho) return AWR_ERR_NULL;
+    int rc = check_segments(hb->n_tok, hb->n_steps, hb->n_traj, hb->n_groups);
+    if (rc) return rc;
+    if (hb->V <= 0 || hb->ld < hb->V) return AWR_ERR_SHAPE;
+    if (hb->logits_dtype != AWR_DTYPE_BF16 && hb->logits_dtype != AWR_DTYPE_F32) return AWR_ERR_DTYPE;
+    rc = check_params(p);
+    if (rc) return rc;
+    if (!ho->loss || !ho->clip_count) return AWR_ERR_NULL;
+    if (hb->n_tok > 0 && (!ho->token_lp || !ho->dlogits)) return AWR_ERR_NULL;
+    if (!hb->step_off || !hb->traj_off || !hb->group_off) return AWR_ERR_NULL;
+    if (hb->n_tok > 0 && (!hb->logits || !hb->target_ids || !hb->behave_lp || !hb->prox_lp)) return AWR_ERR_NULL;
+    if (hb->n_traj > 0 && !hb->rewards) return AWR_ERR_NULL;
+    const size_t esz = hb->logits_dtype == AWR_DTYPE_BF16 ? 2 : 4;
+    if (((size_t)hb->ld * esz) % 16) return AWR_ERR_ALIGN;
+    HostPlan hp = host_plan(hb->n_tok, hb->V, hb->ld, hb->logits_dtype, hb->n_steps, hb->n_traj, hb->n_groups);
+    if (!dev_ws || (reinterpret_cast<uintptr_t>(dev_ws) & 255) || dev_ws_bytes < hp.total) return AWR_ERR_WORKSPACE;
+    const int kernel = resolve_kernel(p->kernel, hb->V, hb->ld, hb->logits_dtype);
+    if (kernel < 0) return AWR_ERR_PARAM;
+    DeviceInfo info;
+    if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    if (info.major != 10) return AWR_ERR_ARCH;
+
+    const int64_t n = hb->n_tok;
+    uint8_t* base = reinterpret_cast<uint8_t*>(dev_ws);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { void* r = base + off; off += align_up(bytes, 256); return r; };
+    int32_t* d_ids = (int32_t*)take((size_t)n * 4);
+    float* d_b = (float*)take((size_t)n * 4);
+    float* d_q = (float*)take((size_t)n * 4);
+    float* d_lp = (float*)take((size_t)n * 4);
+    int32_t* d_so = (int32_t*)take((size_t)(hb->n_steps + 1) * 4);
+    int32_t* d_to = (int32_t*)take((size_t)(hb->n_traj + 1) * 4);
+    int32_t* d_go = (int32_t*)take((size_t)(hb->n_groups + 1) * 4);
+    float* d_rw = (float*)take((size_t)hb->n_traj * 4);
+    uint8_t* d_scal = (uint8_t*)take(256);
+    int32_t* d_tt = (int32_t*)take((size_t)n * 4);
+    float* d_tl = (float*)take((size_t)n * 4);
+    float* d_term = (float*)take((size_t)n * 4);
+    float* d_coef = (float*)take((size_t)n * 4);
+    float* d_adv = (float*)take((size_t)hb->n_traj * 4);
+    off = hp.small_bytes;
+    void* d_ws = base + off; off += hp.ws_bytes;
+    uint8_t* d_panel = base + off;
+    float* d_loss = (float*)d_scal;
+    int64_t* d_cnt = (int64_t*)(d_scal + 8);
+    uint32_t* d_err = (uint32_t*)(d_scal + 16);
+
+    cudaStream_t user = reinterpret_cast<cudaStream_t>(stream);
+    cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_in[kPanelBufs] = {}, ev_k[kPanelBufs] = {}, ev_out[kPanelBufs] = {};
+    cudaError_t e = cudaSuccess;
+#define AWR_TRY(x) do { if (e == cudaSuccess) e = (x); } while (0)
+    AWR_TRY(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+    AWR_TRY(cudaStreamCreateWithFlags(&s_k, cudaStreamNonBlocking));
+    AWR_TRY(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+    AWR_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+    for (int i = 0; i < kPanelBufs; ++i) {
+        AWR_TRY(cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming));
+        AWR_TRY(cudaEventCreateWithFlags(&ev_k[i], cudaEventDisableTiming));
+        AWR_TRY(cudaEventCreateWithFlags(&ev_out[i], cudaEventDisableTiming));
+    }
+    AWR_TRY(cudaEventRecord(ev_start, user));
+    AWR_TRY(cudaStreamWaitEvent(s_in, ev_start, 0));
+    AWR_TRY(cudaStreamWaitEvent(s_k, ev_start, 0));
+    AWR_TRY(cudaStreamWaitEvent(s_out, ev_start, 0));
+    // small arrays + a0, a1 on the kernel stream
+    const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
+    if (n > 0) {
+        AWR_TRY(cudaMemcpyAsync(d_ids, hb->target_ids, (size_t)n * 4, H2D, s_k));
+        AWR_TRY(cudaMemcpyAsync(d_b, hb->behave_lp, (size_t)n * 4, H2D, s_k));
+        AWR_TRY(cudaMemcpyAsync(d_q, hb->prox_lp, (size_t)n * 4, H2D, s_k));
+    }
+    AWR_TRY(cudaMemcpyAsync(d_so, hb->step_off, (size_t)(hb->n_steps + 1) * 4, H2D, s_k));
+    AWR_TRY(cudaMemcpyAsync(d_to, hb->traj_off, (size_t)(hb->n_traj + 1) * 4, H2D, s_k));
+    AWR_TRY(cudaMemcpyAsync(d_go, hb->group_off, (size_t)(hb->n_groups + 1) * 4, H2D, s_k));
+    if (hb->n_traj > 0) AWR_TRY(cudaMemcpyAsync(d_rw, hb->rewards, (size_t)hb->n_traj * 4, H2D, s_k));
+    Workspace w = carve(d_ws, n, hb->n_traj);
+    AWR_TRY(cudaMemsetAsync(d_ws, 0, w.zero_bytes, s_k));
+    AWR_TRY(cudaMemsetAsync(d_scal, 0, 256, s_k));
+    if (hb->n_traj > 0) AWR_TRY(cudaMemsetAsync(d_adv, 0, (size_t)hb->n_traj * 4, s_k));
+    AWR_TRY(launch_segment_expand(d_so, d_to, d_go, n, hb->n_steps, hb->n_traj, hb->n_groups, d_tt, d_err, s_k));
+    AWR_TRY(launch_group_advantage(d_rw, d_go, d_to, hb->n_groups, hb->n_traj, p->flags, p->normalizer,
+                                   p->k_norm, p->loss_scale, d_adv, w.traj_scale, s_k));
+    // row panels: H2D -> kernel (in place) -> D2H, three buffers in flight
+    const size_t row_bytes = (size_t)hb->ld * esz;
+    int64_t panel = 0;
+    for (int64_t r0 = 0; r0 < n && e == cudaSuccess; r0 += hp.panel_rows, ++panel) {
+        const int bi = (int)(panel % kPanelBufs);
+        const int64_t rows = (n - r0 < hp.panel_rows) ? (n - r0) : hp.panel_rows;
+        uint8_t* buf = d_panel + (size_t)bi * hp.panel_bytes;
+        if (panel >= kPanelBufs) AWR_TRY(cudaStreamWaitEvent(s_in, ev_out[bi], 0));
+        AWR_TRY(cudaMemcpyAsync(buf, (const uint8_t*)hb->logits + (size_t)r0 * row_bytes,
+                                (size_t)rows * row_bytes, H2D, s_in));
+        AWR_TRY(cudaEventRecord(ev_in[bi], s_in));
+        AWR_TRY(cudaStreamWaitEvent(s_k, ev_in[bi], 0));
+        RowArgs a;
+        a.logits = buf; a.dlogits = buf;                 // in place on the panel
+        a.n_tok = rows; a.V = hb->V; a.ld = hb->ld;
+        a.target_ids = d_ids + r0; a.behave_lp = d_b + r0; a.prox_lp = d_q + r0;
+        a.tok_traj = d_tt + r0; a.adv = d_adv; a.traj_scale = w.traj_scale;
+        a.token_lp = d_lp + r0; a.tok_term = d_term + r0; a.tok_coef = d_coef + r0;
+        a.target_logit = d_tl + r0; a.tok_flag = w.tok_flag + r0; a.err_word = d_err;
+        a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap;
+        AWR_TRY(kernel == AWR_KERNEL_CLUSTER ? launch_rows_cluster(a, info.num_sms, s_k)
+                                             : launch_rows_generic(a, hb->logits_dtype, info.num_sms, s_k));
+        AWR_TRY(cudaEventRecord(ev_k[bi], s_k));
+        AWR_TRY(cudaStreamWaitEvent(s_out, ev_k[bi], 0));
+        AWR_TRY(cudaMemcpyAsync((uint8_t*)ho->dlogits + (size_t)r0 * row_bytes, buf,
+                                (size_t)rows * row_bytes, D2H, s_out));
+        AWR_TRY(cudaEventRecord(ev_out[bi], s_out));
+    }
+    AWR_TRY(launch_final_reduce(d_term, w.tok_flag, n, d_loss, d_cnt, s_k));
+    AWR_TRY(cudaMemcpyAsync(ho->loss, d_loss, 4, D2H, s_k));
+    AWR_TRY(cudaMemcpyAsync(ho->clip_count, d_cnt, 8, D2H, s_k));
+    if (ho->err_word) AWR_TRY(cudaMemcpyAsync(ho->err_word, d_err, 4, D2H, s_k));
+    if (n > 0) {
+        AWR_TRY(cudaMemcpyAsync(ho->token_lp, d_lp, (size_t)n * 4, D2H, s_k));
+        if (ho->tok_traj) AWR_TRY(cudaMemcpyAsync(ho->tok_traj, d_tt, (size_t)n * 4, D2H, s_k));
+        if (ho->target_logit) AWR_TRY(cudaMemcpyAsync(ho->target_logit, d_tl, (size_t)n * 4, D2H, s_k));
+        if (ho->tok_term) AWR_TRY(cudaMemcpyAsync(ho->tok_term, d_term, (size_t)n * 4, D2H, s_k));
+        if (ho->tok_coef) AWR_TRY(cudaMemcpyAsync(ho->tok_coef, d_coef, (size_t)n * 4, D2H, s_k));
+    }
+    if (ho->adv && hb->n_traj > 0) AWR_TRY(cudaMemcpyAsync(ho->adv, d_adv, (size_t)hb->n_traj * 4, D2H, s_k));
+    if (s_in) { cudaError_t e2 = cudaStreamSynchronize(s_in); if (e == cudaSuccess) e = e2; }
+    if (s_k) { cudaError_t e2 = cudaStreamSynchronize(s_k); if (e == cudaSuccess) e = e2; }
+    if (s_out) { cudaError_t e2 = cudaStreamSynchronize(s_out); if (e == cudaSuccess) e = e2; }
+#undef AWR_TRY
+    for (int i = 0; i < kPanelBufs; ++i) {
+        if (ev_in[i]) cudaEventDestroy(ev_in[i]);
+        if (ev_k[i]) cudaEventDestroy(ev_k[i]);
+        if (ev_out[i]) cudaEventDestroy(ev_out[i]);
+    }
+    if (ev_start) cudaEventDestroy(ev_start);
+    if (s_in) cudaStreamDestroy(s_in);
+    if (s_k) cudaStreamDestroy(s_k);
+    if (s_out) cudaStreamDestroy(s_out);
+    if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    return AWR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,29 @@
+// Internal launcher declarations (host side).  Not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace awr {
+
+struct RowArgs;
+
+cudaError_t launch_segment_expand(const int32_t* step_off, const int32_t* traj_off,
+                                  const int32_t* group_off, int64_t n_tok, int n_steps,
+                                  int n_traj, int n_groups, int32_t* tok_traj, uint32_t* err,
+                                  cudaStream_t st);
+cudaError_t launch_group_advantage(const float* rewards, const int32_t* group_off,
+                                   const int32_t* traj_off, int n_groups, int n_traj,
+                                   uint32_t flags, int normalizer, float k_norm,
+                                   float loss_scale, float* adv, float* traj_scale,
+                                   cudaStream_t st);
+cudaError_t launch_final_reduce(const float* tok_term, const uint8_t* tok_flag, int64_t n_tok,
+                                float* loss, int64_t* clip_count, cudaStream_t st);
+
+// a2 + a3 + a4, one CTA per row, any V / dtype (second pass re-reads the row through L2).
+cudaError_t launch_rows_generic(const RowArgs& a, int dtype, int num_sms, cudaStream_t st);
+
+// a2 + a3 + a4, bf16 rows resident in the shared memory of a 2-CTA cluster (TMA bulk copies).
+bool rows_cluster_supported(int64_t V, int64_t ld, int dtype);
+cudaError_t launch_rows_cluster(const RowArgs& a, int num_sms, cudaStream_t st);
+
+}  // namespace awr

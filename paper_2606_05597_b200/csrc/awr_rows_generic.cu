@@ -1,0 +1,159 @@
+// Generic row kernel: a2 (online log-sum-exp + target gather), a3 (ratio / clip / normalizer)
+// and a4 (dlogits write) for any V, any row stride and both dtypes.  One CTA per row; the
+// gradient pass re-reads the row, which at one row per CTA is an L2 hit (<= 148*8 rows of
+// <= 300 KB in flight against 126 MB of L2), so HBM sees one read and one write per element.
+// Plain (coherent) loads: dlogits may alias logits exactly.
+// This is the correctness-first kernel and the path for fp32 logits / small or odd V; large
+// bf16 rows go to the cluster kernel (awr_rows_cluster.cu).
+// PAPER.md:57 (Eq. 1), :435 (token-level IS); gradient: SURVEY.md 8(c) O8.
+#include "awr_common.cuh"
+#include "awr_kernels.h"
+
+namespace awr {
+
+constexpr int kGenericThreads = 256;
+
+template <typename T> struct Elem;
+template <> struct Elem<float> {
+    static constexpr int kPerVec = 4;
+    static __device__ __forceinline__ void unpack(const uint4& v, float* x) {
+        x[0] = __uint_as_float(v.x); x[1] = __uint_as_float(v.y);
+        x[2] = __uint_as_float(v.z); x[3] = __uint_as_float(v.w);
+    }
+    static __device__ __forceinline__ uint4 pack(const float* x) {
+        return make_uint4(__float_as_uint(x[0]), __float_as_uint(x[1]), __float_as_uint(x[2]),
+                          __float_as_uint(x[3]));
+    }
+    static __device__ __forceinline__ float load(const float* p) { return *p; }
+    static __device__ __forceinline__ void store(float* p, float v) { *p = v; }
+};
+template <> struct Elem<__nv_bfloat16> {
+    static constexpr int kPerVec = 8;
+    static __device__ __forceinline__ void unpack(const uint4& v, float* x) {
+        x[0] = bf16_lo(v.x); x[1] = bf16_hi(v.x); x[2] = bf16_lo(v.y); x[3] = bf16_hi(v.y);
+        x[4] = bf16_lo(v.z); x[5] = bf16_hi(v.z); x[6] = bf16_lo(v.w); x[7] = bf16_hi(v.w);
+    }
+    static __device__ __forceinline__ uint4 pack(const float* x) {
+        return make_uint4(pack_bf16x2(x[0], x[1]), pack_bf16x2(x[2], x[3]),
+                          pack_bf16x2(x[4], x[5]), pack_bf16x2(x[6], x[7]));
+    }
+    static __device__ __forceinline__ float load(const __nv_bfloat16* p) {
+        return __bfloat162float(*p);
+    }
+    static __device__ __forceinline__ void store(__nv_bfloat16* p, float v) {
+        *p = __float2bfloat16_rn(v);
+    }
+};
+
+template <typename T>
+__global__ void __launch_bounds__(kGenericThreads)
+rows_generic_kernel(RowArgs a) {
+    using E = Elem<T>;
+    constexpr int EPV = E::kPerVec;
+    __shared__ MaxSum s_red[kGenericThreads / 32];
+    __shared__ float s_coef, s_lse, s_gy;
+    __shared__ int s_y;
+    const int tid = threadIdx.x;
+    const int64_t nvec = a.V / EPV;
+    const int64_t tail0 = nvec * EPV;
+
+    for (int64_t row = blockIdx.x; row < a.n_tok; row += gridDim.x) {
+        const T* z = reinterpret_cast<const T*>(a.logits) + row * a.ld;
+        RowHeader h;
+        bool valid = false;
+        if (tid == 0) h = load_row_header(a, row, valid, sizeof(T) == 2);
+
+        // ---- a2: one streaming pass, per-thread online (max, sum)
+        MaxSum ms{-INFINITY, 0.f};
+        const uint4* zv = reinterpret_cast<const uint4*>(z);
+        for (int64_t i = tid; i < nvec; i += kGenericThreads) {
+            uint4 v = zv[i];
+            float x[EPV];
+            E::unpack(v, x);
+            float cm = x[0];
+#pragma unroll
+            for (int k = 1; k < EPV; ++k) cm = fmaxf(cm, x[k]);
+            if (cm > ms.m) {
+                ms.s *= ex2_approx((ms.m - cm) * kLog2e);
+                ms.m = cm;
+            }
+            float ml = (ms.m == -INFINITY) ? 0.f : ms.m * kLog2e;   // all -inf so far: no NaN
+            float acc = 0.f;
+#pragma unroll
+            for (int k = 0; k < EPV; ++k) acc += ex2_approx(fmaf(x[k], kLog2e, -ml));
+            ms.s += acc;
+        }
+        for (int64_t i = tail0 + tid; i < a.V; i += kGenericThreads) {
+            float x = E::load(z + i);
+            if (x > ms.m) {
+                ms.s *= ex2_approx((ms.m - x) * kLog2e);
+                ms.m = x;
+            }
+            if (ms.m != -INFINITY) ms.s += ex2_approx((x - ms.m) * kLog2e);
+        }
+        ms = warp_combine(ms);
+        if ((tid & 31) == 0) s_red[tid >> 5] = ms;
+        __syncthreads();
+        if (tid == 0) {
+            MaxSum tot = s_red[0];
+#pragma unroll
+            for (int w = 1; w < kGenericThreads / 32; ++w) tot = combine(tot, s_red[w]);
+            float lse = tot.m + logf(tot.s);
+            // ---- a3
+            TokenScalars ts = token_scalars(h, lse, valid, a.clip_eps, a.stale_cap);
+            store_token_outputs(a, row, h, ts, valid);
+            s_coef = ts.coef;
+            s_lse = lse;
+            s_y = valid ? h.y : -1;
+            s_gy = ts.coef * (expf(ts.lp) - 1.0f);   // c_t (p_y - 1)
+        }
+        __syncthreads();
+
+        // ---- a4
+        if (a.dlogits != nullptr) {
+            T* g = reinterpret_cast<T*>(a.dlogits) + row * a.ld;
+            uint4* gv = reinterpret_cast<uint4*>(g);
+            const float coef = s_coef;
+            const int y = s_y;
+            if (coef == 0.f) {
+                const uint4 zero = make_uint4(0, 0, 0, 0);
+                for (int64_t i = tid; i < nvec; i += kGenericThreads) gv[i] = zero;
+                for (int64_t i = tail0 + tid; i < a.V; i += kGenericThreads) E::store(g + i, 0.f);
+            } else {
+                const float nl = -s_lse * kLog2e;
+                const float gy = s_gy;
+                for (int64_t i = tid; i < nvec; i += kGenericThreads) {
+                    uint4 v = zv[i];
+                    float x[EPV];
+                    E::unpack(v, x);
+#pragma unroll
+                    for (int k = 0; k < EPV; ++k) x[k] = coef * ex2_approx(fmaf(x[k], kLog2e, nl));
+                    int64_t base = i * EPV;
+                    if (y >= base && y < base + EPV) x[y - base] = gy;
+                    gv[i] = E::pack(x);
+                }
+                for (int64_t i = tail0 + tid; i < a.V; i += kGenericThreads) {
+                    float x = E::load(z + i);
+                    float gval = (i == y) ? gy : coef * ex2_approx(fmaf(x, kLog2e, nl));
+                    E::store(g + i, gval);
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+cudaError_t launch_rows_generic(const RowArgs& a, int dtype, int num_sms, cudaStream_t st) {
+    if (a.n_tok <= 0) return cudaSuccess;
+    int64_t blocks = a.n_tok;
+    int64_t cap = (int64_t)num_sms * 8;
+    if (blocks > cap) blocks = cap;
+    if (dtype == AWR_DTYPE_BF16) {
+        rows_generic_kernel<__nv_bfloat16><<<(int)blocks, kGenericThreads, 0, st>>>(a);
+    } else {
+        rows_generic_kernel<float><<<(int)blocks, kGenericThreads, 0, st>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace awr

@@ -1,0 +1,252 @@
+"""GPU parity: the CUDA path (through the C ABI / binding) against the fp64 oracle on the same
+seeded inputs, element by element.  Run on the B200 box: pytest -m gpu."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_05597_b200 as A
+from gen import workloads as W
+from oracle import awr_oracle as O
+from tests import parity_util as P
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _require_gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device (run them with gpurun)")
+
+
+@pytest.fixture(autouse=True, scope="module")
+def _gpu():
+    _require_gpu()
+    assert torch.cuda.get_device_capability(0)[0] == 10, "sm_100 only"
+    yield
+
+
+# ------------------------------------------------------------------ config 0 (fp32, V = 1024)
+@pytest.mark.parametrize("norm", [A.NORM_CONST_K, A.NORM_PER_TRAJ])
+@pytest.mark.parametrize("over", [dict(), dict(clip_eps=0.01), dict(stale_cap=1.02),
+                                  dict(k_norm=4.0), dict(flags=A.FLAG_SAMPLE_STD)])
+def test_config0_tiny(norm, over):
+    """BASELINE.json configs[0]: 1 group, k = 4, steps {2,3,5,6}, 16 tokens/step, fp32
+    [256, 1024]; eps 0.2, cap 2.0, both normalizers; parity-only reruns."""
+    w = W.workload(0, normalizer=norm, **over)
+    batch = W.make_batch(w, seed=0, device=DEV)
+    gpu, ora = P.full_check(batch)
+    if over.get("clip_eps") == 0.01:
+        assert ora["clip_count"] > 0
+
+
+def test_config0_all_ratios_one():
+    """P2/P3 on the GPU: b = q = l -> loss is exactly 0 in exact arithmetic, gradient is not."""
+    w = W.workload(0)
+    batch = W.make_batch(w, seed=0, device=DEV)
+    lp = A.awr_loss_fwd(batch["logits"], batch["target_ids"], batch["behave_lp"],
+                        batch["prox_lp"], batch["step_off"], batch["traj_off"],
+                        batch["group_off"], batch["rewards"], **batch["params"])["token_lp"]
+    batch["prox_lp"] = lp.clone()
+    batch["behave_lp"] = lp.clone()
+    gpu, ora = P.full_check(batch)
+    assert int(gpu["clip_count"][0]) == 0
+    assert abs(float(gpu["loss"][0])) < 1e-6
+    assert float(gpu["dlogits"].abs().max()) > 1e-4
+
+
+# ------------------------------------------------------------------ generic kernel, odd shapes
+@pytest.mark.parametrize("V,ld,dtype", [(1003, 1008, torch.bfloat16), (4096, 4096, torch.bfloat16),
+                                        (777, 780, torch.float32), (8, 8, torch.bfloat16),
+                                        (5, 8, torch.float32)])
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_generic_small(V, ld, dtype, cfg):
+    w = W.workload(cfg, n_groups=5, group_size=4, n_tok=700, V=V, dtype=dtype)
+    batch = W.make_batch(w, seed=11 + cfg, device=DEV, ld=ld, masked_frac=0.05)
+    batch["params"]["kernel"] = A.KERNEL_GENERIC
+    P.full_check(batch)
+    P.full_check(batch, backward=False)
+
+
+# ------------------------------------------------------------------ cluster kernel
+CLUSTER_SHAPES = [(151_936, 151_936), (40_000, 40_008), (32_768, 32_768), (65_544, 65_560),
+                  (131_072, 131_072)]
+
+
+@pytest.mark.parametrize("V,ld", CLUSTER_SHAPES)
+def test_cluster_vs_oracle(V, ld):
+    """bf16 rows resident in the shared memory of a 2-CTA cluster; 300+ rows = several rows
+    per cluster plus a ragged tail; masked tokens, zero-advantage groups, clip triggers."""
+    assert A.select_kernel(V, ld, torch.bfloat16) == A.KERNEL_CLUSTER
+    w = W.workload(3, n_groups=6, group_size=4, n_tok=331, V=V)
+    batch = W.make_batch(w, seed=5, device=DEV, ld=ld, masked_frac=0.04)
+    batch["params"]["kernel"] = A.KERNEL_CLUSTER
+    gpu, ora = P.full_check(batch)
+    assert ora["clip_count"] > 0 and (ora["coef"] == 0).sum() > ora["clip_count"]
+    P.full_check(batch, backward=False)
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_cluster_configs_small(cfg):
+    w = W.workload(cfg, n_groups=4, group_size=8, n_tok=450)
+    batch = W.make_batch(w, seed=cfg, device=DEV)
+    batch["params"]["kernel"] = A.KERNEL_CLUSTER
+    P.full_check(batch)
+    P.full_check(batch, normalizer=A.NORM_PER_TRAJ)
+
+
+def test_cluster_matches_generic_bitwise_on_integers():
+    """Both row kernels give the same integers and the same zero pattern."""
+    w = W.workload(3, n_groups=6, group_size=4, n_tok=500, V=50_000)
+    batch = W.make_batch(w, seed=9, device=DEV, ld=50_000)
+    a = P.run_gpu(batch, kernel=A.KERNEL_CLUSTER)
+    b = P.run_gpu(batch, kernel=A.KERNEL_GENERIC)
+    assert torch.equal(a["tok_traj"], b["tok_traj"])
+    assert torch.equal(a["target_logit"], b["target_logit"])
+    assert int(a["clip_count"][0]) == int(b["clip_count"][0])
+    assert torch.equal(a["tok_coef"] == 0, b["tok_coef"] == 0)
+    assert float((a["token_lp"] - b["token_lp"]).abs().max()) < 2e-5
+
+
+@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER])
+def test_in_place(kernel):
+    """dlogits may alias logits exactly (include/awr.h)."""
+    w = W.workload(3, n_groups=4, group_size=4, n_tok=300, V=40_000)
+    batch = W.make_batch(w, seed=2, device=DEV)
+    batch["params"]["kernel"] = kernel
+    ref = P.run_gpu(batch)
+    z = batch["logits"].clone()
+    out = A.awr_loss_fwd_bwd(z, batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+                             batch["step_off"], batch["traj_off"], batch["group_off"],
+                             batch["rewards"], dlogits=z, **batch["params"])
+    torch.cuda.synchronize()
+    assert out["dlogits"].data_ptr() == z.data_ptr()
+    assert torch.equal(z, ref["dlogits"])
+    assert torch.equal(out["token_lp"], ref["token_lp"])
+    assert float(out["loss"][0]) == float(ref["loss"][0])
+
+
+def test_deterministic():
+    """Fixed-order reductions: two runs give identical bits."""
+    w = W.workload(2, n_groups=4, group_size=8, n_tok=600, V=151_936)
+    batch = W.make_batch(w, seed=4, device=DEV)
+    a = P.run_gpu(batch)
+    b = P.run_gpu(batch)
+    for k in a:
+        assert torch.equal(a[k], b[k]), k
+
+
+# ------------------------------------------------------------------ edge cases
+def test_empty_batch():
+    z = torch.empty(0, 1024, dtype=torch.bfloat16, device=DEV)
+    i32 = lambda x: torch.tensor(x, dtype=torch.int32, device=DEV)
+    f32 = lambda x: torch.tensor(x, dtype=torch.float32, device=DEV)
+    out = A.awr_loss_fwd_bwd(z, i32([]), f32([]), f32([]), i32([0]), i32([0]), i32([0]), f32([]))
+    torch.cuda.synchronize()
+    assert float(out["loss"][0]) == 0.0 and int(out["clip_count"][0]) == 0
+    assert int(out["err_word"][0]) == 0
+
+
+def test_empty_steps_trajectories_groups():
+    """A10: empty step counts toward |tau_i|; empty trajectory enters its group's statistics;
+    single-member and empty groups give A = 0."""
+    V = 2048
+    step_off = np.array([0, 3, 3, 10, 10, 10, 25, 40], dtype=np.int32)    # steps 1,3,4 empty
+    traj_off = np.array([0, 2, 2, 5, 6, 7], dtype=np.int32)               # traj 1 has no steps
+    group_off = np.array([0, 3, 3, 4, 5], dtype=np.int32)                 # group 1 empty, 2/3 single
+    rewards = np.array([1, 0, 0.5, 1, 0], dtype=np.float32)
+    g = torch.Generator(DEV).manual_seed(3)
+    n = 40
+    z = (torch.randn(n, V, generator=g, device=DEV) * 3).to(torch.bfloat16)
+    y = torch.randint(0, V, (n,), generator=g, device=DEV).to(torch.int32)
+    lp = torch.log_softmax(z.float(), 1)[torch.arange(n, device=DEV), y.long()]
+    q = lp + 0.1 * torch.randn(n, generator=g, device=DEV)
+    b = q + 0.1 * torch.randn(n, generator=g, device=DEV)
+    batch = dict(logits=z, target_ids=y, behave_lp=b, prox_lp=q, V=V, ld=V, n_tok=n,
+                 step_off=torch.from_numpy(step_off).to(DEV),
+                 traj_off=torch.from_numpy(traj_off).to(DEV),
+                 group_off=torch.from_numpy(group_off).to(DEV),
+                 rewards=torch.from_numpy(rewards).to(DEV),
+                 params=dict(k_norm=10.0, clip_eps=0.2, stale_cap=2.0, normalizer=A.NORM_PER_TRAJ,
+                             flags=0, loss_scale=0.5))
+    gpu, ora = P.full_check(batch)
+    assert ora["adv"][3] == 0 and ora["adv"][4] == 0
+    P.full_check(batch, normalizer=A.NORM_CONST_K)
+
+
+def test_error_word_bits():
+    w = W.workload(1, n_groups=2, group_size=4, n_tok=120, V=1024, dtype=torch.float32)
+    batch = W.make_batch(w, seed=1, device=DEV)
+    ids = batch["target_ids"].clone()
+    ids[7] = 1024
+    ids[9] = 5000
+    batch["target_ids"] = ids
+    gpu, ora = P.full_check(batch)
+    assert int(gpu["err_word"][0]) == A.ERRBIT_TARGET_RANGE
+    assert float(gpu["token_lp"][7]) == 0.0 and float(gpu["dlogits"][7].abs().max()) == 0.0
+    bad = batch["step_off"].clone()
+    bad[3] = bad[2] - 1
+    out = A.awr_loss_fwd(batch["logits"], ids, batch["behave_lp"], batch["prox_lp"], bad,
+                         batch["traj_off"], batch["group_off"], batch["rewards"])
+    torch.cuda.synchronize()
+    assert int(out["err_word"][0]) & A.ERRBIT_STEP_OFF
+    bad = batch["group_off"].clone()
+    bad[-1] += 1
+    out = A.awr_loss_fwd(batch["logits"], ids, batch["behave_lp"], batch["prox_lp"],
+                         batch["step_off"], batch["traj_off"], bad, batch["rewards"])
+    torch.cuda.synchronize()
+    assert int(out["err_word"][0]) & A.ERRBIT_GROUP_OFF
+
+
+def test_status_codes_on_device():
+    w = W.workload(1, n_groups=2, group_size=4, n_tok=64, V=1024, dtype=torch.float32)
+    batch = W.make_batch(w, seed=1, device=DEV)
+    args = (batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+            batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"])
+    with pytest.raises(A.AwrError) as e:
+        A.awr_loss_fwd_bwd(*args, clip_eps=1.5)
+    assert e.value.status == -5
+    with pytest.raises(A.AwrError) as e:
+        A.awr_loss_fwd_bwd(*args, workspace=torch.empty(256, dtype=torch.uint8, device=DEV))
+    assert e.value.status == -6
+    with pytest.raises(A.AwrError) as e:
+        A.awr_loss_fwd_bwd(*args, kernel=A.KERNEL_CLUSTER)      # fp32 / small V: unsupported
+    assert e.value.status == -5
+    with pytest.raises(A.AwrError) as e:
+        A.awr_loss_fwd_bwd(batch["logits"][:, 1:], *args[1:])  # rows not 16-byte aligned
+    assert e.value.status == -4
+
+
+def test_group_advantage_kernel():
+    rng = np.random.default_rng(0)
+    sizes = [8, 1, 0, 33, 64, 100, 2, 16]
+    off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int32)
+    R = rng.normal(size=off[-1]).astype(np.float32)
+    R[off[4]:off[5]] = 0.25                                     # an all-equal group
+    for flags in (0, A.FLAG_SAMPLE_STD):
+        adv = A.awr_group_advantage(torch.from_numpy(R).to(DEV), torch.from_numpy(off).to(DEV),
+                                    flags=flags).cpu().numpy()
+        ref = O.group_advantage(R, off, flags)
+        np.testing.assert_allclose(adv, ref, rtol=0, atol=5e-6)
+        assert np.all(adv[off[4]:off[5]] == 0) and adv[off[1]] == 0
+
+
+def test_graph_capture():
+    """The call only enqueues work: it can be captured into a CUDA graph and replayed."""
+    w = W.workload(1, n_groups=2, group_size=4, n_tok=200, V=40_000)
+    batch = W.make_batch(w, seed=6, device=DEV)
+    call = A.LossCall(batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+                      batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"],
+                      **batch["params"])
+    ref = {k: v.clone() for k, v in call.run().items()}
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            call.run(stream=s)
+    for v in call.out.values():
+        v.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    for k in ref:
+        assert torch.equal(ref[k], call.out[k]), k
