@@ -7,7 +7,7 @@ import torch
 import paper_2606_05597_b200 as A
 from gen import workloads as W
 from oracle import awr_oracle as O
-from tests import parity_util as P
+import parity_util as P
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda:0"
