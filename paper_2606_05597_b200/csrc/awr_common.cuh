@@ -58,20 +58,33 @@ struct RowHeader {
 
 struct TokenScalars {
     float lp;    // l_t
+    float lse;   // log-sum-exp of the whole row (= zy - l_t for a valid token)
     float term;  // contribution to J
     float coef;  // c_t
+    float gy;    // c_t (p_y - 1): the target entry of the gradient row
     bool trig;
 };
 
 // a3: ratio, clip, normalizer (Eq. 1), fp32.
-__device__ __forceinline__ TokenScalars token_scalars(const RowHeader& h, float lse, bool valid,
-                                                      float clip_eps, float stale_cap) {
+//
+// lse_rest is the log-sum-exp of the row WITHOUT its target entry (of the whole row when the
+// token is not valid).  With d = lse_rest - z_y:  l_t = -softplus(d),  1 - p_y = sigmoid(d).
+// Both stay accurate to f32 rounding when p_y -> 1, where z_y - lse and exp(l_t) - 1 cancel
+// (DESIGN.md "Numerics").
+__device__ __forceinline__ TokenScalars token_scalars(const RowHeader& h, float lse_rest,
+                                                      bool valid, float clip_eps,
+                                                      float stale_cap) {
     TokenScalars t;
     if (!valid) {
-        t.lp = 0.f; t.term = 0.f; t.coef = 0.f; t.trig = false;
+        t.lp = 0.f; t.lse = lse_rest; t.term = 0.f; t.coef = 0.f; t.gy = 0.f; t.trig = false;
         return t;
     }
-    t.lp = h.zy - lse;
+    const float d = lse_rest - h.zy;                  // -inf if the row has no other entry
+    const float e = expf(-fabsf(d));                  // in [0, 1]
+    const float sp = fmaxf(d, 0.f) + log1pf(e);       // softplus(d) = -l_t
+    const float one_minus_p = (d >= 0.f ? 1.0f : e) / (1.0f + e);   // sigmoid(d) = 1 - p_y
+    t.lp = -sp;
+    t.lse = h.zy + sp;
     float r = expf(t.lp - h.q);                       // pi_theta / pi_prox
     float w = expf(h.q - h.b);                        // pi_prox / pi_behave (staleness weight)
     if (stale_cap > 0.f && stale_cap < INFINITY) w = fminf(w, stale_cap);
@@ -81,6 +94,7 @@ __device__ __forceinline__ TokenScalars token_scalars(const RowHeader& h, float 
     float sw = h.scale * w;
     t.term = sw * fminf(u, v);
     t.coef = t.trig ? 0.f : sw * u;
+    t.gy = -t.coef * one_minus_p;
     return t;
 }
 

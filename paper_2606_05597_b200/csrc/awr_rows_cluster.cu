@@ -197,6 +197,7 @@ rows_cluster_kernel(RowArgs a, ClusterPlan p) {
     refill();                 // prologue: sequence numbers 0 .. S-1 fill the ring
 
     int par = 0;
+    int y_next = cluster < a.n_tok ? a.target_ids[cluster] : -1;
     for (int64_t row = cluster; row < a.n_tok; row += p.num_clusters, par ^= 1) {
         // ---- row header (one thread per CTA; both CTAs load the same values)
         if (tid == 0) {
@@ -205,6 +206,18 @@ rows_cluster_kernel(RowArgs a, ClusterPlan p) {
             ctrl->hdr[par] = h;
             ctrl->hdr_valid[par] = valid ? 1 : 0;
         }
+        // The target entry is left out of the (max, sum) state (token_scalars works from
+        // lse_rest).  Every thread knows its position; the next row's id is fetched now so
+        // that its latency hides behind this row.  A masked / out-of-range id matches no unit.
+        const int y_row = y_next;
+        {
+            const int64_t nrow = row + p.num_clusters;
+            y_next = nrow < a.n_tok ? a.target_ids[nrow] : -1;
+        }
+        const int y_unit1 = (y_row >> 3) - part0;            // unit index inside this part
+        const uint32_t y_word = (uint32_t)(y_row & 7) >> 1;
+        const uint32_t y_keep = (y_row & 1) ? 0x0000ffffu : 0xffff0000u;
+        const uint32_t y_ninf = 0xff80ff80u & ~y_keep;       // bf16 -inf in the target's half
 
         // ---- pass 1 (a2): online (max, sum) over this warp's part, as the chunks land
         MaxSum ms{-INFINITY, 0.f};
@@ -227,6 +240,17 @@ rows_cluster_kernel(RowArgs a, ClusterPlan p) {
                 int pos = start_unit + u; if (pos >= ring_units) pos -= ring_units;
                 v[k] = ok[k] ? lds128(ring + (uint32_t)pos * 16u)
                              : make_uint4(0xff80ff80u, 0xff80ff80u, 0xff80ff80u, 0xff80ff80u);
+            }
+            if (y_unit1 >= ubase && y_unit1 < uend) {          // warp-uniform, once per row
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    if (ubase + k * 32 + lane == y_unit1) {
+                        v[k].x = y_word == 0 ? (v[k].x & y_keep) | y_ninf : v[k].x;
+                        v[k].y = y_word == 1 ? (v[k].y & y_keep) | y_ninf : v[k].y;
+                        v[k].z = y_word == 2 ? (v[k].z & y_keep) | y_ninf : v[k].z;
+                        v[k].w = y_word == 3 ? (v[k].w & y_keep) | y_ninf : v[k].w;
+                    }
+                }
             }
             // packed running max of the round (bf16x2), then one rescale check
             uint32_t m2 = max_bf16x2(max_bf16x2(v[0].x, v[0].y), max_bf16x2(v[0].z, v[0].w));
@@ -282,12 +306,13 @@ rows_cluster_kernel(RowArgs a, ClusterPlan p) {
         cluster_arrive();
         cluster_wait();
         const MaxSum tot = combine(ctrl->stats[par][0], ctrl->stats[par][1]);
-        const float lse = tot.m + logf(tot.s);
+        const float lse_rest = tot.m + logf(tot.s);          // -inf if nothing but the target
         const RowHeader h = ctrl->hdr[par];
         const bool valid = ctrl->hdr_valid[par] != 0;
 
         // ---- a3: per-token scalars (every thread, identical arithmetic)
-        const TokenScalars ts = token_scalars(h, lse, valid, a.clip_eps, a.stale_cap);
+        const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap);
+        const float lse = ts.lse;
         if (tid == 0 && rank == 0) store_token_outputs(a, row, h, ts, valid);
 
         // ---- pass 2 (a4)
@@ -314,9 +339,8 @@ rows_cluster_kernel(RowArgs a, ClusterPlan p) {
             const bool neg = ts.coef < 0.f;
             const uint32_t sign = neg ? 0x80008000u : 0u;
             // target entry: c (p_y - 1); patched by the lane that owns its 16-byte unit
-            const int y_unit = (h.y >> 3) - part0;           // unit index inside this part
-            const uint16_t gy_bits =
-                __bfloat16_as_ushort(__float2bfloat16_rn(ts.coef * (expf(ts.lp) - 1.0f)));
+            const int y_unit = y_unit1;
+            const uint16_t gy_bits = __bfloat16_as_ushort(__float2bfloat16_rn(ts.gy));
             int stored = 0;   // chunks of this row already handed to the TMA store
             for (int ubase = 0; ubase < part_units; ubase += kRound) {
                 const int uend = min(ubase + kRound, part_units);

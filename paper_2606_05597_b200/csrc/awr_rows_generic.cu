@@ -62,6 +62,11 @@ rows_generic_kernel(RowArgs a) {
         RowHeader h;
         bool valid = false;
         if (tid == 0) h = load_row_header(a, row, valid, sizeof(T) == 2);
+        // every thread knows the target column: it is left out of the (max, sum) state, so
+        // that l_t and 1 - p_y come from lse_rest without cancellation (token_scalars)
+        const int yt = a.target_ids[row];
+        const int64_t ycol = (yt >= 0 && yt < a.V) ? (int64_t)yt : (int64_t)-1;
+        const int64_t yvec = ycol >= 0 ? ycol / EPV : (int64_t)-1;
 
         // ---- a2: one streaming pass, per-thread online (max, sum)
         MaxSum ms{-INFINITY, 0.f};
@@ -70,6 +75,11 @@ rows_generic_kernel(RowArgs a) {
             uint4 v = zv[i];
             float x[EPV];
             E::unpack(v, x);
+            if (i == yvec) {
+                const int yk = (int)(ycol - i * EPV);
+#pragma unroll
+                for (int k = 0; k < EPV; ++k) x[k] = (k == yk) ? -INFINITY : x[k];
+            }
             float cm = x[0];
 #pragma unroll
             for (int k = 1; k < EPV; ++k) cm = fmaxf(cm, x[k]);
@@ -84,7 +94,7 @@ rows_generic_kernel(RowArgs a) {
             ms.s += acc;
         }
         for (int64_t i = tail0 + tid; i < a.V; i += kGenericThreads) {
-            float x = E::load(z + i);
+            float x = (i == ycol) ? -INFINITY : E::load(z + i);
             if (x > ms.m) {
                 ms.s *= ex2_approx((ms.m - x) * kLog2e);
                 ms.m = x;
@@ -98,14 +108,14 @@ rows_generic_kernel(RowArgs a) {
             MaxSum tot = s_red[0];
 #pragma unroll
             for (int w = 1; w < kGenericThreads / 32; ++w) tot = combine(tot, s_red[w]);
-            float lse = tot.m + logf(tot.s);
+            float lse_rest = tot.m + logf(tot.s);   // -inf when the row has no other entry
             // ---- a3
-            TokenScalars ts = token_scalars(h, lse, valid, a.clip_eps, a.stale_cap);
+            TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap);
             store_token_outputs(a, row, h, ts, valid);
             s_coef = ts.coef;
-            s_lse = lse;
+            s_lse = ts.lse;
             s_y = valid ? h.y : -1;
-            s_gy = ts.coef * (expf(ts.lp) - 1.0f);   // c_t (p_y - 1)
+            s_gy = ts.gy;                           // c_t (p_y - 1)
         }
         __syncthreads();
 
