@@ -216,12 +216,10 @@ class HostLossCall:
         self.device = torch.device(device)
         n_tok, n_traj = self.batch.n_tok, self.batch.n_traj
         self.out = alloc_outputs(n_tok, n_traj, "cpu", None, want)
+        if pin:                           # small arrays: a pinned copy is cheap
+            self.out = {k: v.pin_memory() for k, v in self.out.items()}
         self.out["dlogits"] = dlogits if dlogits is not None else torch.empty_strided(
-            logits.shape, logits.stride(), dtype=logits.dtype)
-        if pin:
-            for k, v in list(self.out.items()):
-                if not v.is_pinned():
-                    self.out[k] = v.pin_memory()
+            logits.shape, logits.stride(), dtype=logits.dtype, pin_memory=pin)
         self.outs = _out_struct(self.out)
         need = host_workspace_bytes(n_tok, self.batch.V, self.batch.ld, logits.dtype,
                                     self.batch.n_steps, n_traj, self.batch.n_groups)
