@@ -73,7 +73,9 @@ enum { AWR_FLAG_SAMPLE_STD = 1u /* A2: std with 1/(G-1) instead of the default 1
 enum { AWR_W_K_BY_V = 0 /* w_head[k * V + v] */, AWR_W_V_BY_K = 1 /* w_head[v * K + k] */ };
 enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_GENERIC = 1,  /* one CTA per row, second pass re-reads the row through L2 */
-       AWR_KERNEL_CLUSTER = 2   /* row resident in the shared memory of a 2-CTA cluster (bf16) */ };
+       AWR_KERNEL_CLUSTER = 2,  /* row resident in the shared memory of a 2-CTA cluster (bf16) */
+       AWR_KERNEL_CLUSTER_RF = 3 /* row resident in the register files of a 2-CTA cluster (bf16,
+                                    16K <= V <= 163,840); shared memory is a TMA load FIFO */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u };
 
@@ -199,7 +201,7 @@ AWR_API const char* awr_status_string(int status);
 AWR_API int awr_version(void);
 
 /* Introspection for benchmarks and tests: which row kernel AWR_KERNEL_AUTO resolves to for
- * this shape (AWR_KERNEL_GENERIC or AWR_KERNEL_CLUSTER), and the number of kernel launches one
+ * this shape (AWR_KERNEL_GENERIC, AWR_KERNEL_CLUSTER or AWR_KERNEL_CLUSTER_RF), and the number of kernel launches one
  * awr_loss_fwd_bwd call enqueues. */
 AWR_API int awr_select_kernel(int64_t V, int64_t ld, int32_t logits_dtype);
 AWR_API int awr_launches_per_call(void);

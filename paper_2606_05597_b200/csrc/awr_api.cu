@@ -66,7 +66,7 @@ static int check_params(const awr_params* p) {
     if (p->dual_clip_c > 1.f) return AWR_ERR_PARAM;          // Eq. (2) reserved
     if (p->normalizer != AWR_NORM_CONST_K && p->normalizer != AWR_NORM_PER_TRAJ) return AWR_ERR_PARAM;
     if (p->flags & ~(uint32_t)AWR_FLAG_SAMPLE_STD) return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER_RF) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -78,10 +78,21 @@ static int check_segments(int64_t n_tok, int32_t n_steps, int32_t n_traj, int32_
 
 static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype) {
     const bool ok = rows_cluster_supported(V, ld, dtype);
+    const bool ok_rf = rows_rf_supported(V, ld, dtype);
     if (requested == AWR_KERNEL_CLUSTER) return ok ? AWR_KERNEL_CLUSTER : -1;
+    if (requested == AWR_KERNEL_CLUSTER_RF) return ok_rf ? AWR_KERNEL_CLUSTER_RF : -1;
     if (requested == AWR_KERNEL_GENERIC) return AWR_KERNEL_GENERIC;
-    // auto: the cluster kernel pays off once a row is a sizeable fraction of shared memory
-    return (ok && V * 2 >= 65536) ? AWR_KERNEL_CLUSTER : AWR_KERNEL_GENERIC;
+    // auto: the cluster kernels pay off once a row is a sizeable fraction of shared memory
+    if (V * 2 < 65536) return AWR_KERNEL_GENERIC;
+    if (ok_rf) return AWR_KERNEL_CLUSTER_RF;
+    return ok ? AWR_KERNEL_CLUSTER : AWR_KERNEL_GENERIC;
+}
+
+static cudaError_t launch_rows(int kernel, const RowArgs& a, int dtype, int num_sms,
+                               cudaStream_t st) {
+    if (kernel == AWR_KERNEL_CLUSTER_RF) return launch_rows_rf(a, num_sms, st);
+    if (kernel == AWR_KERNEL_CLUSTER) return launch_rows_cluster(a, num_sms, st);
+    return launch_rows_generic(a, dtype, num_sms, st);
 }
 
 static cudaEvent_t g_prof_before = nullptr, g_prof_after = nullptr;
@@ -145,8 +156,7 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     g_prof_before = g_prof_after = nullptr;
     if (e == cudaSuccess && ev0) e = cudaEventRecord(ev0, st);
     if (e == cudaSuccess) {
-        e = kernel == AWR_KERNEL_CLUSTER ? launch_rows_cluster(a, info.num_sms, st)
-                                         : launch_rows_generic(a, b->logits_dtype, info.num_sms, st);
+        e = launch_rows(kernel, a, b->logits_dtype, info.num_sms, st);
     }
     if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, st);
     // a3 final reduction
@@ -374,8 +384,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
         a.token_lp = d_lp + r0; a.tok_term = d_term + r0; a.tok_coef = d_coef + r0;
         a.target_logit = d_tl + r0; a.tok_flag = w.tok_flag + r0; a.err_word = d_err;
         a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap;
-        AWR_TRY(kernel == AWR_KERNEL_CLUSTER ? launch_rows_cluster(a, info.num_sms, s_k)
-                                             : launch_rows_generic(a, hb->logits_dtype, info.num_sms, s_k));
+        AWR_TRY(launch_rows(kernel, a, hb->logits_dtype, info.num_sms, s_k));
         AWR_TRY(cudaEventRecord(ev_k[bi], s_k));
         AWR_TRY(cudaStreamWaitEvent(s_out, ev_k[bi], 0));
         AWR_TRY(cudaMemcpyAsync((uint8_t*)ho->dlogits + (size_t)r0 * row_bytes, buf,

@@ -1,0 +1,388 @@
+// Register-file row kernel: a2 + a3 + a4 for bf16 vocabularies of 16K..163K entries with one HBM
+// read and one HBM write per element.  PAPER.md:57 (Eq. 1), :435; gradient SURVEY.md 8(c) O8.
+//
+// Design:
+//   * A 151,936-entry bf16 row (303,872 B) fits neither one SM's shared memory (227 KB) nor one
+//     SM's register file (256 KB) next to the staging it needs, so a row is split across a
+//     2-CTA thread-block cluster and each half (148 KB) lives in the REGISTER FILE of its SM:
+//     16 warps x 32 lanes x up to 20 packed 16-byte units per lane.
+//   * Shared memory is a pure FIFO between HBM and the registers: every warp owns a ring of
+//     2 KB slots that TMA bulk copies (cp.async.bulk + mbarrier complete_tx) fill with its part
+//     of the rows to come; a slot is refilled the moment the warp has moved it into registers,
+//     so up to 224 KB of loads per SM are in flight while the current row is being worked on.
+//   * Pass 0 moves the warp's part to registers and takes its max with packed bf16x2 max.
+//     Pass 1 replaces every logit, in registers, by e = exp2((z - m_w) log2 e) rounded to bf16
+//     and sums the unrounded values in f32.  The 32 warps of the cluster exchange (m_w, s_w)
+//     through distributed shared memory, one cluster barrier per row.  Pass 2 is then a packed
+//     multiply: dlogits = e * (c_t exp(m_w - lse)), two bf16x2 instructions per pair (the factor
+//     is split hi + lo so that it carries 16 significant bits), written with 16-byte coalesced
+//     global stores straight from registers.  One MUFU and ~8 issue slots per element in total.
+//   * Persistent: one cluster per SM pair, rows dealt round-robin to clusters (static schedule,
+//     deterministic results).  Rows with c_t = 0 (masked, zero advantage, clip triggered) skip
+//     pass 2 and are written as zeros.
+#include "awr_common.cuh"
+#include "awr_kernels.h"
+
+namespace awr {
+
+constexpr int kRfWarps = 16;
+constexpr int kRfThreads = kRfWarps * 32;
+constexpr int kRfSlots = 7;                 // ring slots per warp
+constexpr int kRfChunkRounds = 4;           // rounds (32 units each) per slot / per TMA copy
+constexpr int kRfChunkUnits = 32 * kRfChunkRounds;
+constexpr int kRfSlotBytes = kRfChunkUnits * 16;
+constexpr int kRfCtrlBytes = 2048;
+constexpr int kRfSmemBytes = kRfCtrlBytes + kRfWarps * kRfSlots * kRfSlotBytes;   // 231,424
+constexpr int kRfMinNU = 3, kRfMaxNU = 20;
+constexpr uint32_t kNegInf2 = 0xff80ff80u;  // bf16x2 (-inf, -inf)
+
+struct RfPlan {
+    int units_per_row;   // 16-byte units in one row (V / 8)
+    int num_clusters;
+};
+
+struct RfCtrl {
+    uint64_t full[kRfWarps * 8];   // one mbarrier per ring slot per warp (8 >= kRfSlots)
+    float2 stats[2][32];           // [row parity][part] (max, sum) of every warp of the cluster
+};
+static_assert(sizeof(RfCtrl) <= kRfCtrlBytes, "control block");
+static_assert(kRfSmemBytes <= 232448, "227 KB of dynamic shared memory per CTA on sm_100");
+
+namespace rf {
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes,
+                                          uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void cluster_arrive() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_wait() {
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t cluster_id_x() {
+    uint32_t r;
+    asm("mov.u32 %0, %%clusterid.x;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_f32x2(uint32_t local_addr, uint32_t rank, float a,
+                                                 float b) {
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(rank));
+    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(remote), "f"(a), "f"(b)
+                 : "memory");
+}
+__device__ __forceinline__ void lds128(uint32_t (&v)[4], uint32_t addr) {
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
+                 : "r"(addr));
+}
+__device__ __forceinline__ void stg128(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(a), "r"(b), "r"(c),
+                 "r"(d)
+                 : "memory");
+}
+__device__ __forceinline__ uint32_t mul_bf16x2(uint32_t a, uint32_t b) {
+    uint32_t r;
+    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+    return r;
+}
+__device__ __forceinline__ uint32_t fma_bf16x2(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+}  // namespace rf
+
+// ---------------------------------------------------------------- the kernel
+// NU = rounds per warp part = ceil(max part units / 32); every round but the last is full for
+// every warp (parts differ by at most one unit and NU is exact, see make_rf_plan).
+template <int NU>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kRfThreads, 1)
+rows_rf_kernel(RowArgs a, RfPlan p) {
+    using namespace rf;
+    constexpr int NCH = (NU + kRfChunkRounds - 1) / kRfChunkRounds;
+    extern __shared__ __align__(128) uint8_t smem[];
+    RfCtrl* ctrl = reinterpret_cast<RfCtrl*>(smem);
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int warp = tid >> 5;
+    const uint32_t rank = cluster_ctarank();
+    const int cluster = (int)cluster_id_x();
+    const uint32_t ring = smem_u32(smem + kRfCtrlBytes) + (uint32_t)warp * (kRfSlots * kRfSlotBytes);
+    const uint32_t bar0 = smem_u32(&ctrl->full[warp * 8]);
+
+    // this warp's part of the row, in 16-byte units: [part0, part0 + part_units)
+    const int part_idx = (int)rank * kRfWarps + warp;
+    constexpr int nparts = 2 * kRfWarps;
+    const int part0 = (int)(((int64_t)p.units_per_row * part_idx) / nparts);
+    const int part_units = (int)(((int64_t)p.units_per_row * (part_idx + 1)) / nparts) - part0;
+    const int nch = (part_units + kRfChunkUnits - 1) / kRfChunkUnits;     // <= NCH
+
+    const int my_rows = (int)((a.n_tok - cluster + p.num_clusters - 1) / p.num_clusters);
+    const int total_seq = my_rows * nch;
+    const bool backward = a.dlogits != nullptr;
+    const uint8_t* lbase = reinterpret_cast<const uint8_t*>(a.logits) + (int64_t)part0 * 16;
+    uint8_t* gbase = reinterpret_cast<uint8_t*>(a.dlogits) + (int64_t)part0 * 16 + lane * 16;
+    const int64_t row_bytes = a.ld * 2;
+
+    if (lane == 0)
+        for (int s = 0; s < kRfSlots; ++s) mbar_init(bar0 + 8u * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+    cluster_arrive();     // both CTAs are resident before any distributed-shared-memory store
+    cluster_wait();
+
+    // ---- TMA producer state (warp-uniform; lane 0 issues)
+    int ld_seq = 0, ld_ch = 0, ld_slot = 0;
+    int64_t ld_row = cluster;
+    int cons_seq = 0, cons_slot = 0;
+    uint32_t cons_phase = 0;
+    auto refill = [&]() {
+        while (ld_seq < total_seq && ld_seq < cons_seq + kRfSlots) {
+            if (lane == 0) {
+                const int u0 = ld_ch * kRfChunkUnits;
+                const uint32_t bytes = (uint32_t)min(kRfChunkUnits, part_units - u0) * 16u;
+                const uint32_t bar = bar0 + 8u * ld_slot;
+                mbar_expect_tx(bar, bytes);
+                bulk_load(ring + (uint32_t)ld_slot * kRfSlotBytes,
+                          lbase + ld_row * row_bytes + (int64_t)u0 * 16, bytes, bar);
+            }
+            ++ld_seq;
+            if (++ld_ch == nch) { ld_ch = 0; ld_row += p.num_clusters; }
+            if (++ld_slot == kRfSlots) ld_slot = 0;
+        }
+    };
+    refill();
+
+    int y_next = -1, traj_next = -1;
+    if (cluster < a.n_tok) { y_next = a.target_ids[cluster]; traj_next = a.tok_traj[cluster]; }
+    int par = 0;
+    for (int64_t row = cluster; row < a.n_tok; row += p.num_clusters, par ^= 1) {
+        // ---- row header: every thread loads the same words (one sector each); the values are
+        // not needed before the cluster barrier, so their latency hides behind passes 0 and 1
+        RowHeader h;
+        h.y = y_next;
+        const int traj = traj_next;
+        {
+            const int64_t nrow = row + p.num_clusters;
+            if (nrow < a.n_tok) { y_next = a.target_ids[nrow]; traj_next = a.tok_traj[nrow]; }
+        }
+        const bool valid = (h.y >= 0) && (h.y < a.V);
+        h.q = a.prox_lp[row];
+        h.b = a.behave_lp[row];
+        h.A = traj >= 0 ? a.adv[traj] : 0.f;
+        h.scale = traj >= 0 ? a.traj_scale[traj] : 0.f;
+        h.zy = valid ? __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(a.logits)[row * a.ld + h.y])
+                     : 0.f;
+        // The target entry is left out of the (max, sum) state (token_scalars works from
+        // lse_rest): the warp whose part holds it masks it to -inf on the way to registers.
+        const int y_unit = valid ? (h.y >> 3) - part0 : -1;
+        const bool owner = (y_unit >= 0) && (y_unit < part_units);        // warp-uniform
+        const int y_word = (h.y & 7) >> 1;
+        const uint32_t y_keep = (h.y & 1) ? 0x0000ffffu : 0xffff0000u;     // the OTHER half
+
+        // ---- pass 0: ring -> registers, packed running max
+        uint32_t v[NU][4];
+        uint32_t mx2 = kNegInf2;
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            const bool have = c < nch;                                    // warp-uniform
+            if (have) mbar_wait(bar0 + 8u * cons_slot, cons_phase);
+            const uint32_t src = ring + (uint32_t)cons_slot * kRfSlotBytes + (uint32_t)lane * 16u;
+#pragma unroll
+            for (int kk = 0; kk < kRfChunkRounds; ++kk) {
+                const int k = c * kRfChunkRounds + kk;
+                if (k < NU) {
+                    if (k < NU - 1 || k * 32 + lane < part_units) {
+                        lds128(v[k], src + kk * (32 * 16));
+                    } else {
+                        v[k][0] = v[k][1] = v[k][2] = v[k][3] = kNegInf2;
+                    }
+                    if (owner && k * 32 + lane == y_unit) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            v[k][j] = (j == y_word) ? ((v[k][j] & y_keep) | (kNegInf2 & ~y_keep))
+                                                    : v[k][j];
+                    }
+                    mx2 = max_bf16x2(mx2, max_bf16x2(max_bf16x2(v[k][0], v[k][1]),
+                                                     max_bf16x2(v[k][2], v[k][3])));
+                }
+            }
+            if (have) {
+                // the max above consumed the loaded registers: the slot has been read out
+                ++cons_seq;
+                if (++cons_slot == kRfSlots) { cons_slot = 0; cons_phase ^= 1u; }
+                __syncwarp();
+                refill();
+            }
+        }
+        float m = fmaxf(bf16_lo(mx2), bf16_hi(mx2));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(kFull, m, o));
+
+        // ---- pass 1: z -> e = exp2((z - m) log2 e) as bf16, in registers; f32 sum
+        const float nref = (m == -INFINITY) ? 0.f : -m * kLog2e;
+        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int k = 0; k < NU; ++k) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float e0 = ex2_approx(fmaf(bf16_lo(v[k][j]), kLog2e, nref));
+                const float e1 = ex2_approx(fmaf(bf16_hi(v[k][j]), kLog2e, nref));
+                acc[j] += e0;
+                acc[j] += e1;
+                v[k][j] = pack_bf16x2(e0, e1);
+            }
+        }
+        float s = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(kFull, s, o);
+
+        // ---- exchange: every warp of the cluster publishes (m_w, s_w) to both CTAs
+        if (lane == 0) {
+            const uint32_t addr = smem_u32(&ctrl->stats[par][part_idx]);
+            st_cluster_f32x2(addr, 0, m, s);
+            st_cluster_f32x2(addr, 1, m, s);
+        }
+        __syncwarp();
+        cluster_arrive();
+        cluster_wait();
+        const float2 st = ctrl->stats[par][lane];
+        float M = st.x;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(kFull, M, o));
+        float S = (M == -INFINITY) ? 0.f : st.y * ex2_approx((st.x - M) * kLog2e);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) S += __shfl_xor_sync(kFull, S, o);
+        const float lse_rest = M + logf(S);                   // -inf if nothing but the target
+
+        // ---- a3: per-token scalars (every thread, identical arithmetic)
+        const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap);
+        if (tid == 0 && rank == 0) {
+            if (h.y >= a.V) atomicOr(a.err_word, AWR_ERRBIT_TARGET_RANGE);
+            store_token_outputs(a, row, h, ts, valid);
+        }
+
+        // ---- pass 2 (a4): dlogits = e * (c_t exp(m - lse)), straight from registers
+        if (backward) {
+            uint8_t* g = gbase + row * row_bytes;
+            if (ts.coef == 0.f) {
+#pragma unroll
+                for (int k = 0; k < NU; ++k)
+                    if (k < NU - 1 || k * 32 + lane < part_units)
+                        stg128(g + k * (32 * 16), 0u, 0u, 0u, 0u);
+            } else {
+                // e was taken relative to m (0 if the part held nothing finite)
+                const float F = ts.coef * ex2_approx(fmaf(-ts.lse, kLog2e, -nref));
+                const __nv_bfloat16 fh = __float2bfloat16_rn(F);
+                const __nv_bfloat16 fl = __float2bfloat16_rn(F - __bfloat162float(fh));
+                const uint32_t Fh = (uint32_t)__bfloat16_as_ushort(fh) * 0x00010001u;
+                const uint32_t Fl = (uint32_t)__bfloat16_as_ushort(fl) * 0x00010001u;
+                const uint32_t gy_bits = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(ts.gy));
+                const uint32_t gy2 = (h.y & 1) ? (gy_bits << 16) : gy_bits;
+#pragma unroll
+                for (int k = 0; k < NU; ++k) {
+                    uint32_t o[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) o[j] = fma_bf16x2(v[k][j], Fh, mul_bf16x2(v[k][j], Fl));
+                    if (owner && k * 32 + lane == y_unit) {     // target entry: c (p_y - 1)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            o[j] = (j == y_word) ? ((o[j] & y_keep) | gy2) : o[j];
+                    }
+                    if (k < NU - 1 || k * 32 + lane < part_units)
+                        stg128(g + k * (32 * 16), o[0], o[1], o[2], o[3]);
+                }
+            }
+        }
+    }
+    cluster_arrive();
+    cluster_wait();
+}
+
+// ---------------------------------------------------------------- host side
+static bool make_rf_plan(int64_t V, int64_t ld, int dtype, int num_sms, int64_t n_tok, RfPlan& p,
+                         int& nu) {
+    if (dtype != AWR_DTYPE_BF16) return false;
+    if (V % 8 != 0 || ld % 8 != 0) return false;
+    const int64_t units = V / 8;
+    const int nparts = 2 * kRfWarps;
+    const int64_t part_max = (units + nparts - 1) / nparts;
+    const int64_t n = (part_max + 31) / 32;
+    if (n < kRfMinNU || n > kRfMaxNU) return false;
+    p.units_per_row = (int)units;
+    int nc = num_sms / 2;
+    if ((int64_t)nc > n_tok) nc = (int)n_tok;
+    if (nc < 1) nc = 1;
+    p.num_clusters = nc;
+    nu = (int)n;
+    return true;
+}
+
+bool rows_rf_supported(int64_t V, int64_t ld, int dtype) {
+    RfPlan p;
+    int nu;
+    return make_rf_plan(V, ld, dtype, 148, 1 << 20, p, nu);
+}
+
+template <int NU>
+static cudaError_t launch_nu(const RowArgs& a, const RfPlan& p, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(rows_rf_kernel<NU>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             kRfSmemBytes);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    rows_rf_kernel<NU><<<2 * p.num_clusters, kRfThreads, kRfSmemBytes, st>>>(a, p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, cudaStream_t st) {
+    if (a.n_tok <= 0) return cudaSuccess;
+    RfPlan p;
+    int nu = 0;
+    if (!make_rf_plan(a.V, a.ld, AWR_DTYPE_BF16, num_sms, a.n_tok, p, nu)) return cudaErrorInvalidValue;
+    switch (nu) {
+#define AWR_RF_CASE(N) case N: return launch_nu<N>(a, p, st);
+        AWR_RF_CASE(3) AWR_RF_CASE(4) AWR_RF_CASE(5) AWR_RF_CASE(6) AWR_RF_CASE(7) AWR_RF_CASE(8)
+        AWR_RF_CASE(9) AWR_RF_CASE(10) AWR_RF_CASE(11) AWR_RF_CASE(12) AWR_RF_CASE(13)
+        AWR_RF_CASE(14) AWR_RF_CASE(15) AWR_RF_CASE(16) AWR_RF_CASE(17) AWR_RF_CASE(18)
+        AWR_RF_CASE(19) AWR_RF_CASE(20)
+#undef AWR_RF_CASE
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace awr

@@ -88,7 +88,7 @@ def test_host_side_status_codes():
     assert lib.awr_status_string(_abi.AWR_ERR_ARCH).decode().startswith("device is not sm_100")
     assert lib.awr_workspace_bytes(1000, 151936, 10, 8, 2) % 256 == 0
     assert lib.awr_workspace_bytes(-1, 1, 1, 1, 1) == 0
-    assert lib.awr_select_kernel(151936, 151936, 0) == _abi.KERNEL_CLUSTER
+    assert lib.awr_select_kernel(151936, 151936, 0) in (_abi.KERNEL_CLUSTER, _abi.KERNEL_CLUSTER_RF)
     assert lib.awr_select_kernel(151936, 151936, 1) == _abi.KERNEL_GENERIC
     assert lib.awr_select_kernel(1024, 1024, 0) == _abi.KERNEL_GENERIC
 

@@ -72,33 +72,40 @@ CLUSTER_SHAPES = [(151_936, 151_936), (40_000, 40_008), (32_768, 32_768), (65_54
                   (131_072, 131_072)]
 
 
+CLUSTER_KERNELS = [A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF]
+
+
+@pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
 @pytest.mark.parametrize("V,ld", CLUSTER_SHAPES)
-def test_cluster_vs_oracle(V, ld):
-    """bf16 rows resident in the shared memory of a 2-CTA cluster; 300+ rows = several rows
-    per cluster plus a ragged tail; masked tokens, zero-advantage groups, clip triggers."""
-    assert A.select_kernel(V, ld, torch.bfloat16) == A.KERNEL_CLUSTER
+def test_cluster_vs_oracle(V, ld, kernel):
+    """bf16 rows resident in the shared memory (CLUSTER) or the register files (CLUSTER_RF) of a
+    2-CTA cluster; 300+ rows = several rows per cluster plus a ragged tail; masked tokens,
+    zero-advantage groups, clip triggers."""
+    assert A.select_kernel(V, ld, torch.bfloat16) in CLUSTER_KERNELS
     w = W.workload(3, n_groups=6, group_size=4, n_tok=331, V=V)
     batch = W.make_batch(w, seed=5, device=DEV, ld=ld, masked_frac=0.04)
-    batch["params"]["kernel"] = A.KERNEL_CLUSTER
+    batch["params"]["kernel"] = kernel
     gpu, ora = P.full_check(batch)
     assert ora["clip_count"] > 0 and (ora["coef"] == 0).sum() > ora["clip_count"]
     P.full_check(batch, backward=False)
 
 
+@pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
 @pytest.mark.parametrize("cfg", [1, 2])
-def test_cluster_configs_small(cfg):
+def test_cluster_configs_small(cfg, kernel):
     w = W.workload(cfg, n_groups=4, group_size=8, n_tok=450)
     batch = W.make_batch(w, seed=cfg, device=DEV)
-    batch["params"]["kernel"] = A.KERNEL_CLUSTER
+    batch["params"]["kernel"] = kernel
     P.full_check(batch)
     P.full_check(batch, normalizer=A.NORM_PER_TRAJ)
 
 
-def test_cluster_matches_generic_bitwise_on_integers():
-    """Both row kernels give the same integers and the same zero pattern."""
+@pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
+def test_cluster_matches_generic_bitwise_on_integers(kernel):
+    """All row kernels give the same integers and the same zero pattern."""
     w = W.workload(3, n_groups=6, group_size=4, n_tok=500, V=50_000)
     batch = W.make_batch(w, seed=9, device=DEV, ld=50_000)
-    a = P.run_gpu(batch, kernel=A.KERNEL_CLUSTER)
+    a = P.run_gpu(batch, kernel=kernel)
     b = P.run_gpu(batch, kernel=A.KERNEL_GENERIC)
     assert torch.equal(a["tok_traj"], b["tok_traj"])
     assert torch.equal(a["target_logit"], b["target_logit"])
@@ -107,7 +114,7 @@ def test_cluster_matches_generic_bitwise_on_integers():
     assert float((a["token_lp"] - b["token_lp"]).abs().max()) < 2e-5
 
 
-@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER])
+@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF])
 def test_in_place(kernel):
     """dlogits may alias logits exactly (include/awr.h)."""
     w = W.workload(3, n_groups=4, group_size=4, n_tok=300, V=40_000)
