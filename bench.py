@@ -228,7 +228,8 @@ def run_cuda(args):
     esz = logits.element_size()
     params = dict(batch["params"])
     params["kernel"] = {"auto": A.KERNEL_AUTO, "generic": A.KERNEL_GENERIC,
-                        "cluster": A.KERNEL_CLUSTER, "rf": A.KERNEL_CLUSTER_RF}[args.kernel]
+                        "cluster": A.KERNEL_CLUSTER, "rf": A.KERNEL_CLUSTER_RF,
+                        "rf4": A.KERNEL_CLUSTER_RF4}[args.kernel]
     call = A.LossCall(logits, batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
                       batch["step_off"], batch["traj_off"], batch["group_off"],
                       batch["rewards"], want=("err_word",), **params)
@@ -278,7 +279,8 @@ def run_cuda(args):
                 "frac": achieved / peak, "traffic": load_traffic(args.config),
                 "kernel": {A.KERNEL_GENERIC: "rows_generic_kernel",
                            A.KERNEL_CLUSTER: "rows_cluster_kernel",
-                           A.KERNEL_CLUSTER_RF: "rows_rf_kernel"}[kern],
+                           A.KERNEL_CLUSTER_RF: "rows_rf_kernel<NU,2>",
+                           A.KERNEL_CLUSTER_RF4: "rows_rf_kernel<NU,4>"}[kern],
                 "kernel_ms": row_avg_ms, "kernel_share_of_step": row_avg_ms / (local_ms / args.steps),
                 "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src}
 
@@ -378,7 +380,7 @@ def main(argv=None):
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3])
     ap.add_argument("--n-tok", type=int, default=0, help="override the config's token count")
     ap.add_argument("--normalizer", type=int, default=None, choices=[0, 1])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4"])
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: --steps")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

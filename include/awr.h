@@ -74,8 +74,10 @@ enum { AWR_W_K_BY_V = 0 /* w_head[k * V + v] */, AWR_W_V_BY_K = 1 /* w_head[v * 
 enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_GENERIC = 1,  /* one CTA per row, second pass re-reads the row through L2 */
        AWR_KERNEL_CLUSTER = 2,  /* row resident in the shared memory of a 2-CTA cluster (bf16) */
-       AWR_KERNEL_CLUSTER_RF = 3 /* row resident in the register files of a 2-CTA cluster (bf16,
-                                    16K <= V <= 163,840); shared memory is a TMA load FIFO */ };
+       AWR_KERNEL_CLUSTER_RF = 3, /* row resident in the register files of a 2-CTA cluster (bf16,
+                                    16K <= V <= 163,840); shared memory is a TMA load FIFO */
+       AWR_KERNEL_CLUSTER_RF4 = 4 /* the same with a row quarter per CTA of a 4-CTA cluster and
+                                    two CTAs (of different rows) resident per SM */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u };
 

@@ -20,7 +20,7 @@ DTYPE_BF16, DTYPE_F32 = 0, 1
 NORM_CONST_K, NORM_PER_TRAJ = 0, 1
 FLAG_SAMPLE_STD = 1
 W_K_BY_V, W_V_BY_K = 0, 1
-KERNEL_AUTO, KERNEL_GENERIC, KERNEL_CLUSTER, KERNEL_CLUSTER_RF = 0, 1, 2, 3
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_CLUSTER, KERNEL_CLUSTER_RF, KERNEL_CLUSTER_RF4 = 0, 1, 2, 3, 4
 ERRBIT_STEP_OFF, ERRBIT_TRAJ_OFF, ERRBIT_GROUP_OFF, ERRBIT_TARGET_RANGE = 1, 2, 4, 8
 
 _vp = C.c_void_p

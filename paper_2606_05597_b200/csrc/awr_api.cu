@@ -66,7 +66,7 @@ static int check_params(const awr_params* p) {
     if (p->dual_clip_c > 1.f) return AWR_ERR_PARAM;          // Eq. (2) reserved
     if (p->normalizer != AWR_NORM_CONST_K && p->normalizer != AWR_NORM_PER_TRAJ) return AWR_ERR_PARAM;
     if (p->flags & ~(uint32_t)AWR_FLAG_SAMPLE_STD) return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER_RF) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER_RF4) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -81,6 +81,7 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype) {
     const bool ok_rf = rows_rf_supported(V, ld, dtype);
     if (requested == AWR_KERNEL_CLUSTER) return ok ? AWR_KERNEL_CLUSTER : -1;
     if (requested == AWR_KERNEL_CLUSTER_RF) return ok_rf ? AWR_KERNEL_CLUSTER_RF : -1;
+    if (requested == AWR_KERNEL_CLUSTER_RF4) return ok_rf ? AWR_KERNEL_CLUSTER_RF4 : -1;
     if (requested == AWR_KERNEL_GENERIC) return AWR_KERNEL_GENERIC;
     // auto: the cluster kernels pay off once a row is a sizeable fraction of shared memory
     if (V * 2 < 65536) return AWR_KERNEL_GENERIC;
@@ -90,7 +91,8 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype) {
 
 static cudaError_t launch_rows(int kernel, const RowArgs& a, int dtype, int num_sms,
                                cudaStream_t st) {
-    if (kernel == AWR_KERNEL_CLUSTER_RF) return launch_rows_rf(a, num_sms, st);
+    if (kernel == AWR_KERNEL_CLUSTER_RF) return launch_rows_rf(a, num_sms, 2, st);
+    if (kernel == AWR_KERNEL_CLUSTER_RF4) return launch_rows_rf(a, num_sms, 4, st);
     if (kernel == AWR_KERNEL_CLUSTER) return launch_rows_cluster(a, num_sms, st);
     return launch_rows_generic(a, dtype, num_sms, st);
 }

@@ -29,6 +29,6 @@ cudaError_t launch_rows_cluster(const RowArgs& a, int num_sms, cudaStream_t st);
 // a2 + a3 + a4, bf16 rows resident in the register files of a 2-CTA cluster; shared memory is a
 // TMA load FIFO, gradient written with coalesced 16-byte stores.
 bool rows_rf_supported(int64_t V, int64_t ld, int dtype);
-cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, cudaStream_t st);
+cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, int cluster_size, cudaStream_t st);
 
 }  // namespace awr

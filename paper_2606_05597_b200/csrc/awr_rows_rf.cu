@@ -25,16 +25,29 @@
 
 namespace awr {
 
-constexpr int kRfWarps = 16;
-constexpr int kRfThreads = kRfWarps * 32;
-constexpr int kRfSlots = 7;                 // ring slots per warp
+constexpr int kRfParts = 32;                // warps per row (over the whole cluster)
 constexpr int kRfChunkRounds = 4;           // rounds (32 units each) per slot / per TMA copy
 constexpr int kRfChunkUnits = 32 * kRfChunkRounds;
 constexpr int kRfSlotBytes = kRfChunkUnits * 16;
 constexpr int kRfCtrlBytes = 2048;
-constexpr int kRfSmemBytes = kRfCtrlBytes + kRfWarps * kRfSlots * kRfSlotBytes;   // 231,424
 constexpr int kRfMinNU = 3, kRfMaxNU = 20;
 constexpr uint32_t kNegInf2 = 0xff80ff80u;  // bf16x2 (-inf, -inf)
+
+// Two shapes of the same kernel (CL CTAs per cluster x WARPS warps per CTA = 32 parts per row):
+//   CL = 2, WARPS = 16: one CTA per SM, a row half per SM, 7 ring slots per warp (224 KB).
+//   CL = 4, WARPS = 8 : two CTAs per SM (of different rows), a row quarter per CTA, 6 ring slots
+//                       per warp (96 KB per CTA).  The two co-resident CTAs drift out of phase,
+//                       so one's exp pass overlaps the other's load / store passes.
+template <int CL>
+struct RfShape {
+    static constexpr int kWarps = kRfParts / CL;
+    static constexpr int kThreads = kWarps * 32;
+    static constexpr int kSlots = CL == 2 ? 7 : 6;
+    static constexpr int kCtasPerSm = CL == 2 ? 1 : 2;
+    static constexpr int kSmemBytes = kRfCtrlBytes + kWarps * kSlots * kRfSlotBytes;
+};
+static_assert(RfShape<2>::kSmemBytes <= 232448, "227 KB of dynamic shared memory per CTA");
+static_assert(2 * (RfShape<4>::kSmemBytes + 1024) <= 233472, "two CTAs in 228 KB per SM");
 
 struct RfPlan {
     int units_per_row;   // 16-byte units in one row (V / 8)
@@ -42,11 +55,10 @@ struct RfPlan {
 };
 
 struct RfCtrl {
-    uint64_t full[kRfWarps * 8];   // one mbarrier per ring slot per warp (8 >= kRfSlots)
-    float2 stats[2][32];           // [row parity][part] (max, sum) of every warp of the cluster
+    uint64_t full[16 * 8];         // one mbarrier per ring slot per warp (8 >= slots)
+    float2 stats[2][kRfParts];     // [row parity][part] (max, sum) of every warp of the cluster
 };
 static_assert(sizeof(RfCtrl) <= kRfCtrlBytes, "control block");
-static_assert(kRfSmemBytes <= 232448, "227 KB of dynamic shared memory per CTA on sm_100");
 
 namespace rf {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -126,10 +138,12 @@ __device__ __forceinline__ uint32_t fma_bf16x2(uint32_t a, uint32_t b, uint32_t 
 // ---------------------------------------------------------------- the kernel
 // NU = rounds per warp part = ceil(max part units / 32); every round but the last is full for
 // every warp (parts differ by at most one unit and NU is exact, see make_rf_plan).
-template <int NU>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kRfThreads, 1)
+template <int NU, int CL>
+__global__ void __launch_bounds__(RfShape<CL>::kThreads, RfShape<CL>::kCtasPerSm)
 rows_rf_kernel(RowArgs a, RfPlan p) {
     using namespace rf;
+    constexpr int kRfWarps = RfShape<CL>::kWarps;
+    constexpr int kRfSlots = RfShape<CL>::kSlots;
     constexpr int NCH = (NU + kRfChunkRounds - 1) / kRfChunkRounds;
     extern __shared__ __align__(128) uint8_t smem[];
     RfCtrl* ctrl = reinterpret_cast<RfCtrl*>(smem);
@@ -143,7 +157,7 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
 
     // this warp's part of the row, in 16-byte units: [part0, part0 + part_units)
     const int part_idx = (int)rank * kRfWarps + warp;
-    constexpr int nparts = 2 * kRfWarps;
+    constexpr int nparts = kRfParts;
     const int part0 = (int)(((int64_t)p.units_per_row * part_idx) / nparts);
     const int part_units = (int)(((int64_t)p.units_per_row * (part_idx + 1)) / nparts) - part0;
     const int nch = (part_units + kRfChunkUnits - 1) / kRfChunkUnits;     // <= NCH
@@ -269,11 +283,7 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
         for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(kFull, s, o);
 
         // ---- exchange: every warp of the cluster publishes (m_w, s_w) to both CTAs
-        if (lane == 0) {
-            const uint32_t addr = smem_u32(&ctrl->stats[par][part_idx]);
-            st_cluster_f32x2(addr, 0, m, s);
-            st_cluster_f32x2(addr, 1, m, s);
-        }
+        if (lane < CL) st_cluster_f32x2(smem_u32(&ctrl->stats[par][part_idx]), (uint32_t)lane, m, s);
         __syncwarp();
         cluster_arrive();
         cluster_wait();
@@ -331,20 +341,15 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
 }
 
 // ---------------------------------------------------------------- host side
-static bool make_rf_plan(int64_t V, int64_t ld, int dtype, int num_sms, int64_t n_tok, RfPlan& p,
-                         int& nu) {
+static bool make_rf_plan(int64_t V, int64_t ld, int dtype, RfPlan& p, int& nu) {
     if (dtype != AWR_DTYPE_BF16) return false;
     if (V % 8 != 0 || ld % 8 != 0) return false;
     const int64_t units = V / 8;
-    const int nparts = 2 * kRfWarps;
-    const int64_t part_max = (units + nparts - 1) / nparts;
+    const int64_t part_max = (units + kRfParts - 1) / kRfParts;
     const int64_t n = (part_max + 31) / 32;
     if (n < kRfMinNU || n > kRfMaxNU) return false;
     p.units_per_row = (int)units;
-    int nc = num_sms / 2;
-    if ((int64_t)nc > n_tok) nc = (int)n_tok;
-    if (nc < 1) nc = 1;
-    p.num_clusters = nc;
+    p.num_clusters = 0;
     nu = (int)n;
     return true;
 }
@@ -352,30 +357,54 @@ static bool make_rf_plan(int64_t V, int64_t ld, int dtype, int num_sms, int64_t 
 bool rows_rf_supported(int64_t V, int64_t ld, int dtype) {
     RfPlan p;
     int nu;
-    return make_rf_plan(V, ld, dtype, 148, 1 << 20, p, nu);
+    return make_rf_plan(V, ld, dtype, p, nu);
 }
 
-template <int NU>
-static cudaError_t launch_nu(const RowArgs& a, const RfPlan& p, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(rows_rf_kernel<NU>,
+template <int NU, int CL>
+static cudaError_t launch_nu(const RowArgs& a, RfPlan p, int num_sms, cudaStream_t st) {
+    using S = RfShape<CL>;
+    static int max_clusters = -1;            // co-resident clusters (device query, cached)
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CL;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(S::kThreads, 1, 1);
+    cfg.dynamicSmemBytes = S::kSmemBytes;
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (max_clusters < 0) {
+        cudaError_t e = cudaFuncSetAttribute(rows_rf_kernel<NU, CL>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             kRfSmemBytes);
+                                             S::kSmemBytes);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        cfg.gridDim = dim3(CL * num_sms, 1, 1);
+        int n = 0;
+        e = cudaOccupancyMaxActiveClusters(&n, rows_rf_kernel<NU, CL>, &cfg);
+        if (e != cudaSuccess) return e;
+        const int want = num_sms * S::kCtasPerSm / CL;
+        max_clusters = n < 1 ? 1 : (n > want ? want : n);
     }
-    rows_rf_kernel<NU><<<2 * p.num_clusters, kRfThreads, kRfSmemBytes, st>>>(a, p);
-    return cudaGetLastError();
+    int nc = max_clusters;
+    if ((int64_t)nc > a.n_tok) nc = (int)a.n_tok;
+    p.num_clusters = nc;
+    cfg.gridDim = dim3(CL * nc, 1, 1);
+    return cudaLaunchKernelEx(&cfg, rows_rf_kernel<NU, CL>, a, p);
 }
 
-cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, cudaStream_t st) {
+cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, int cluster_size, cudaStream_t st) {
     if (a.n_tok <= 0) return cudaSuccess;
     RfPlan p;
     int nu = 0;
-    if (!make_rf_plan(a.V, a.ld, AWR_DTYPE_BF16, num_sms, a.n_tok, p, nu)) return cudaErrorInvalidValue;
+    if (!make_rf_plan(a.V, a.ld, AWR_DTYPE_BF16, p, nu)) return cudaErrorInvalidValue;
+    if (cluster_size != 2 && cluster_size != 4) return cudaErrorInvalidValue;
     switch (nu) {
-#define AWR_RF_CASE(N) case N: return launch_nu<N>(a, p, st);
+#define AWR_RF_CASE(N)                                                       \
+    case N:                                                                  \
+        return cluster_size == 2 ? launch_nu<N, 2>(a, p, num_sms, st)        \
+                                 : launch_nu<N, 4>(a, p, num_sms, st);
         AWR_RF_CASE(3) AWR_RF_CASE(4) AWR_RF_CASE(5) AWR_RF_CASE(6) AWR_RF_CASE(7) AWR_RF_CASE(8)
         AWR_RF_CASE(9) AWR_RF_CASE(10) AWR_RF_CASE(11) AWR_RF_CASE(12) AWR_RF_CASE(13)
         AWR_RF_CASE(14) AWR_RF_CASE(15) AWR_RF_CASE(16) AWR_RF_CASE(17) AWR_RF_CASE(18)

@@ -72,7 +72,7 @@ CLUSTER_SHAPES = [(151_936, 151_936), (40_000, 40_008), (32_768, 32_768), (65_54
                   (131_072, 131_072)]
 
 
-CLUSTER_KERNELS = [A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF]
+CLUSTER_KERNELS = [A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4]
 
 
 @pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
@@ -114,7 +114,7 @@ def test_cluster_matches_generic_bitwise_on_integers(kernel):
     assert float((a["token_lp"] - b["token_lp"]).abs().max()) < 2e-5
 
 
-@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF])
+@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC] + CLUSTER_KERNELS)
 def test_in_place(kernel):
     """dlogits may alias logits exactly (include/awr.h)."""
     w = W.workload(3, n_groups=4, group_size=4, n_tok=300, V=40_000)
