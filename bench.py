@@ -362,8 +362,8 @@ def run_cuda(args):
 
 def load_traffic(cfg: int):
     """dram bytes (read + write) per launch of the row kernel from the committed `ncu --set full`
-    capture (profiles/traffic.json, written by hand from the capture named there), or null."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    capture (profiles/r1_traffic.txt, JSON text written by hand from the capture named there), or null."""
+    p = os.path.join(ROOT, "profiles", "r1_traffic.txt")
     if not os.path.exists(p):
         return None
     with open(p) as f:
