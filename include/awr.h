@@ -164,7 +164,7 @@ AWR_API size_t awr_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t ld, in
 typedef struct awr_head_batch {
     int64_t n_tok;
     int64_t V;
-    int64_t K;                  /* hidden size; multiple of 64 */
+    int64_t K;                  /* hidden size; multiple of 64 (V: multiple of 8) */
     const void* hidden;         /* bf16 [n_tok, K] row-major */
     const void* w_head;         /* bf16, layout w_layout */
     const int32_t* target_ids;
@@ -198,6 +198,19 @@ AWR_API int awr_loss_fwd_bwd_fused_head(const awr_head_batch* batch, const awr_p
                                 size_t workspace_bytes, void* stream);
 AWR_API size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
                                 int32_t n_traj, int32_t n_groups);
+
+/* Kernel launches one awr_loss_fwd_bwd_fused_head call enqueues for this shape. */
+AWR_API int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K);
+
+/* The tensor-core engine of a5 on its own (tests, benchmarks): C[M, N] = A B, bf16 operands,
+ * fp32 accumulation in tensor memory, bf16 row-major result C[m * ldc + n].  A is [M, Kc] and B
+ * is [Kc, N] as matrices; *_major says which index is contiguous in memory:
+ *   a_major 0: A[m * lda + k]   a_major 1: A[k * lda + m]
+ *   b_major 0: B[n * ldb + k]   b_major 1: B[k * ldb + n]
+ * lda, ldb, ldc and N multiples of 8; pointers 16-byte aligned; device pointers. */
+AWR_API int awr_gemm_bf16(const void* A, int32_t a_major, int64_t lda, const void* B, int32_t b_major,
+                  int64_t ldb, int64_t M, int64_t N, int64_t Kc, void* C, int64_t ldc,
+                  void* stream);
 
 AWR_API const char* awr_status_string(int status);
 AWR_API int awr_version(void);

@@ -77,6 +77,9 @@ SYMBOLS = {
                                               C.POINTER(awr_head_outputs), _vp, C.c_size_t, _vp]),
     "awr_head_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int64, C.c_int64, C.c_int32,
                                               C.c_int32, C.c_int32]),
+    "awr_head_launches_per_call": (C.c_int, [C.c_int64, C.c_int64, C.c_int64]),
+    "awr_gemm_bf16": (C.c_int, [_vp, C.c_int32, C.c_int64, _vp, C.c_int32, C.c_int64, C.c_int64,
+                                C.c_int64, C.c_int64, _vp, C.c_int64, _vp]),
     "awr_status_string": (C.c_char_p, [C.c_int]),
     "awr_version": (C.c_int, []),
     "awr_select_kernel": (C.c_int, [C.c_int64, C.c_int64, C.c_int32]),

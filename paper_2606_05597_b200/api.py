@@ -248,3 +248,108 @@ def awr_loss_fwd_bwd_host(logits, target_ids, behave_lp, prox_lp, step_off, traj
                           rewards, **kw):
     return HostLossCall(logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off,
                         rewards, **kw).run()
+
+
+# ---------------------------------------------------------------------------- a5: fused LM head
+HEAD_OPTIONAL_OUTPUTS = ("adv", "tok_traj", "tok_term", "tok_coef", "err_word")
+
+
+def head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups) -> int:
+    return int(load().awr_head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups))
+
+
+def head_launches_per_call(n_tok, V, K) -> int:
+    return int(load().awr_head_launches_per_call(n_tok, V, K))
+
+
+class HeadLossCall:
+    """One prepared awr_loss_fwd_bwd_fused_head call (hidden states + W_head instead of logits;
+    the logits live only in tensor memory).  ``run()`` enqueues it on the current stream."""
+
+    def __init__(self, hidden, w_head, target_ids, behave_lp, prox_lp, step_off, traj_off,
+                 group_off, rewards, *, w_layout=_abi.W_K_BY_V, want=HEAD_OPTIONAL_OUTPUTS,
+                 workspace=None, **params):
+        self.lib = load()
+        _req(hidden, torch.bfloat16, "hidden")
+        _req(w_head, torch.bfloat16, "w_head")
+        if hidden.dim() != 2 or w_head.dim() != 2:
+            raise TypeError("hidden must be [n_tok, K] and w_head [K, V] or [V, K]")
+        n_tok, K = hidden.shape
+        if w_layout == _abi.W_K_BY_V:
+            if w_head.shape[0] != K:
+                raise ValueError("w_head must be [K, V] for W_K_BY_V")
+            V = w_head.shape[1]
+        else:
+            if w_head.shape[1] != K:
+                raise ValueError("w_head must be [V, K] for W_V_BY_K")
+            V = w_head.shape[0]
+        for t, dt, name in ((target_ids, torch.int32, "target_ids"),
+                            (behave_lp, torch.float32, "behave_lp"),
+                            (prox_lp, torch.float32, "prox_lp"), (step_off, torch.int32, "step_off"),
+                            (traj_off, torch.int32, "traj_off"), (group_off, torch.int32, "group_off"),
+                            (rewards, torch.float32, "rewards")):
+            _req(t, dt, name)
+        if target_ids.numel() != n_tok or behave_lp.numel() != n_tok or prox_lp.numel() != n_tok:
+            raise ValueError("per-token arrays must have n_tok = %d entries" % n_tok)
+        dev = hidden.device
+        self.device = dev
+        n_steps, n_traj, n_groups = step_off.numel() - 1, traj_off.numel() - 1, group_off.numel() - 1
+        self.batch = awr_head_batch(n_tok, V, K, _ptr(hidden), _ptr(w_head), _ptr(target_ids),
+                                    _ptr(behave_lp), _ptr(prox_lp), _ptr(step_off), _ptr(traj_off),
+                                    _ptr(group_off), _ptr(rewards), n_steps, n_traj, n_groups,
+                                    int(w_layout))
+        params.pop("kernel", None)
+        self.params = make_params(**params)
+        o = dict(loss=torch.empty(1, dtype=torch.float32, device=dev),
+                 dhidden=torch.empty_like(hidden), dw_head=torch.empty_like(w_head),
+                 token_lp=torch.empty(n_tok, dtype=torch.float32, device=dev),
+                 clip_count=torch.empty(1, dtype=torch.int64, device=dev))
+        spec = dict(adv=(n_traj, torch.float32), tok_traj=(n_tok, torch.int32),
+                    tok_term=(n_tok, torch.float32), tok_coef=(n_tok, torch.float32),
+                    err_word=(1, torch.int32))
+        for k in want:
+            n, dt = spec[k]
+            o[k] = torch.empty(n, dtype=dt, device=dev)
+        self.out = o
+        g = o.get
+        self.outs = awr_head_outputs(_ptr(g("loss")), _ptr(g("dhidden")), _ptr(g("dw_head")),
+                                     _ptr(g("token_lp")), _ptr(g("clip_count")), _ptr(g("adv")),
+                                     _ptr(g("tok_traj")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
+                                     _ptr(g("err_word")))
+        need = head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups)
+        self.workspace = workspace if workspace is not None else torch.empty(
+            max(need, 256), dtype=torch.uint8, device=dev)
+        self.ws_bytes = self.workspace.numel()
+        self.launches = head_launches_per_call(n_tok, V, K)
+        self._keep = (hidden, w_head, target_ids, behave_lp, prox_lp, step_off, traj_off,
+                      group_off, rewards)
+
+    def run(self, stream=None):
+        rc = self.lib.awr_loss_fwd_bwd_fused_head(
+            C.byref(self.batch), C.byref(self.params), C.byref(self.outs), _ptr(self.workspace),
+            self.ws_bytes, _stream_ptr(stream, self.device))
+        check(rc, "awr_loss_fwd_bwd_fused_head")
+        return self.out
+
+
+def awr_loss_fwd_bwd_fused_head(hidden, w_head, target_ids, behave_lp, prox_lp, step_off, traj_off,
+                                group_off, rewards, stream=None, **kw):
+    """loss, dhidden, dw_head, token_lp, clip_count (+ optional per-token outputs) as a dict."""
+    return HeadLossCall(hidden, w_head, target_ids, behave_lp, prox_lp, step_off, traj_off,
+                        group_off, rewards, **kw).run(stream)
+
+
+def awr_gemm_bf16(a, b, a_major=0, b_major=0, stream=None):
+    """C = A B on the tcgen05 engine of the fused head.  `a` is stored [M, Kc] (a_major 0) or
+    [Kc, M] (a_major 1); `b` is stored [N, Kc] (b_major 0) or [Kc, N] (b_major 1)."""
+    _req(a, torch.bfloat16, "a")
+    _req(b, torch.bfloat16, "b")
+    M, Kc = (a.shape[0], a.shape[1]) if a_major == 0 else (a.shape[1], a.shape[0])
+    N, Kb = (b.shape[0], b.shape[1]) if b_major == 0 else (b.shape[1], b.shape[0])
+    if Kc != Kb:
+        raise ValueError("contraction lengths differ: %d vs %d" % (Kc, Kb))
+    c = torch.empty((M, N), dtype=torch.bfloat16, device=a.device)
+    rc = load().awr_gemm_bf16(_ptr(a), a_major, a.stride(0), _ptr(b), b_major, b.stride(0), M, N, Kc,
+                              _ptr(c), c.stride(0), _stream_ptr(stream, a.device))
+    check(rc, "awr_gemm_bf16")
+    return c

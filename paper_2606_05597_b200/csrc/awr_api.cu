@@ -238,6 +238,95 @@ int awr_group_advantage(const float* rewards, const int32_t* group_off, int32_t 
     return AWR_OK;
 }
 
+// ------------------------------------------------------------------ a5: fused LM head
+size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
+                                int32_t n_traj, int32_t n_groups) {
+    (void)n_steps; (void)n_groups;
+    if (n_tok < 0 || n_traj < 0 || V <= 0 || K <= 0) return 0;
+    return carve(nullptr, n_tok, n_traj).total + head_ws_bytes(n_tok, V, K);
+}
+
+int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K) {
+    return 3 + head_launches(n_tok, V, K);     // a0, a1, [F, scalars, 3 per panel], final sum
+}
+
+int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
+                                const awr_head_outputs* o, void* ws_ptr, size_t ws_bytes,
+                                void* stream) {
+    if (!b || !p || !o) return AWR_ERR_NULL;
+    int rc = check_segments(b->n_tok, b->n_steps, b->n_traj, b->n_groups);
+    if (rc) return rc;
+    if (b->V <= 0 || b->K <= 0 || b->V % 8 != 0 || b->K % 64 != 0) return AWR_ERR_SHAPE;
+    if (b->V > 0x7fffffffLL || b->K > 0x7fffffffLL) return AWR_ERR_SHAPE;
+    if (b->w_layout != AWR_W_K_BY_V && b->w_layout != AWR_W_V_BY_K) return AWR_ERR_DTYPE;
+    rc = check_params(p);
+    if (rc) return rc;
+    if (!o->loss || !o->clip_count || !o->dw_head) return AWR_ERR_NULL;
+    if (b->n_tok > 0 && (!o->token_lp || !o->dhidden)) return AWR_ERR_NULL;
+    if (!b->step_off || !b->traj_off || !b->group_off || !b->w_head) return AWR_ERR_NULL;
+    if (b->n_tok > 0 && (!b->hidden || !b->target_ids || !b->behave_lp || !b->prox_lp)) return AWR_ERR_NULL;
+    if (b->n_traj > 0 && !b->rewards) return AWR_ERR_NULL;
+    if ((reinterpret_cast<uintptr_t>(b->hidden) & 15) || (reinterpret_cast<uintptr_t>(b->w_head) & 15) ||
+        (reinterpret_cast<uintptr_t>(o->dhidden) & 15) || (reinterpret_cast<uintptr_t>(o->dw_head) & 15))
+        return AWR_ERR_ALIGN;
+    const size_t need = awr_head_workspace_bytes(b->n_tok, b->V, b->K, b->n_steps, b->n_traj, b->n_groups);
+    if (!ws_ptr || (reinterpret_cast<uintptr_t>(ws_ptr) & 255) || ws_bytes < need) return AWR_ERR_WORKSPACE;
+    DeviceInfo info;
+    if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    if (info.major != 10) return AWR_ERR_ARCH;
+
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Workspace w = carve(ws_ptr, b->n_tok, b->n_traj);
+    uint32_t* err = o->err_word ? o->err_word : w.err;
+    float* adv = o->adv ? o->adv : w.adv;
+    int32_t* tok_traj = o->tok_traj ? o->tok_traj : w.tok_traj;
+    float* tok_term = o->tok_term ? o->tok_term : w.tok_term;
+
+    cudaError_t e = cudaMemsetAsync(ws_ptr, 0, w.zero_bytes, st);
+    if (e == cudaSuccess && o->err_word) e = cudaMemsetAsync(o->err_word, 0, 4, st);
+    if (e == cudaSuccess && o->adv && b->n_traj > 0) e = cudaMemsetAsync(o->adv, 0, (size_t)b->n_traj * 4, st);
+    if (e == cudaSuccess)
+        e = launch_segment_expand(b->step_off, b->traj_off, b->group_off, b->n_tok, b->n_steps,
+                                  b->n_traj, b->n_groups, tok_traj, err, st);
+    if (e == cudaSuccess)
+        e = launch_group_advantage(b->rewards, b->group_off, b->traj_off, b->n_groups, b->n_traj,
+                                   p->flags, p->normalizer, p->k_norm, p->loss_scale, adv,
+                                   w.traj_scale, st);
+    RowArgs a = {};
+    a.n_tok = b->n_tok; a.V = b->V; a.ld = b->V;
+    a.target_ids = b->target_ids; a.behave_lp = b->behave_lp; a.prox_lp = b->prox_lp;
+    a.tok_traj = tok_traj; a.adv = adv; a.traj_scale = w.traj_scale;
+    a.token_lp = o->token_lp; a.tok_term = tok_term; a.tok_coef = o->tok_coef;
+    a.target_logit = nullptr; a.tok_flag = w.tok_flag; a.err_word = err;
+    a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap;
+    HeadCall c;
+    c.hidden = b->hidden; c.w_head = b->w_head; c.w_layout = b->w_layout;
+    c.n_tok = b->n_tok; c.V = b->V; c.K = b->K; c.rows = &a;
+    c.dhidden = o->dhidden; c.dw_head = o->dw_head;
+    c.ws = reinterpret_cast<uint8_t*>(ws_ptr) + w.total;
+    if (e == cudaSuccess) e = launch_head(c, info.num_sms, st);
+    if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    return AWR_OK;
+}
+
+int awr_gemm_bf16(const void* A, int32_t a_major, int64_t lda, const void* B, int32_t b_major,
+                  int64_t ldb, int64_t M, int64_t N, int64_t Kc, void* C, int64_t ldc, void* stream) {
+    if (!A || !B || !C) return AWR_ERR_NULL;
+    if (M <= 0 || N <= 0 || Kc <= 0 || M > 0x7fffffffLL || N > 0x7fffffffLL || Kc > 0x7fffffffLL) return AWR_ERR_SHAPE;
+    if ((a_major != 0 && a_major != 1) || (b_major != 0 && b_major != 1)) return AWR_ERR_DTYPE;
+    if (lda % 8 || ldb % 8 || ldc % 8 || N % 8) return AWR_ERR_ALIGN;
+    if ((reinterpret_cast<uintptr_t>(A) & 15) || (reinterpret_cast<uintptr_t>(B) & 15) ||
+        (reinterpret_cast<uintptr_t>(C) & 15)) return AWR_ERR_ALIGN;
+    DeviceInfo info;
+    if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    if (info.major != 10) return AWR_ERR_ARCH;
+    cudaError_t e = launch_gemm_bf16(A, a_major, lda, B, b_major, ldb, M, N, Kc, C, ldc, info.num_sms,
+                                     reinterpret_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    return AWR_OK;
+}
+
 // ------------------------------------------------------------------ host-buffer variant
 namespace {
 constexpr int kPanelBufs = 3;

@@ -1,9 +1,537 @@
-// a5 placeholder until the tcgen05 fused LM-head kernels land (next commit).
-#include "awr_common.cuh"
-extern "C" {
-__attribute__((visibility("default")))
-int awr_loss_fwd_bwd_fused_head(const awr_head_batch*, const awr_params*, const awr_head_outputs*,
-                                void*, size_t, void*) { return AWR_ERR_PARAM; }
-__attribute__((visibility("default")))
-size_t awr_head_workspace_bytes(int64_t, int64_t, int64_t, int32_t, int32_t, int32_t) { return 0; }
+// a5: fused LM-head variant (BASELINE.json config 4, readings A17).
+//
+//   logits Z = H W_head are produced tile by tile in tensor memory and never stored:
+//   pass F   Z tile -> per-row (max, sum exp) partials + target gather          (GEMM, kEpiLse)
+//   scalars  partials -> lse, l_t, ratio / clip / normalizer (a3), c_t           (one warp per row)
+//   per panel of P rows (P x V bf16 transient, 1.4 GB at the default P):
+//     pass G1  recompute the Z tile -> dS = c_t (softmax - onehot) in bf16       (GEMM, kEpiDs)
+//     pass G2  dhidden[panel] = dS W_head^T                                      (GEMM, kEpiStoreBf16)
+//     pass G3  dw_head += H[panel]^T dS   (fp32 running sum, bf16 at the end)    (GEMM, kEpiAccum)
+// Every GEMM is the tcgen05 kernel below; see awr_head_gemm.cuh for the engine.
+#include "awr_head_gemm.cuh"
+#include "awr_kernels.h"
+
+namespace awr {
+namespace head {
+
+__device__ __forceinline__ void tile_coords(const GemmArgs& g, int tile, int& m_blk, int& n_blk) {
+    if (g.order == 0) {
+        const int per_group = g.group_m * g.n_tiles;
+        const int gi = tile / per_group;
+        const int r = tile - gi * per_group;
+        const int gm = min(g.group_m, g.m_tiles - gi * g.group_m);
+        m_blk = gi * g.group_m + r % gm;
+        n_blk = r / gm;
+    } else {
+        m_blk = tile / g.n_tiles;
+        n_blk = tile - m_blk * g.n_tiles;
+    }
 }
+
+template <int EPI>
+__global__ void __launch_bounds__(kThreads, 1)
+head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
+                 const __grid_constant__ CUtensorMap tmap_b, const GemmArgs g) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bars = smem_base + kStages * kStageBytes;
+    // barrier words: full[kStages], empty[kStages], tmem_full[2], tmem_empty[2], tmem ptr
+    auto full_bar = [&](int s) { return bars + 8u * s; };
+    auto empty_bar = [&](int s) { return bars + 8u * (kStages + s); };
+    auto tfull_bar = [&](int s) { return bars + 8u * (2 * kStages + s); };
+    auto tempty_bar = [&](int s) { return bars + 8u * (2 * kStages + 2 + s); };
+    const uint32_t tmem_slot = bars + 8u * (2 * kStages + 4);
+    uint32_t* tmem_slot_ptr =
+        reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int num_tiles = g.m_tiles * g.n_tiles;
+    const int num_kb = (g.Kc + kBK - 1) / kBK;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_b) : "memory");
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
+                     "n"(kTmemCols)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                int m_blk, n_blk;
+                tile_coords(g, tile, m_blk, n_blk);
+                const int m0 = m_blk * kBM, n0 = n_blk * kBN;
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    const uint32_t sa = smem_base + stage * kStageBytes;
+                    const uint32_t sb = sa + kABytes;
+                    const uint32_t bar = full_bar(stage);
+                    mbar_expect_tx(bar, kStageBytes);
+                    const int k0 = kb * kBK;
+                    for (uint32_t j = 0; j < g.a.boxes; ++j) {
+                        if (g.a.major == kMajorK) tma_load_2d(sa, &tmap_a, k0, m0, bar);
+                        else tma_load_2d(sa + j * g.a.box_bytes, &tmap_a, m0 + 64 * (int)j, k0, bar);
+                    }
+                    for (uint32_t j = 0; j < g.b.boxes; ++j) {
+                        if (g.b.major == kMajorK) tma_load_2d(sb, &tmap_b, k0, n0, bar);
+                        else tma_load_2d(sb + j * g.b.box_bytes, &tmap_b, n0 + 64 * (int)j, k0, bar);
+                    }
+                    if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int as = 0;
+            uint32_t aphase = 0;
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                mbar_wait(tempty_bar(as), aphase ^ 1u);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)as * kBN;
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    mbar_wait(full_bar(stage), phase);
+                    tc_fence_after();
+                    const uint32_t sa = smem_base + stage * kStageBytes;
+                    const uint32_t sb = sa + kABytes;
+                    const uint32_t a_lo = ((sa >> 4) & 0x3fffu) | g.a.desc_lo;
+                    const uint32_t b_lo = ((sb >> 4) & 0x3fffu) | g.b.desc_lo;
+#pragma unroll
+                    for (int k = 0; k < kBK / kUmmaK; ++k) {
+                        const uint64_t adesc =
+                            ((uint64_t)g.a.desc_hi << 32) | (uint64_t)(a_lo + k * g.a.k_step);
+                        const uint64_t bdesc =
+                            ((uint64_t)g.b.desc_hi << 32) | (uint64_t)(b_lo + k * g.b.k_step);
+                        tc_mma(d_tmem, adesc, bdesc, g.idesc, (uint32_t)((kb | k) != 0));
+                    }
+                    tc_commit(empty_bar(stage));          // smem slot free once these MMAs retire
+                    if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                }
+                tc_commit(tfull_bar(as));                 // accumulator tile complete
+                if (++as == 2) { as = 0; aphase ^= 1u; }
+            }
+        }
+    } else if (warp >= 4) {
+        // ===================== epilogue: one accumulator row per thread
+        const int q = warp & 3;                           // TMEM lane quarter of this warp
+        int as = 0;
+        uint32_t aphase = 0;
+        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            int m_blk, n_blk;
+            tile_coords(g, tile, m_blk, n_blk);
+            const int row = m_blk * kBM + q * 32 + lane;
+            const int n0 = n_blk * kBN;
+            const bool row_ok = row < g.M;
+            mbar_wait(tfull_bar(as), aphase);
+            tc_fence_after();
+            const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)as * kBN;
+            float v[32];
+
+            if constexpr (EPI == kEpiLse) {
+                const int y = row_ok ? g.e.target_ids[row] : -1;
+                float m = -INFINITY, s = 0.f, zy = 0.f;
+                const bool y_here = (y >= n0) && (y < n0 + kBN) && (y < g.N);
+#pragma unroll 1
+                for (int c = 0; c < kBN / 32; ++c) {
+                    tmem_ld32(t_addr + c * 32, v);
+                    const int c0 = n0 + c * 32;
+                    if (c0 + 32 > g.N) {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) if (c0 + j >= g.N) v[j] = -INFINITY;
+                    }
+                    if (y_here && y >= c0 && y < c0 + 32) {
+                        // the target entry is gathered and left out of the (max, sum) state
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) if (c0 + j == y) { zy = v[j]; v[j] = -INFINITY; }
+                    }
+                    float cm = v[0];
+#pragma unroll
+                    for (int j = 1; j < 32; ++j) cm = fmaxf(cm, v[j]);
+                    const float mn = fmaxf(m, cm);
+                    if (mn != -INFINITY) {
+                        const float ref = mn * kLog2e;
+                        float acc = 0.f;
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) acc += ex2_approx(fmaf(v[j], kLog2e, -ref));
+                        s = s * ex2_approx(fmaf(m, kLog2e, -ref)) + acc;
+                        m = mn;
+                    }
+                }
+                if (row_ok) {
+                    g.e.part[(int64_t)n_blk * g.e.part_ld + row] = make_float2(m, s);
+                    if (y_here) g.e.zy[row] = zy;
+                }
+            } else if constexpr (EPI == kEpiDs) {
+                int y = -1;
+                float lse = 0.f, coef = 0.f, gy = 0.f;
+                if (row_ok) {
+                    y = g.e.target_ids[row]; lse = g.e.row_lse[row];
+                    coef = g.e.row_coef[row]; gy = g.e.row_gy[row];
+                }
+                const float nref = -lse * kLog2e;
+                __nv_bfloat16* dst = g.e.ds + (int64_t)row * g.e.ds_ld + n0;
+#pragma unroll 1
+                for (int c = 0; c < kBN / 32; ++c) {
+                    tmem_ld32(t_addr + c * 32, v);
+                    const int c0 = n0 + c * 32;
+                    if (!row_ok || c0 >= g.N) continue;
+                    uint32_t o[16];
+                    if (coef == 0.f) {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) o[j] = 0u;
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) v[j] = coef * ex2_approx(fmaf(v[j], kLog2e, nref));
+                        if (y >= c0 && y < c0 + 32) {
+#pragma unroll
+                            for (int j = 0; j < 32; ++j) if (c0 + j == y) v[j] = gy;
+                        }
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) o[j] = pack_bf16x2(v[2 * j], v[2 * j + 1]);
+                    }
+                    // ds_ld and N are multiples of 8: 16-byte stores, whole 8-column groups
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if (c0 + 8 * j < g.N)
+                            *reinterpret_cast<uint4*>(dst + c * 32 + 8 * j) =
+                                make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+                }
+            } else {
+                const int64_t ro = (int64_t)row * g.e.out_ld + n0;
+#pragma unroll 1
+                for (int c = 0; c < kBN / 32; ++c) {
+                    tmem_ld32(t_addr + c * 32, v);
+                    const int c0 = n0 + c * 32;
+                    if (!row_ok || c0 >= g.N) continue;
+                    bool to_bf16 = true;
+                    if constexpr (EPI == kEpiAccum) {
+                        float* ap = g.e.acc + ro + c * 32;
+                        if (!g.e.first_panel) {
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) {
+                                if (c0 + 4 * j < g.N) {
+                                    const float4 p = *reinterpret_cast<const float4*>(ap + 4 * j);
+                                    v[4 * j] += p.x; v[4 * j + 1] += p.y;
+                                    v[4 * j + 2] += p.z; v[4 * j + 3] += p.w;
+                                }
+                            }
+                        }
+                        to_bf16 = g.e.last_panel != 0;
+                        if (!to_bf16) {
+#pragma unroll
+                            for (int j = 0; j < 8; ++j)
+                                if (c0 + 4 * j < g.N)
+                                    *reinterpret_cast<float4*>(ap + 4 * j) =
+                                        make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+                        }
+                    }
+                    if (to_bf16) {
+                        __nv_bfloat16* dst = g.e.out + ro + c * 32;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            if (c0 + 8 * j < g.N)
+                                *reinterpret_cast<uint4*>(dst + 8 * j) = make_uint4(
+                                    pack_bf16x2(v[8 * j], v[8 * j + 1]), pack_bf16x2(v[8 * j + 2], v[8 * j + 3]),
+                                    pack_bf16x2(v[8 * j + 4], v[8 * j + 5]), pack_bf16x2(v[8 * j + 6], v[8 * j + 7]));
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar(as));
+            if (++as == 2) { as = 0; aphase ^= 1u; }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base),
+                     "n"(kTmemCols)
+                     : "memory");
+    }
+}
+
+}  // namespace head
+}  // namespace awr
+
+// ================================================================== scalars (a3 for the head path)
+namespace awr {
+namespace head {
+
+// One warp per row: combine the per-column-tile (max, sum) partials into the log-sum-exp of
+// the row without its target entry, then the same token_scalars() as the logits path.
+__global__ void __launch_bounds__(256)
+head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld, int n_tiles,
+                    const float* __restrict__ zy, float* __restrict__ row_lse,
+                    float* __restrict__ row_coef, float* __restrict__ row_gy) {
+    const int lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= a.n_tok) return;
+    MaxSum st{-INFINITY, 0.f};
+    for (int j = lane; j < n_tiles; j += 32) {
+        const float2 p = part[(int64_t)j * part_ld + row];
+        st = combine(st, MaxSum{p.x, p.y});
+    }
+    st = warp_combine(st);
+    const float lse_rest = st.m + logf(st.s);          // -inf when nothing but the target
+    RowHeader h;
+    h.y = a.target_ids[row];
+    const bool valid = (h.y >= 0) && (h.y < a.V);
+    const int traj = a.tok_traj[row];
+    h.q = a.prox_lp[row];
+    h.b = a.behave_lp[row];
+    h.A = traj >= 0 ? a.adv[traj] : 0.f;
+    h.scale = traj >= 0 ? a.traj_scale[traj] : 0.f;
+    h.zy = valid ? zy[row] : 0.f;
+    const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap);
+    if (lane == 0) {
+        if (h.y >= a.V) atomicOr(a.err_word, AWR_ERRBIT_TARGET_RANGE);
+        store_token_outputs(a, row, h, ts, valid);
+        row_lse[row] = ts.lse;
+        row_coef[row] = ts.coef;
+        row_gy[row] = ts.gy;
+    }
+}
+
+// ================================================================== host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// A bf16 matrix as the GEMM sees one operand: `mn` rows or columns of the product, `kc`
+// contraction length, element (i_mn, i_k) at base[i_mn * s_mn + i_k * s_k] with one of the two
+// strides equal to 1.
+struct OperandView {
+    const void* base;
+    int64_t mn, kc;
+    int64_t ld;        // the non-unit stride, in elements
+    int major;         // kMajorK: i_k contiguous; kMajorMN: i_mn contiguous
+};
+
+static bool make_operand(const OperandView& v, int tile_mn, CUtensorMap* map, Operand* op) {
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return false;
+    cuuint64_t dims[2], strides[1];
+    cuuint32_t box[2], estr[2] = {1, 1};
+    strides[0] = (cuuint64_t)v.ld * 2;
+    if (v.major == kMajorK) {
+        dims[0] = (cuuint64_t)v.kc; dims[1] = (cuuint64_t)v.mn;
+        box[0] = kBK; box[1] = (cuuint32_t)tile_mn;
+        op->boxes = 1; op->box_bytes = (uint32_t)tile_mn * kBK * 2;
+        op->desc_lo = 1u << 16;                       // leading byte offset: unused with swizzle
+        op->k_step = (kUmmaK * 2) >> 4;               // 32 bytes inside the 128-byte row
+    } else {
+        dims[0] = (cuuint64_t)v.mn; dims[1] = (cuuint64_t)v.kc;
+        box[0] = 64; box[1] = kBK;
+        op->boxes = (uint32_t)tile_mn / 64; op->box_bytes = 64 * kBK * 2;
+        op->desc_lo = (uint32_t)(op->box_bytes >> 4) << 16;   // next 64-wide MN chunk
+        op->k_step = (kUmmaK * 128) >> 4;             // 16 contraction rows of 128 bytes
+    }
+    op->major = (uint32_t)v.major;
+    op->desc_hi = (1024u >> 4) | (1u << 14) | (2u << 29);     // SBO 1024 B, version 1, SWIZZLE_128B
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(v.base), dims,
+                     strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+template <int EPI>
+static cudaError_t launch_gemm_epi(const CUtensorMap& ta, const CUtensorMap& tb, const GemmArgs& g,
+                                   int grid, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(head_gemm_kernel<EPI>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    head_gemm_kernel<EPI><<<grid, kThreads, kSmemBytes, st>>>(ta, tb, g);
+    return cudaGetLastError();
+}
+
+// C[M, N] = A * B with epilogue `epi`; `order` / `group_m` pick the tile raster.
+static cudaError_t launch_gemm(int epi, const OperandView& A, const OperandView& B, int order,
+                               int group_m, const EpiArgs& e, int num_sms, cudaStream_t st) {
+    if (A.mn <= 0 || B.mn <= 0 || A.kc <= 0) return cudaSuccess;
+    if (A.kc != B.kc) return cudaErrorInvalidValue;
+    CUtensorMap ta, tb;
+    GemmArgs g;
+    if (!make_operand(A, kBM, &ta, &g.a) || !make_operand(B, kBN, &tb, &g.b)) return cudaErrorInvalidValue;
+    g.M = (int32_t)A.mn; g.N = (int32_t)B.mn; g.Kc = (int32_t)A.kc;
+    g.m_tiles = (g.M + kBM - 1) / kBM;
+    g.n_tiles = (g.N + kBN - 1) / kBN;
+    g.order = order; g.group_m = group_m < 1 ? 1 : group_m;
+    g.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)A.major << 15) |
+              ((uint32_t)B.major << 16) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
+    g.e = e;
+    const int64_t tiles = (int64_t)g.m_tiles * g.n_tiles;
+    const int grid = (int)(tiles < num_sms ? tiles : num_sms);
+    switch (epi) {
+        case kEpiLse: return launch_gemm_epi<kEpiLse>(ta, tb, g, grid, st);
+        case kEpiDs: return launch_gemm_epi<kEpiDs>(ta, tb, g, grid, st);
+        case kEpiStoreBf16: return launch_gemm_epi<kEpiStoreBf16>(ta, tb, g, grid, st);
+        case kEpiAccum: return launch_gemm_epi<kEpiAccum>(ta, tb, g, grid, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace head
+}  // namespace awr
+
+// ================================================================== the a5 pass sequence
+namespace awr {
+
+using namespace head;
+
+static inline size_t up256(size_t x) { return (x + 255) / 256 * 256; }
+
+struct HeadWs {
+    float *zy, *row_lse, *row_coef, *row_gy;
+    float2* part;
+    __nv_bfloat16* ds;
+    float* dw_acc;
+    int64_t part_ld, ds_ld, panel_rows;
+    int n_vtiles, n_panels;
+    size_t total;
+};
+
+static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K) {
+    HeadWs w;
+    uint8_t* p = reinterpret_cast<uint8_t*>(base);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { void* r = p + off; off += up256(bytes); return r; };
+    const int64_t n_pad = (n_tok + kBM - 1) / kBM * kBM;
+    w.part_ld = n_pad;
+    w.ds_ld = (V + 7) / 8 * 8;
+    w.n_vtiles = (int)((V + kBN - 1) / kBN);
+    w.panel_rows = n_pad < kHeadPanelRows ? n_pad : kHeadPanelRows;
+    w.n_panels = n_tok > 0 ? (int)((n_tok + w.panel_rows - 1) / w.panel_rows) : 0;
+    w.zy = (float*)take((size_t)n_pad * 4);
+    w.row_lse = (float*)take((size_t)n_pad * 4);
+    w.row_coef = (float*)take((size_t)n_pad * 4);
+    w.row_gy = (float*)take((size_t)n_pad * 4);
+    w.part = (float2*)take((size_t)w.n_vtiles * n_pad * 8);
+    w.ds = (__nv_bfloat16*)take((size_t)w.panel_rows * w.ds_ld * 2);
+    w.dw_acc = (float*)take(w.n_panels > 1 ? (size_t)K * V * 4 : 0);
+    w.total = off;
+    return w;
+}
+
+size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K) {
+    return head_carve(nullptr, n_tok, V, K).total;
+}
+
+cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
+    if (c.n_tok <= 0) {
+        // no rows: the gradient of the head is zero
+        return cudaMemsetAsync(c.dw_head, 0, (size_t)c.K * c.V * 2, st);
+    }
+    const HeadWs w = head_carve(c.ws, c.n_tok, c.V, c.K);
+    const bool kv = c.w_layout == AWR_W_K_BY_V;
+    const __nv_bfloat16* H = reinterpret_cast<const __nv_bfloat16*>(c.hidden);
+    // W as the B operand of Z = H W (n = v, contraction = k) and of dH = dS W^T (n = k, contraction = v)
+    const OperandView w_fwd{c.w_head, c.V, c.K, kv ? c.V : c.K, kv ? kMajorMN : kMajorK};
+    const OperandView w_bwd{c.w_head, c.K, c.V, kv ? c.V : c.K, kv ? kMajorK : kMajorMN};
+    cudaError_t e = cudaMemsetAsync(w.zy, 0, (size_t)w.part_ld * 4, st);
+    if (e != cudaSuccess) return e;
+
+    // ---- pass F: log-sum-exp partials + gather over all rows
+    EpiArgs ea = {};
+    ea.part = w.part; ea.part_ld = w.part_ld; ea.zy = w.zy; ea.target_ids = c.rows->target_ids;
+    e = launch_gemm(kEpiLse, OperandView{H, c.n_tok, c.K, c.K, kMajorK}, w_fwd, 0, 32, ea, num_sms, st);
+    if (e != cudaSuccess) return e;
+
+    // ---- a3
+    {
+        const int warps = 8;
+        const unsigned blocks = (unsigned)((c.n_tok + warps - 1) / warps);
+        head_scalars_kernel<<<blocks, warps * 32, 0, st>>>(*c.rows, w.part, w.part_ld, w.n_vtiles,
+                                                           w.zy, w.row_lse, w.row_coef, w.row_gy);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+
+    // ---- row panels: dS, dhidden, dw_head
+    for (int p = 0; p < w.n_panels; ++p) {
+        const int64_t r0 = (int64_t)p * w.panel_rows;
+        const int64_t rows = (c.n_tok - r0 < w.panel_rows) ? (c.n_tok - r0) : w.panel_rows;
+        const __nv_bfloat16* Hp = H + r0 * c.K;
+        EpiArgs e1 = {};
+        e1.target_ids = c.rows->target_ids + r0; e1.row_lse = w.row_lse + r0;
+        e1.row_coef = w.row_coef + r0; e1.row_gy = w.row_gy + r0;
+        e1.ds = w.ds; e1.ds_ld = w.ds_ld;
+        e = launch_gemm(kEpiDs, OperandView{Hp, rows, c.K, c.K, kMajorK}, w_fwd, 0, 32, e1, num_sms, st);
+        if (e != cudaSuccess) return e;
+
+        EpiArgs e2 = {};
+        e2.out = reinterpret_cast<__nv_bfloat16*>(c.dhidden) + r0 * c.K; e2.out_ld = c.K;
+        e = launch_gemm(kEpiStoreBf16, OperandView{w.ds, rows, c.V, w.ds_ld, kMajorK}, w_bwd, 1, 1, e2,
+                        num_sms, st);
+        if (e != cudaSuccess) return e;
+
+        EpiArgs e3 = {};
+        e3.out = reinterpret_cast<__nv_bfloat16*>(c.dw_head); e3.acc = w.dw_acc;
+        e3.first_panel = p == 0; e3.last_panel = p == w.n_panels - 1;
+        const OperandView ht{Hp, c.K, rows, c.K, kMajorMN};          // H^T: m = k, contraction = t
+        const OperandView dst{w.ds, c.V, rows, w.ds_ld, kMajorMN};   // dS:  n = v, contraction = t
+        if (kv) {            // dw_head[k, v]
+            e3.out_ld = c.V;
+            e = launch_gemm(kEpiAccum, ht, dst, 0, 16, e3, num_sms, st);
+        } else {             // dw_head[v, k] = (dS^T H)[v, k]
+            e3.out_ld = c.K;
+            e = launch_gemm(kEpiAccum, dst, ht, 1, 1, e3, num_sms, st);
+        }
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+int head_launches(int64_t n_tok, int64_t V, int64_t K) {
+    const HeadWs w = head_carve(nullptr, n_tok, V, K);
+    return 2 + 3 * w.n_panels;
+}
+
+cudaError_t launch_gemm_bf16(const void* A, int a_major, int64_t lda, const void* B, int b_major,
+                             int64_t ldb, int64_t M, int64_t N, int64_t Kc, void* C, int64_t ldc,
+                             int num_sms, cudaStream_t st) {
+    EpiArgs e = {};
+    e.out = reinterpret_cast<__nv_bfloat16*>(C); e.out_ld = ldc;
+    return launch_gemm(kEpiStoreBf16, OperandView{A, M, Kc, lda, a_major}, OperandView{B, N, Kc, ldb, b_major},
+                       0, 8, e, num_sms, st);
+}
+
+}  // namespace awr

@@ -1,0 +1,158 @@
+// tcgen05 / TMEM / TMA GEMM engine of the fused LM-head path (a5, BASELINE.json config 4).
+//
+//   C[M, N] = A[M, Kc] * B[Kc, N],  bf16 x bf16 -> fp32 accumulators in tensor memory,
+//
+// with the epilogue applied to the accumulator tile while it is still on chip, so the logits
+// Z = H * W_head are never written to memory (reading A17: the fp32
+// accumulators go straight into the log-sum-exp).
+//
+// One persistent CTA per SM, 256 threads, warp-specialised:
+//   warp 0    TMA producer: cp.async.bulk.tensor (128-byte swizzle) into a 4-stage smem ring
+//   warp 1    MMA issuer: one lane issues tcgen05.mma.cta_group::1.kind::f16, 128 x 256 x 16,
+//             accumulating into one of two 256-column TMEM buffers
+//   warp 2    TMEM allocator (512 columns = two accumulator tiles)
+//   warps 4-7 epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 with tcgen05.ld, one
+//             accumulator row per thread, 32 columns at a time; runs while the MMA warp fills
+//             the other TMEM buffer with the next tile
+// Operands may be K-major (contraction index contiguous in memory) or MN-major (row / column
+// index contiguous); both are staged by TMA in the canonical 128-byte-swizzled UMMA layouts,
+// so H^T dS (both operands MN-major) needs no transposed copy of anything.
+#pragma once
+
+#include <cuda.h>
+
+#include "awr_common.cuh"
+
+namespace awr {
+namespace head {
+
+constexpr int kBM = 128;           // tile rows  (UMMA M)
+constexpr int kBN = 256;           // tile cols  (UMMA N)
+constexpr int kBK = 64;            // contraction elements per stage (= one 128-byte swizzle row)
+constexpr int kUmmaK = 16;         // contraction elements per tcgen05.mma (bf16)
+constexpr int kStages = 4;
+constexpr int kThreads = 256;
+constexpr int kABytes = kBM * kBK * 2;      // 16 KB
+constexpr int kBBytes = kBN * kBK * 2;      // 32 KB
+constexpr int kStageBytes = kABytes + kBBytes;
+constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment */ + 256 /* barriers */;
+constexpr int kTmemCols = 512;
+
+enum { kMajorK = 0, kMajorMN = 1 };
+enum { kEpiLse = 0,      // a2 on the tile: per-row (max, sum exp) partials + target gather
+       kEpiDs = 1,       // a4 on the tile: dS = c_t (exp(z - lse) - onehot) -> bf16 panel
+       kEpiStoreBf16 = 2,// C -> bf16 (dhidden)
+       kEpiAccum = 3 };  // C accumulated over row panels in fp32, bf16 on the last panel (dw_head)
+
+// How one operand is staged and described to the tensor core (all runtime values).
+struct Operand {
+    uint32_t major;       // kMajorK / kMajorMN
+    uint32_t boxes;       // TMA boxes per stage
+    uint32_t box_bytes;   // shared-memory bytes per box
+    uint32_t desc_lo;     // leading-byte-offset field of the smem descriptor (bits 16..29)
+    uint32_t desc_hi;     // stride-byte-offset, version 1, SWIZZLE_128B (upper 32 bits)
+    uint32_t k_step;      // added to the start-address field per UMMA_K step (16-byte units)
+};
+
+struct EpiArgs {
+    // kEpiLse
+    float2* part;              // [n_tiles][part_ld] (max, sum) of every row over one column tile
+    int64_t part_ld;
+    float* zy;                 // [M] gathered target logit (fp32 accumulator value)
+    const int32_t* target_ids; // [M] (kEpiLse, kEpiDs), already offset to row 0 of this GEMM
+    // kEpiDs
+    const float* row_lse;      // [M] log-sum-exp of the whole row
+    const float* row_coef;     // [M] c_t
+    const float* row_gy;       // [M] c_t (p_y - 1)
+    __nv_bfloat16* ds;         // [M, ds_ld]
+    int64_t ds_ld;
+    // kEpiStoreBf16 / kEpiAccum
+    __nv_bfloat16* out;        // [M, out_ld]
+    float* acc;                // [M, out_ld] fp32 running sum over panels
+    int64_t out_ld;
+    int32_t first_panel, last_panel;
+};
+
+struct GemmArgs {
+    int32_t M, N, Kc;          // logical sizes (rows / cols beyond them are masked)
+    int32_t m_tiles, n_tiles;
+    int32_t order;             // 0: m fastest inside groups of group_m row tiles; 1: n fastest
+    int32_t group_m;
+    uint32_t idesc;            // tcgen05 instruction descriptor
+    Operand a, b;
+    EpiArgs e;
+};
+
+// ------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1,
+                                            uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes "
+        "[%0], [%1, {%2, %3}], [%4];" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+}
+__device__ __forceinline__ void tc_fence_after() {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+}
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void tc_mma(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc,
+                                       uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// 32 lanes x 32 consecutive columns -> 32 registers per thread (thread = TMEM lane = tile row)
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
+    uint32_t r[32];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]),
+          "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]),
+          "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]),
+          "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]),
+          "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+}  // namespace head
+}  // namespace awr

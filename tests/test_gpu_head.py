@@ -1,0 +1,165 @@
+"""GPU parity of the fused LM-head path (a5, BASELINE.json config 4) against the fp64 oracle:
+the tcgen05 GEMM engine on its own (every operand-major combination, ragged sizes) and
+awr_loss_fwd_bwd_fused_head end to end.  Run on the B200 box: pytest -m gpu.
+
+Bars: token_lp 1e-4 absolute; loss as the logits path; clip_count,
+tok_traj exact; dhidden / dw_head: relative Frobenius error <= 5e-3 and max-abs error
+<= 1e-2 max|oracle| (proposed for config 4)."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_05597_b200 as A
+from gen import workloads as W
+from oracle import awr_oracle as O
+import parity_util as P
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+@pytest.fixture(autouse=True, scope="module")
+def _gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device (run them with gpurun)")
+    assert torch.cuda.get_device_capability(0)[0] == 10, "sm_100 only"
+    yield
+
+
+def _f64(t):
+    return t.float().cpu().numpy().astype(np.float64)
+
+
+# ------------------------------------------------------------------ the GEMM engine alone
+@pytest.mark.parametrize("a_major,b_major", [(0, 0), (0, 1), (1, 0), (1, 1)])
+@pytest.mark.parametrize("M,N,Kc", [(128, 256, 64), (256, 512, 256), (300, 1000, 200),
+                                    (131, 264, 72), (1000, 2048, 1096)])
+def test_gemm_engine_matches_fp64_matmul(a_major, b_major, M, N, Kc):
+    """C = A B for K-major and MN-major operands; sizes span one tile, several tiles, ragged
+    row / column / contraction tails (TMA zero fill).  The expected value is the float64
+    product of the same bf16 inputs; the result is rounded once to bf16."""
+    if a_major == 1 and M % 8:
+        M = (M + 7) // 8 * 8          # an MN-major operand needs a 16-byte-aligned row stride
+    if Kc % 8:
+        Kc = (Kc + 7) // 8 * 8
+    g = torch.Generator(DEV).manual_seed(M * 7 + N * 3 + Kc)
+    a = torch.randn(M, Kc, generator=g, device=DEV).to(torch.bfloat16)
+    b = torch.randn(Kc, N, generator=g, device=DEV).to(torch.bfloat16)
+    a_st = a if a_major == 0 else a.t().contiguous()          # stored [Kc, M]
+    b_st = b.t().contiguous() if b_major == 0 else b          # stored [N, Kc] / [Kc, N]
+    c = A.awr_gemm_bf16(a_st, b_st, a_major, b_major)
+    torch.cuda.synchronize()
+    ref = _f64(a) @ _f64(b)
+    got = _f64(c)
+    tol = 2.0 ** -8 * np.abs(ref) + 1e-3 * np.sqrt(Kc)
+    bad = np.abs(got - ref) > tol
+    assert not bad.any(), "%d bad entries, first at %s" % (bad.sum(), np.argwhere(bad)[0])
+
+
+# ------------------------------------------------------------------ a5 end to end
+def _head_batch(n_tok, K, V, seed, n_groups=4, group_size=4, masked_frac=0.0, lp_mode=None):
+    over = dict(n_groups=n_groups, group_size=group_size, n_tok=n_tok, V=V, hidden=K)
+    if lp_mode is not None:
+        over["lp_mode"] = lp_mode
+    w = W.workload(4, **over)
+    return W.make_batch(w, seed=seed, device=DEV, masked_frac=masked_frac)
+
+
+def _run_head(batch, w_layout=A.W_K_BY_V, **over):
+    params = dict(batch["params"])
+    params.update(over)
+    wh = batch["w_head"] if w_layout == A.W_K_BY_V else batch["w_head"].t().contiguous()
+    out = A.awr_loss_fwd_bwd_fused_head(batch["hidden"], wh, batch["target_ids"],
+                                        batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+                                        batch["traj_off"], batch["group_off"], batch["rewards"],
+                                        w_layout=w_layout, **params)
+    torch.cuda.synchronize()
+    return out
+
+
+def _oracle_head(batch, **over):
+    host = W.to_host(batch)
+    args, kw = W.oracle_args(host)
+    kw.update(over)
+    kw.pop("kernel", None)
+    return O.awr_loss_fwd_bwd_fused_head(*args, **kw)
+
+
+def _check_head(gpu, ora, w_layout):
+    assert int(gpu["err_word"][0]) == 0
+    assert np.array_equal(gpu["tok_traj"].cpu().numpy(), ora["tok_traj"].astype(np.int32))
+    lp = gpu["token_lp"].cpu().numpy().astype(np.float64)
+    assert np.abs(lp - ora["token_lp"]).max() <= P.LP_ATOL
+    assert int(gpu["clip_count"][0]) == ora["clip_count"]
+    tol = P.LOSS_RTOL * abs(ora["loss"]) + P.LOSS_COND_FLOOR * np.abs(ora["term"]).sum()
+    assert abs(float(gpu["loss"][0]) - ora["loss"]) <= tol
+    coef = gpu["tok_coef"].cpu().numpy()
+    assert np.array_equal(coef == 0, ora["coef"] == 0)
+    dh = _f64(gpu["dhidden"])
+    dw = _f64(gpu["dw_head"])
+    if w_layout == A.W_V_BY_K:
+        dw = dw.T
+    for name, got, ref in (("dhidden", dh, ora["dhidden"]), ("dw_head", dw, ora["dw_head"])):
+        fro = np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300)
+        mx = np.abs(got - ref).max() / max(np.abs(ref).max(), 1e-300)
+        assert fro <= 5e-3, "%s relative Frobenius error %.3e" % (name, fro)
+        assert mx <= 1e-2, "%s max-abs error %.3e of max|oracle|" % (name, mx)
+    # rows with c_t = 0 contribute nothing: their dhidden rows are exactly zero
+    zero_rows = ora["coef"] == 0
+    if zero_rows.any():
+        assert not gpu["dhidden"][torch.from_numpy(zero_rows).to(DEV)].any()
+
+
+@pytest.mark.parametrize("w_layout", [A.W_K_BY_V, A.W_V_BY_K])
+@pytest.mark.parametrize("n_tok,K,V", [(300, 128, 1000), (128, 64, 256), (517, 192, 2056)])
+def test_head_vs_oracle(n_tok, K, V, w_layout):
+    """Ragged row tile, ragged vocabulary tile, several contraction blocks; masked tokens; the
+    config-3 drift law so that clips and zero-advantage rows occur."""
+    batch = _head_batch(n_tok, K, V, seed=11, masked_frac=0.03, lp_mode="drift")
+    gpu = _run_head(batch, w_layout, stale_cap=2.0)
+    ora = _oracle_head(batch, stale_cap=2.0)
+    assert ora["clip_count"] > 0
+    _check_head(gpu, ora, w_layout)
+
+
+@pytest.mark.parametrize("norm", [A.NORM_CONST_K, A.NORM_PER_TRAJ])
+def test_head_several_panels(norm):
+    """More rows than one dS panel (4,736): dw_head accumulates across panels in fp32."""
+    batch = _head_batch(9700, 64, 512, seed=3, n_groups=8, group_size=8)
+    gpu = _run_head(batch, A.W_K_BY_V, normalizer=norm)
+    ora = _oracle_head(batch, normalizer=norm)
+    _check_head(gpu, ora, A.W_K_BY_V)
+    assert A.head_launches_per_call(9700, 512, 64) == 3 + 2 + 3 * 3
+
+
+def test_head_matches_logits_path():
+    """The same batch through the logits entry point (fp32 logits = H W computed in fp32) gives
+    the same integers and, within tolerance, the same per-token values."""
+    batch = _head_batch(384, 128, 1024, seed=5, lp_mode="drift")
+    gpu = _run_head(batch)
+    z = (batch["hidden"].float() @ batch["w_head"].float()).contiguous()
+    ref = A.awr_loss_fwd_bwd(z, batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+                             batch["step_off"], batch["traj_off"], batch["group_off"],
+                             batch["rewards"], **batch["params"])
+    torch.cuda.synchronize()
+    assert int(gpu["clip_count"][0]) == int(ref["clip_count"][0])
+    assert torch.equal(gpu["tok_traj"], ref["tok_traj"])
+    assert (gpu["token_lp"] - ref["token_lp"]).abs().max().item() <= 2e-5
+
+
+def test_head_empty_and_status_codes():
+    batch = _head_batch(128, 64, 256, seed=1)
+    with pytest.raises(A.AwrError) as ei:        # K not a multiple of 64
+        A.awr_loss_fwd_bwd_fused_head(batch["hidden"][:, :40].contiguous(),
+                                      batch["w_head"][:40].contiguous(), batch["target_ids"],
+                                      batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+                                      batch["traj_off"], batch["group_off"], batch["rewards"])
+    assert ei.value.status == -2
+    z = torch.zeros(0, dtype=torch.float32, device=DEV)
+    zi = torch.zeros(0, dtype=torch.int32, device=DEV)
+    off = torch.zeros(1, dtype=torch.int32, device=DEV)
+    out = A.awr_loss_fwd_bwd_fused_head(torch.zeros(0, 64, dtype=torch.bfloat16, device=DEV),
+                                        batch["w_head"], zi, z, z, off, off, off, z)
+    torch.cuda.synchronize()
+    assert float(out["loss"][0]) == 0.0 and int(out["clip_count"][0]) == 0
+    assert not out["dw_head"].any()
