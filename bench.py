@@ -360,6 +360,83 @@ def run_cuda(args):
     return 0
 
 
+def run_head(args):
+    """--config 4: the fused LM-head variant (a5).  A step = one awr_loss_fwd_bwd_fused_head call
+    (hidden [32,768, 2048] and W_head [2048, 151,936] in, loss / dhidden / dw_head out).  The
+    roofline is the tensor pipe: algorithmic flops 6 K V per token (logits, dH, dW); the path
+    executes 8 K V (the logits tile is recomputed for the backward), shown beside it."""
+    import torch
+
+    import paper_2606_05597_b200 as A
+    from gen import workloads as W
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: there is no CPU path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    init_dist("nccl")
+    over = {}
+    if args.n_tok:
+        over["n_tok"] = args.n_tok
+    w = W.workload(4, **over)
+    batch = W.make_batch(w, seed=1000 + rank, device=dev)
+    n_tok, V, K = batch["n_tok"], batch["V"], w.hidden
+    call = A.HeadLossCall(batch["hidden"], batch["w_head"], batch["target_ids"],
+                          batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+                          batch["traj_off"], batch["group_off"], batch["rewards"],
+                          want=("err_word",), **batch["params"])
+    stream = torch.cuda.current_stream(dev)
+    for _ in range(args.warmup):
+        call.run()
+    torch.cuda.synchronize(dev)
+    assert int(call.out["err_word"][0]) == 0
+    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(world)
+    with ClockSampler(local_rank) as clk:
+        t_beg.record(stream)
+        for _ in range(args.steps):
+            call.run()
+        t_end.record(stream)
+        torch.cuda.synchronize(dev)
+    barrier(world)
+    local_ms = t_beg.elapsed_time(t_end)
+    total_ms, total_tok = aggregate(local_ms, n_tok * args.steps, world, dev)
+    ms_per_step = total_ms / args.steps
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        with open(peaks_path) as f:
+            peak = float(json.load(f)["bf16_tflops_sustained"])
+        peak_src = "MEASURED_PEAKS.json bf16_tflops_sustained (of measured)"
+    else:
+        peak, peak_src = 1400.0, "B200_PROFILING.md fallback (of fallback)"
+    alg_flops = 6.0 * K * V * n_tok
+    achieved = alg_flops / (local_ms / args.steps / 1e3) / 1e12
+    if rank == 0:
+        line = {"metric": METRIC + " (fused LM-head variant)", "value": total_tok / (total_ms / 1e3),
+                "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "bf16 x bf16 -> f32 (TMEM)", "data": "synthetic",
+                "config": {"workload": "BASELINE.json configs[4] (%s)" % w.name,
+                           "n_tok_per_gpu": n_tok, "V": V, "K": K, "w_layout": "K_BY_V",
+                           "parallelism": "replicas only x%d" % world,
+                           "l2": "W_head (622 MB) + dS panels (1.4 GB) larger than L2, no flush"},
+                "roofline": {"bound": "tensor", "achieved": achieved, "peak": peak,
+                             "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                             "kernel": "head_gemm_kernel (4 epilogues), whole step",
+                             "algorithmic_flops_per_step": alg_flops,
+                             "executed_flops_per_step": alg_flops * 8 / 6,
+                             "executed_tflops": achieved * 8 / 6, "peak_source": peak_src},
+                "cpu_baseline": None, "e2e": None, "gpu_launches": call.launches * args.steps,
+                "clocks": clk.summary(), "loss": float(call.out["loss"][0]),
+                "clip_count": int(call.out["clip_count"][0])}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
 def load_traffic(cfg: int):
     """dram bytes (read + write) per launch of the row kernel from the committed `ncu --set full`
     capture (profiles/r1_traffic.txt, JSON text written by hand from the capture named there), or null."""
@@ -377,7 +454,7 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--n-tok", type=int, default=0, help="override the config's token count")
     ap.add_argument("--normalizer", type=int, default=None, choices=[0, 1])
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4"])
@@ -393,6 +470,8 @@ def main(argv=None):
                          "--nproc-per-node N --master-addr 127.0.0.1 bench.py --gpus N ...")
     if args.impl == "reference":
         return run_reference(args)
+    if args.config == 4:
+        return run_head(args)
     return run_cuda(args)
 
 
