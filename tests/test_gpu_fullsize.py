@@ -1,0 +1,145 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs 1-3: 40,960 / 65,536 / 131,072 rows of
+V = 151,936 bf16), in the launch configuration bench.py times (kernel = AUTO, device buffers).
+
+The fp64 oracle cannot do 10^10 exps in seconds, so per config:
+  * sampled rows (first, last, the rows around every cluster-schedule wrap, random ones,
+    masked / triggered / zero-advantage ones) go through the oracle's own step functions
+    (O2..O8 of oracle/awr_oracle.py, the same ones its awr_loss_fwd_bwd chains) and are compared
+    element by element at the usual bars;
+  * properties that hold at any size cover every row: tok_traj against the oracle's expansion
+    (exact), loss = -(sum of the per-token terms in token order) in fp64, clip_count = number of
+    trigger-flagged tokens implied by tok_coef / tok_term, all-bits-zero gradient rows exactly
+    where c_t = 0, every non-zero gradient row sums to ~0 (P8), and token_lp against the
+    library log-softmax (torch, fp32) on all rows.
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_05597_b200 as A
+from gen import workloads as W
+from oracle import awr_oracle as O
+import parity_util as P
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+N_SAMPLE = 160
+
+
+@pytest.fixture(autouse=True, scope="module")
+def _gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device (run them with gpurun)")
+    assert torch.cuda.get_device_capability(0)[0] == 10, "sm_100 only"
+    yield
+
+
+def _sample_rows(n_tok, extra, rng):
+    edge = [0, 1, n_tok - 2, n_tok - 1]
+    for c in (74, 148):                      # row schedule wraps of the persistent kernels
+        edge += [c - 1, c, c + 1, n_tok - c, n_tok - c - 1]
+    rows = np.unique(np.clip(np.concatenate([
+        np.asarray(edge), np.asarray(extra, dtype=np.int64),
+        rng.integers(0, n_tok, size=N_SAMPLE)]), 0, n_tok - 1))
+    return rows
+
+
+def _oracle_on_rows(batch, rows, params):
+    """Chain the oracle's step functions on a subset of rows (offsets are the full ones)."""
+    so, to, go = (batch[k].cpu().numpy() for k in ("step_off", "traj_off", "group_off"))
+    rewards = batch["rewards"].cpu().numpy()
+    seg = O.segment_expand(so, to, go)
+    adv = O.group_advantage(rewards, go, params.get("flags", 0))
+    scale = O.traj_scale(so, to, go, params["k_norm"], params["normalizer"],
+                         params.get("loss_scale", 1.0))
+    idx = torch.as_tensor(rows, device=DEV)
+    V = batch["V"]
+    z = batch["logits"][idx][:, :V].float().cpu().numpy()          # exact widening of bf16
+    y = batch["target_ids"][idx].cpu().numpy().astype(np.int64)
+    q = batch["prox_lp"][idx].cpu().numpy()
+    b = batch["behave_lp"][idx].cpu().numpy()
+    tt = seg["tok_traj"][rows]
+    valid = (y >= 0) & (y < V)
+    lse, lp, zy = O.token_logprob(z, y)
+    term, coef, trig, r, w = O.token_terms(lp, q, b, adv[tt], scale[tt], params["clip_eps"],
+                                           params["stale_cap"], valid)
+    g = O.dlogits_rows(z, y, lse, coef)
+    return dict(seg=seg, adv=adv, lp=lp, zy=zy, term=term, coef=coef, trig=trig, dlogits=g,
+                grad_rows=np.arange(rows.size))
+
+
+@pytest.mark.parametrize("cfg,in_place", [(1, False), (2, False), (3, True)])
+def test_full_size_sampled(cfg, in_place):
+    w = W.workload(cfg)
+    batch = W.make_batch(w, seed=100 + cfg, device=DEV, masked_frac=0.001 if cfg == 3 else 0.0)
+    n_tok, V = batch["n_tok"], batch["V"]
+    assert n_tok == w.n_tok and V == 151_936
+    params = dict(batch["params"])
+    rng = np.random.Generator(np.random.PCG64(cfg))
+    masked = torch.nonzero(batch["target_ids"] < 0).flatten().cpu().numpy()[:8]
+    rows = _sample_rows(n_tok, masked, rng)
+    ora = _oracle_on_rows(batch, rows, params)          # BEFORE the call: config 3 runs in place
+
+    assert A.select_kernel(V, batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RF
+    kw = dict(dlogits=batch["logits"]) if in_place else {}
+    if in_place:
+        ref_lp = None
+    out = A.awr_loss_fwd_bwd(batch["logits"], batch["target_ids"], batch["behave_lp"],
+                             batch["prox_lp"], batch["step_off"], batch["traj_off"],
+                             batch["group_off"], batch["rewards"], V=V, **params, **kw)
+    torch.cuda.synchronize()
+    assert int(out["err_word"][0]) == 0
+    dl = out["dlogits"]
+
+    # ---- all rows: integers and properties
+    assert np.array_equal(out["tok_traj"].cpu().numpy(), ora["seg"]["tok_traj"].astype(np.int32))
+    np.testing.assert_allclose(out["adv"].cpu().numpy(), ora["adv"], rtol=0, atol=4e-6)
+    term_all = out["tok_term"].double().cpu().numpy()
+    coef_all = out["tok_coef"].cpu().numpy()
+    loss_seq = 0.0
+    for t in term_all:                                   # token order, fp64 (O7)
+        loss_seq -= t
+    assert abs(float(out["loss"][0]) - loss_seq) <= 1e-6 * abs(loss_seq) + 1e-7 * np.abs(term_all).sum()
+    # a triggered token has a non-zero term and a zero coefficient (A5); masked and
+    # zero-advantage tokens have both zero
+    trig_all = (coef_all == 0) & (term_all != 0)
+    assert int(out["clip_count"][0]) == int(trig_all.sum())
+    if cfg == 3:
+        rate = trig_all.mean()
+        assert 0.10 < rate < 0.30, "config 3 should drive a clip-trigger rate of ~20 %%, got %g" % rate
+    zero_rows = torch.as_tensor(coef_all == 0, device=DEV)
+    for lo in range(0, n_tok, 4096):
+        blk = dl[lo:lo + 4096, :V]
+        nz = (blk.view(torch.int16) != 0).any(dim=1)
+        assert torch.equal(nz, ~zero_rows[lo:lo + 4096]), "zero pattern of the gradient rows"
+        s = blk.float().sum(dim=1)
+        mx = blk.float().abs().amax(dim=1)
+        assert bool((s.abs() <= 0.05 * mx + 1e-30).all()), "a gradient row does not sum to ~0 (P8)"
+
+    # ---- sampled rows against the oracle, element by element
+    sel = rows
+    lp_gpu = out["token_lp"].cpu().numpy()[sel].astype(np.float64)
+    assert np.abs(lp_gpu - ora["lp"]).max() <= P.LP_ATOL
+    assert np.array_equal(out["target_logit"].cpu().numpy()[sel], ora["zy"].astype(np.float32))
+    assert np.array_equal(coef_all[sel] == 0, ora["coef"] == 0)
+    cs = np.abs(ora["coef"]).max()
+    np.testing.assert_allclose(coef_all[sel], ora["coef"], rtol=2e-4, atol=1e-6 * cs + 1e-30)
+    ts = np.abs(ora["term"]).max()
+    np.testing.assert_allclose(term_all[sel], ora["term"], rtol=2e-4, atol=1e-6 * ts + 1e-30)
+    flags_gpu = (coef_all[sel] == 0) & (term_all[sel] != 0)
+    assert np.array_equal(flags_gpu, ora["trig"])
+    sub = dl[torch.as_tensor(sel, device=DEV)]
+    P.check_dlogits(sub, dict(dlogits=ora["dlogits"], grad_rows=ora["grad_rows"],
+                              coef=ora["coef"]), V)
+
+    # ---- all rows: token_lp against the library log-softmax (not possible after in-place)
+    if not in_place:
+        worst = 0.0
+        for lo in range(0, n_tok, 2048):
+            zf = batch["logits"][lo:lo + 2048, :V].float()
+            y = batch["target_ids"][lo:lo + 2048].long()
+            ok = y >= 0
+            lp = torch.log_softmax(zf, dim=1).gather(1, y.clamp(min=0)[:, None])[:, 0]
+            d = torch.where(ok, (lp - out["token_lp"][lo:lo + 2048]).abs(), torch.zeros_like(lp))
+            worst = max(worst, float(d.max()))
+        assert worst <= P.LP_ATOL
