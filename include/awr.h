@@ -76,8 +76,11 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_CLUSTER = 2,  /* row resident in the shared memory of a 2-CTA cluster (bf16) */
        AWR_KERNEL_CLUSTER_RF = 3, /* row resident in the register files of a 2-CTA cluster (bf16,
                                     16K <= V <= 163,840); shared memory is a TMA load FIFO */
-       AWR_KERNEL_CLUSTER_RF4 = 4 /* the same with a row quarter per CTA of a 4-CTA cluster and
-                                    two CTAs (of different rows) resident per SM */ };
+       AWR_KERNEL_CLUSTER_RF4 = 4, /* the same with a row quarter per CTA of a 4-CTA cluster and
+                                    two CTAs (of different rows) resident per SM */
+       /* fused-head entry points only (AUTO = AWR_KERNEL_HEAD_2CTA): */
+       AWR_KERNEL_HEAD_1CTA = 5, /* tcgen05 cta_group::1, 128 x 256 tiles, one CTA per SM */
+       AWR_KERNEL_HEAD_2CTA = 6  /* tcgen05 cta_group::2, 256 x 256 tiles on CTA pairs */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u };
 
@@ -200,17 +203,18 @@ AWR_API size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int
                                 int32_t n_traj, int32_t n_groups);
 
 /* Kernel launches one awr_loss_fwd_bwd_fused_head call enqueues for this shape. */
-AWR_API int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K);
+AWR_API int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K, int32_t kernel);
 
 /* The tensor-core engine of a5 on its own (tests, benchmarks): C[M, N] = A B, bf16 operands,
  * fp32 accumulation in tensor memory, bf16 row-major result C[m * ldc + n].  A is [M, Kc] and B
  * is [Kc, N] as matrices; *_major says which index is contiguous in memory:
  *   a_major 0: A[m * lda + k]   a_major 1: A[k * lda + m]
  *   b_major 0: B[n * ldb + k]   b_major 1: B[k * ldb + n]
- * lda, ldb, ldc and N multiples of 8; pointers 16-byte aligned; device pointers. */
+ * lda, ldb, ldc and N multiples of 8; pointers 16-byte aligned; device pointers.
+ * kernel: AWR_KERNEL_AUTO, AWR_KERNEL_HEAD_1CTA or AWR_KERNEL_HEAD_2CTA. */
 AWR_API int awr_gemm_bf16(const void* A, int32_t a_major, int64_t lda, const void* B, int32_t b_major,
                   int64_t ldb, int64_t M, int64_t N, int64_t Kc, void* C, int64_t ldc,
-                  void* stream);
+                  int32_t kernel, void* stream);
 
 AWR_API const char* awr_status_string(int status);
 AWR_API int awr_version(void);

@@ -21,6 +21,7 @@ NORM_CONST_K, NORM_PER_TRAJ = 0, 1
 FLAG_SAMPLE_STD = 1
 W_K_BY_V, W_V_BY_K = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_CLUSTER, KERNEL_CLUSTER_RF, KERNEL_CLUSTER_RF4 = 0, 1, 2, 3, 4
+KERNEL_HEAD_1CTA, KERNEL_HEAD_2CTA = 5, 6
 ERRBIT_STEP_OFF, ERRBIT_TRAJ_OFF, ERRBIT_GROUP_OFF, ERRBIT_TARGET_RANGE = 1, 2, 4, 8
 
 _vp = C.c_void_p
@@ -77,9 +78,9 @@ SYMBOLS = {
                                               C.POINTER(awr_head_outputs), _vp, C.c_size_t, _vp]),
     "awr_head_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int64, C.c_int64, C.c_int32,
                                               C.c_int32, C.c_int32]),
-    "awr_head_launches_per_call": (C.c_int, [C.c_int64, C.c_int64, C.c_int64]),
+    "awr_head_launches_per_call": (C.c_int, [C.c_int64, C.c_int64, C.c_int64, C.c_int32]),
     "awr_gemm_bf16": (C.c_int, [_vp, C.c_int32, C.c_int64, _vp, C.c_int32, C.c_int64, C.c_int64,
-                                C.c_int64, C.c_int64, _vp, C.c_int64, _vp]),
+                                C.c_int64, C.c_int64, _vp, C.c_int64, C.c_int32, _vp]),
     "awr_status_string": (C.c_char_p, [C.c_int]),
     "awr_version": (C.c_int, []),
     "awr_select_kernel": (C.c_int, [C.c_int64, C.c_int64, C.c_int32]),

@@ -258,8 +258,8 @@ def head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups) -> int:
     return int(load().awr_head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups))
 
 
-def head_launches_per_call(n_tok, V, K) -> int:
-    return int(load().awr_head_launches_per_call(n_tok, V, K))
+def head_launches_per_call(n_tok, V, K, kernel=KERNEL_AUTO) -> int:
+    return int(load().awr_head_launches_per_call(n_tok, V, K, int(kernel)))
 
 
 class HeadLossCall:
@@ -298,7 +298,6 @@ class HeadLossCall:
                                     _ptr(behave_lp), _ptr(prox_lp), _ptr(step_off), _ptr(traj_off),
                                     _ptr(group_off), _ptr(rewards), n_steps, n_traj, n_groups,
                                     int(w_layout))
-        params.pop("kernel", None)
         self.params = make_params(**params)
         o = dict(loss=torch.empty(1, dtype=torch.float32, device=dev),
                  dhidden=torch.empty_like(hidden), dw_head=torch.empty_like(w_head),
@@ -320,7 +319,7 @@ class HeadLossCall:
         self.workspace = workspace if workspace is not None else torch.empty(
             max(need, 256), dtype=torch.uint8, device=dev)
         self.ws_bytes = self.workspace.numel()
-        self.launches = head_launches_per_call(n_tok, V, K)
+        self.launches = head_launches_per_call(n_tok, V, K, self.params.kernel)
         self._keep = (hidden, w_head, target_ids, behave_lp, prox_lp, step_off, traj_off,
                       group_off, rewards)
 
@@ -339,7 +338,7 @@ def awr_loss_fwd_bwd_fused_head(hidden, w_head, target_ids, behave_lp, prox_lp, 
                         group_off, rewards, **kw).run(stream)
 
 
-def awr_gemm_bf16(a, b, a_major=0, b_major=0, stream=None):
+def awr_gemm_bf16(a, b, a_major=0, b_major=0, kernel=KERNEL_AUTO, stream=None):
     """C = A B on the tcgen05 engine of the fused head.  `a` is stored [M, Kc] (a_major 0) or
     [Kc, M] (a_major 1); `b` is stored [N, Kc] (b_major 0) or [Kc, N] (b_major 1)."""
     _req(a, torch.bfloat16, "a")
@@ -350,6 +349,6 @@ def awr_gemm_bf16(a, b, a_major=0, b_major=0, stream=None):
         raise ValueError("contraction lengths differ: %d vs %d" % (Kc, Kb))
     c = torch.empty((M, N), dtype=torch.bfloat16, device=a.device)
     rc = load().awr_gemm_bf16(_ptr(a), a_major, a.stride(0), _ptr(b), b_major, b.stride(0), M, N, Kc,
-                              _ptr(c), c.stride(0), _stream_ptr(stream, a.device))
+                              _ptr(c), c.stride(0), int(kernel), _stream_ptr(stream, a.device))
     check(rc, "awr_gemm_bf16")
     return c

@@ -66,7 +66,7 @@ static int check_params(const awr_params* p) {
     if (p->dual_clip_c > 1.f) return AWR_ERR_PARAM;          // Eq. (2) reserved
     if (p->normalizer != AWR_NORM_CONST_K && p->normalizer != AWR_NORM_PER_TRAJ) return AWR_ERR_PARAM;
     if (p->flags & ~(uint32_t)AWR_FLAG_SAMPLE_STD) return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER_RF4) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -76,7 +76,15 @@ static int check_segments(int64_t n_tok, int32_t n_steps, int32_t n_traj, int32_
     return AWR_OK;
 }
 
+// fused-head entry points: which tcgen05 shape (CTAs per tile) a kernel request means, or -1
+static int resolve_head_ctas(int requested) {
+    if (requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA) return 2;
+    if (requested == AWR_KERNEL_HEAD_1CTA) return 1;
+    return -1;
+}
+
 static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype) {
+    if (requested > AWR_KERNEL_CLUSTER_RF4) return -1;        // a fused-head kernel id
     const bool ok = rows_cluster_supported(V, ld, dtype);
     const bool ok_rf = rows_rf_supported(V, ld, dtype);
     if (requested == AWR_KERNEL_CLUSTER) return ok ? AWR_KERNEL_CLUSTER : -1;
@@ -246,8 +254,10 @@ size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_s
     return carve(nullptr, n_tok, n_traj).total + head_ws_bytes(n_tok, V, K);
 }
 
-int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K) {
-    return 3 + head_launches(n_tok, V, K);     // a0, a1, [F, scalars, 3 per panel], final sum
+int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K, int32_t kernel) {
+    const int ctas = resolve_head_ctas(kernel);
+    if (ctas < 0) return AWR_ERR_PARAM;
+    return 3 + head_launches(n_tok, V, K, ctas);     // a0, a1, [F, scalars, 3 per panel], final sum
 }
 
 int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
@@ -261,6 +271,7 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     if (b->w_layout != AWR_W_K_BY_V && b->w_layout != AWR_W_V_BY_K) return AWR_ERR_DTYPE;
     rc = check_params(p);
     if (rc) return rc;
+    if (resolve_head_ctas(p->kernel) < 0) return AWR_ERR_PARAM;
     if (!o->loss || !o->clip_count || !o->dw_head) return AWR_ERR_NULL;
     if (b->n_tok > 0 && (!o->token_lp || !o->dhidden)) return AWR_ERR_NULL;
     if (!b->step_off || !b->traj_off || !b->group_off || !b->w_head) return AWR_ERR_NULL;
@@ -304,6 +315,7 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     c.n_tok = b->n_tok; c.V = b->V; c.K = b->K; c.rows = &a;
     c.dhidden = o->dhidden; c.dw_head = o->dw_head;
     c.ws = reinterpret_cast<uint8_t*>(ws_ptr) + w.total;
+    c.ctas = resolve_head_ctas(p->kernel);
     if (e == cudaSuccess) e = launch_head(c, info.num_sms, st);
     if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count, st);
     if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
@@ -311,8 +323,11 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
 }
 
 int awr_gemm_bf16(const void* A, int32_t a_major, int64_t lda, const void* B, int32_t b_major,
-                  int64_t ldb, int64_t M, int64_t N, int64_t Kc, void* C, int64_t ldc, void* stream) {
+                  int64_t ldb, int64_t M, int64_t N, int64_t Kc, void* C, int64_t ldc, int32_t kernel,
+                  void* stream) {
     if (!A || !B || !C) return AWR_ERR_NULL;
+    const int ctas = resolve_head_ctas(kernel);
+    if (ctas < 0) return AWR_ERR_PARAM;
     if (M <= 0 || N <= 0 || Kc <= 0 || M > 0x7fffffffLL || N > 0x7fffffffLL || Kc > 0x7fffffffLL) return AWR_ERR_SHAPE;
     if ((a_major != 0 && a_major != 1) || (b_major != 0 && b_major != 1)) return AWR_ERR_DTYPE;
     if (lda % 8 || ldb % 8 || ldc % 8 || N % 8) return AWR_ERR_ALIGN;
@@ -322,7 +337,7 @@ int awr_gemm_bf16(const void* A, int32_t a_major, int64_t lda, const void* B, in
     if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
     if (info.major != 10) return AWR_ERR_ARCH;
     cudaError_t e = launch_gemm_bf16(A, a_major, lda, B, b_major, ldb, M, N, Kc, C, ldc, info.num_sms,
-                                     reinterpret_cast<cudaStream_t>(stream));
+                                     ctas, reinterpret_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
     return AWR_OK;
 }

@@ -28,10 +28,13 @@ __device__ __forceinline__ void tile_coords(const GemmArgs& g, int tile, int& m_
     }
 }
 
-template <int EPI>
+template <int EPI, int CTAS>
 __global__ void __launch_bounds__(kThreads, 1)
 head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                  const __grid_constant__ CUtensorMap tmap_b, const GemmArgs g) {
+    using G = Geo<CTAS>;
+    constexpr int kStages = G::kStages;
+    constexpr int kStageBytes = G::kStageBytes;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bars = smem_base + kStages * kStageBytes;
@@ -48,6 +51,10 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
     const int lane = threadIdx.x & 31;
     const int num_tiles = g.m_tiles * g.n_tiles;
     const int num_kb = (g.Kc + kBK - 1) / kBK;
+    // CTAS = 2: both CTAs of a pair walk the same tile sequence; rank 0 is the leader
+    const uint32_t rank = CTAS == 2 ? cluster_rank() : 0u;
+    const int tile0 = CTAS == 2 ? (int)cluster_id() : (int)blockIdx.x;
+    const int tile_step = CTAS == 2 ? (int)num_clusters() : (int)gridDim.x;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
@@ -55,56 +62,65 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4 * CTAS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
-                     "n"(kTmemCols)
-                     : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        if constexpr (CTAS == 1) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
+                         "n"(kTmemCols)
+                         : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
+                         "n"(kTmemCols)
+                         : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        }
     }
     tc_fence_before();
-    __syncthreads();
+    if constexpr (CTAS == 2) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     if (warp == 0) {
-        // ===================== TMA producer
+        // ===================== TMA producer (every CTA stages its own rows of A and columns of B)
         if (lane == 0) {
             int stage = 0;
             uint32_t phase = 0;
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            for (int tile = tile0; tile < num_tiles; tile += tile_step) {
                 int m_blk, n_blk;
                 tile_coords(g, tile, m_blk, n_blk);
-                const int m0 = m_blk * kBM, n0 = n_blk * kBN;
+                const int m0 = m_blk * G::kTileM + (int)rank * kBM;
+                const int n0 = n_blk * kBN + (int)rank * G::kLoadN;
                 for (int kb = 0; kb < num_kb; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = smem_base + stage * kStageBytes;
                     const uint32_t sb = sa + kABytes;
-                    const uint32_t bar = full_bar(stage);
-                    mbar_expect_tx(bar, kStageBytes);
+                    uint32_t bar = full_bar(stage);
+                    if (rank == 0) mbar_expect_tx(bar, kStageBytes * CTAS);
+                    if constexpr (CTAS == 2) bar = map_to_cta(bar, 0);
                     const int k0 = kb * kBK;
                     for (uint32_t j = 0; j < g.a.boxes; ++j) {
-                        if (g.a.major == kMajorK) tma_load_2d(sa, &tmap_a, k0, m0, bar);
-                        else tma_load_2d(sa + j * g.a.box_bytes, &tmap_a, m0 + 64 * (int)j, k0, bar);
+                        if (g.a.major == kMajorK) tma_load_2d<CTAS>(sa, &tmap_a, k0, m0, bar);
+                        else tma_load_2d<CTAS>(sa + j * g.a.box_bytes, &tmap_a, m0 + 64 * (int)j, k0, bar);
                     }
                     for (uint32_t j = 0; j < g.b.boxes; ++j) {
-                        if (g.b.major == kMajorK) tma_load_2d(sb, &tmap_b, k0, n0, bar);
-                        else tma_load_2d(sb + j * g.b.box_bytes, &tmap_b, n0 + 64 * (int)j, k0, bar);
+                        if (g.b.major == kMajorK) tma_load_2d<CTAS>(sb, &tmap_b, k0, n0, bar);
+                        else tma_load_2d<CTAS>(sb + j * g.b.box_bytes, &tmap_b, n0 + 64 * (int)j, k0, bar);
                     }
                     if (++stage == kStages) { stage = 0; phase ^= 1u; }
                 }
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer
-        if (lane == 0) {
+        // ===================== MMA issuer (leader CTA only)
+        if (lane == 0 && rank == 0) {
             int stage = 0;
             uint32_t phase = 0;
             int as = 0;
             uint32_t aphase = 0;
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            for (int tile = tile0; tile < num_tiles; tile += tile_step) {
                 mbar_wait(tempty_bar(as), aphase ^ 1u);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)as * kBN;
@@ -121,12 +137,12 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                             ((uint64_t)g.a.desc_hi << 32) | (uint64_t)(a_lo + k * g.a.k_step);
                         const uint64_t bdesc =
                             ((uint64_t)g.b.desc_hi << 32) | (uint64_t)(b_lo + k * g.b.k_step);
-                        tc_mma(d_tmem, adesc, bdesc, g.idesc, (uint32_t)((kb | k) != 0));
+                        tc_mma<CTAS>(d_tmem, adesc, bdesc, g.idesc, (uint32_t)((kb | k) != 0));
                     }
-                    tc_commit(empty_bar(stage));          // smem slot free once these MMAs retire
+                    tc_commit<CTAS>(empty_bar(stage));    // smem slot free once these MMAs retire
                     if (++stage == kStages) { stage = 0; phase ^= 1u; }
                 }
-                tc_commit(tfull_bar(as));                 // accumulator tile complete
+                tc_commit<CTAS>(tfull_bar(as));           // accumulator tile complete
                 if (++as == 2) { as = 0; aphase ^= 1u; }
             }
         }
@@ -135,10 +151,10 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
         const int q = warp & 3;                           // TMEM lane quarter of this warp
         int as = 0;
         uint32_t aphase = 0;
-        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        for (int tile = tile0; tile < num_tiles; tile += tile_step) {
             int m_blk, n_blk;
             tile_coords(g, tile, m_blk, n_blk);
-            const int row = m_blk * kBM + q * 32 + lane;
+            const int row = m_blk * G::kTileM + (int)rank * kBM + q * 32 + lane;
             const int n0 = n_blk * kBN;
             const bool row_ok = row < g.M;
             mbar_wait(tfull_bar(as), aphase);
@@ -257,18 +273,27 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(tempty_bar(as));
+            if (lane == 0) {
+                // the accumulator buffer is released on the leader's barrier (the MMA issuer's)
+                if constexpr (CTAS == 2) mbar_arrive_cluster(map_to_cta(tempty_bar(as), 0));
+                else mbar_arrive(tempty_bar(as));
+            }
             if (++as == 2) { as = 0; aphase ^= 1u; }
         }
     }
 
     tc_fence_before();
-    __syncthreads();
+    if constexpr (CTAS == 2) cluster_sync_all(); else __syncthreads();
     if (warp == 2) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base),
-                     "n"(kTmemCols)
-                     : "memory");
+        if constexpr (CTAS == 1)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base),
+                         "n"(kTmemCols)
+                         : "memory");
+        else
+            asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base),
+                         "n"(kTmemCols)
+                         : "memory");
     }
 }
 
@@ -369,44 +394,61 @@ static bool make_operand(const OperandView& v, int tile_mn, CUtensorMap* map, Op
     return r == CUDA_SUCCESS;
 }
 
-template <int EPI>
+template <int EPI, int CTAS>
 static cudaError_t launch_gemm_epi(const CUtensorMap& ta, const CUtensorMap& tb, const GemmArgs& g,
                                    int grid, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(head_gemm_kernel<EPI>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+        cudaError_t e = cudaFuncSetAttribute(head_gemm_kernel<EPI, CTAS>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             Geo<CTAS>::kSmemBytes);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    head_gemm_kernel<EPI><<<grid, kThreads, kSmemBytes, st>>>(ta, tb, g);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CTAS;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(kThreads, 1, 1);
+    cfg.dynamicSmemBytes = Geo<CTAS>::kSmemBytes;
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, head_gemm_kernel<EPI, CTAS>, ta, tb, g);
 }
 
-// C[M, N] = A * B with epilogue `epi`; `order` / `group_m` pick the tile raster.
+// C[M, N] = A * B with epilogue `epi`; `order` / `group_m` pick the tile raster (group_m in row
+// tiles of 128 * ctas rows); ctas = 1: one CTA per tile, 2: a CTA pair per 256-row tile.
 static cudaError_t launch_gemm(int epi, const OperandView& A, const OperandView& B, int order,
-                               int group_m, const EpiArgs& e, int num_sms, cudaStream_t st) {
+                               int group_m, const EpiArgs& e, int num_sms, int ctas, cudaStream_t st) {
     if (A.mn <= 0 || B.mn <= 0 || A.kc <= 0) return cudaSuccess;
     if (A.kc != B.kc) return cudaErrorInvalidValue;
     CUtensorMap ta, tb;
     GemmArgs g;
-    if (!make_operand(A, kBM, &ta, &g.a) || !make_operand(B, kBN, &tb, &g.b)) return cudaErrorInvalidValue;
+    if (!make_operand(A, kBM, &ta, &g.a) || !make_operand(B, kBN / ctas, &tb, &g.b)) return cudaErrorInvalidValue;
+    const int tile_m = kBM * ctas;
     g.M = (int32_t)A.mn; g.N = (int32_t)B.mn; g.Kc = (int32_t)A.kc;
-    g.m_tiles = (g.M + kBM - 1) / kBM;
+    g.m_tiles = (g.M + tile_m - 1) / tile_m;
     g.n_tiles = (g.N + kBN - 1) / kBN;
     g.order = order; g.group_m = group_m < 1 ? 1 : group_m;
     g.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)A.major << 15) |
-              ((uint32_t)B.major << 16) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
+              ((uint32_t)B.major << 16) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)(tile_m >> 4) << 24);
     g.e = e;
     const int64_t tiles = (int64_t)g.m_tiles * g.n_tiles;
-    const int grid = (int)(tiles < num_sms ? tiles : num_sms);
+    const int slots = num_sms / ctas;                    // persistent CTAs / CTA pairs
+    const int grid = (int)(tiles < slots ? tiles : slots) * ctas;
+#define AWR_HEAD_CASE(E)                                                            \
+    case E:                                                                         \
+        return ctas == 2 ? launch_gemm_epi<E, 2>(ta, tb, g, grid, st)               \
+                         : launch_gemm_epi<E, 1>(ta, tb, g, grid, st);
     switch (epi) {
-        case kEpiLse: return launch_gemm_epi<kEpiLse>(ta, tb, g, grid, st);
-        case kEpiDs: return launch_gemm_epi<kEpiDs>(ta, tb, g, grid, st);
-        case kEpiStoreBf16: return launch_gemm_epi<kEpiStoreBf16>(ta, tb, g, grid, st);
-        case kEpiAccum: return launch_gemm_epi<kEpiAccum>(ta, tb, g, grid, st);
+        AWR_HEAD_CASE(kEpiLse) AWR_HEAD_CASE(kEpiDs) AWR_HEAD_CASE(kEpiStoreBf16) AWR_HEAD_CASE(kEpiAccum)
         default: return cudaErrorInvalidValue;
     }
+#undef AWR_HEAD_CASE
 }
 
 }  // namespace head
@@ -429,7 +471,12 @@ struct HeadWs {
     size_t total;
 };
 
-static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K) {
+// Rows per panel: the dhidden GEMM of a panel has (rows / tile rows) x (K / 256) tiles of V-long
+// contractions, so the panel is sized to fill whole waves of the persistent grid at K = 2048:
+// 37 x 8 = 296 tiles = 2 x 148 CTAs (ctas = 1) or 4 x 74 CTA pairs (ctas = 2).
+static int64_t head_panel_rows(int ctas) { return ctas == 2 ? 2 * kHeadPanelRows : kHeadPanelRows; }
+
+static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ctas) {
     HeadWs w;
     uint8_t* p = reinterpret_cast<uint8_t*>(base);
     size_t off = 0;
@@ -438,7 +485,7 @@ static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K) {
     w.part_ld = n_pad;
     w.ds_ld = (V + 7) / 8 * 8;
     w.n_vtiles = (int)((V + kBN - 1) / kBN);
-    w.panel_rows = n_pad < kHeadPanelRows ? n_pad : kHeadPanelRows;
+    w.panel_rows = n_pad < head_panel_rows(ctas) ? n_pad : head_panel_rows(ctas);
     w.n_panels = n_tok > 0 ? (int)((n_tok + w.panel_rows - 1) / w.panel_rows) : 0;
     w.zy = (float*)take((size_t)n_pad * 4);
     w.row_lse = (float*)take((size_t)n_pad * 4);
@@ -452,7 +499,9 @@ static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K) {
 }
 
 size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K) {
-    return head_carve(nullptr, n_tok, V, K).total;
+    const size_t a = head_carve(nullptr, n_tok, V, K, 1).total;
+    const size_t b = head_carve(nullptr, n_tok, V, K, 2).total;
+    return a > b ? a : b;
 }
 
 cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
@@ -460,7 +509,9 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         // no rows: the gradient of the head is zero
         return cudaMemsetAsync(c.dw_head, 0, (size_t)c.K * c.V * 2, st);
     }
-    const HeadWs w = head_carve(c.ws, c.n_tok, c.V, c.K);
+    const int ctas = c.ctas == 1 ? 1 : 2;
+    const int gm = 4096 / (kBM * ctas);               // raster groups of 4096 rows
+    const HeadWs w = head_carve(c.ws, c.n_tok, c.V, c.K, ctas);
     const bool kv = c.w_layout == AWR_W_K_BY_V;
     const __nv_bfloat16* H = reinterpret_cast<const __nv_bfloat16*>(c.hidden);
     // W as the B operand of Z = H W (n = v, contraction = k) and of dH = dS W^T (n = k, contraction = v)
@@ -472,7 +523,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     // ---- pass F: log-sum-exp partials + gather over all rows
     EpiArgs ea = {};
     ea.part = w.part; ea.part_ld = w.part_ld; ea.zy = w.zy; ea.target_ids = c.rows->target_ids;
-    e = launch_gemm(kEpiLse, OperandView{H, c.n_tok, c.K, c.K, kMajorK}, w_fwd, 0, 32, ea, num_sms, st);
+    e = launch_gemm(kEpiLse, OperandView{H, c.n_tok, c.K, c.K, kMajorK}, w_fwd, 0, gm, ea, num_sms, ctas, st);
     if (e != cudaSuccess) return e;
 
     // ---- a3
@@ -494,13 +545,13 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         e1.target_ids = c.rows->target_ids + r0; e1.row_lse = w.row_lse + r0;
         e1.row_coef = w.row_coef + r0; e1.row_gy = w.row_gy + r0;
         e1.ds = w.ds; e1.ds_ld = w.ds_ld;
-        e = launch_gemm(kEpiDs, OperandView{Hp, rows, c.K, c.K, kMajorK}, w_fwd, 0, 32, e1, num_sms, st);
+        e = launch_gemm(kEpiDs, OperandView{Hp, rows, c.K, c.K, kMajorK}, w_fwd, 0, gm, e1, num_sms, ctas, st);
         if (e != cudaSuccess) return e;
 
         EpiArgs e2 = {};
         e2.out = reinterpret_cast<__nv_bfloat16*>(c.dhidden) + r0 * c.K; e2.out_ld = c.K;
         e = launch_gemm(kEpiStoreBf16, OperandView{w.ds, rows, c.V, w.ds_ld, kMajorK}, w_bwd, 1, 1, e2,
-                        num_sms, st);
+                        num_sms, ctas, st);
         if (e != cudaSuccess) return e;
 
         EpiArgs e3 = {};
@@ -510,28 +561,29 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         const OperandView dst{w.ds, c.V, rows, w.ds_ld, kMajorMN};   // dS:  n = v, contraction = t
         if (kv) {            // dw_head[k, v]
             e3.out_ld = c.V;
-            e = launch_gemm(kEpiAccum, ht, dst, 0, 16, e3, num_sms, st);
+            e = launch_gemm(kEpiAccum, ht, dst, 0, 16 / ctas, e3, num_sms, ctas, st);
         } else {             // dw_head[v, k] = (dS^T H)[v, k]
             e3.out_ld = c.K;
-            e = launch_gemm(kEpiAccum, dst, ht, 1, 1, e3, num_sms, st);
+            e = launch_gemm(kEpiAccum, dst, ht, 1, 1, e3, num_sms, ctas, st);
         }
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
 }
 
-int head_launches(int64_t n_tok, int64_t V, int64_t K) {
-    const HeadWs w = head_carve(nullptr, n_tok, V, K);
+int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas) {
+    const HeadWs w = head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2);
     return 2 + 3 * w.n_panels;
 }
 
 cudaError_t launch_gemm_bf16(const void* A, int a_major, int64_t lda, const void* B, int b_major,
                              int64_t ldb, int64_t M, int64_t N, int64_t Kc, void* C, int64_t ldc,
-                             int num_sms, cudaStream_t st) {
+                             int num_sms, int ctas, cudaStream_t st) {
     EpiArgs e = {};
     e.out = reinterpret_cast<__nv_bfloat16*>(C); e.out_ld = ldc;
+    ctas = ctas == 1 ? 1 : 2;
     return launch_gemm(kEpiStoreBf16, OperandView{A, M, Kc, lda, a_major}, OperandView{B, N, Kc, ldb, b_major},
-                       0, 8, e, num_sms, st);
+                       0, 8 / ctas, e, num_sms, ctas, st);
 }
 
 }  // namespace awr

@@ -7,13 +7,25 @@
 // accumulators go straight into the log-sum-exp).
 //
 // One persistent CTA per SM, 256 threads, warp-specialised:
-//   warp 0    TMA producer: cp.async.bulk.tensor (128-byte swizzle) into a 4-stage smem ring
-//   warp 1    MMA issuer: one lane issues tcgen05.mma.cta_group::1.kind::f16, 128 x 256 x 16,
-//             accumulating into one of two 256-column TMEM buffers
+//   warp 0    TMA producer: cp.async.bulk.tensor (128-byte swizzle) into a smem ring
+//   warp 1    MMA issuer: one lane issues tcgen05.mma.kind::f16, accumulating into one of two
+//             256-column TMEM buffers
 //   warp 2    TMEM allocator (512 columns = two accumulator tiles)
 //   warps 4-7 epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 with tcgen05.ld, one
 //             accumulator row per thread, 32 columns at a time; runs while the MMA warp fills
 //             the other TMEM buffer with the next tile
+// Two shapes of the same kernel (template parameter CTAS):
+//   CTAS = 1  cta_group::1, tile 128 x 256, every CTA stages A 128 x 64 + B 256 x 64 per stage
+//             (48 KB, 4 stages).  The tensor core reads 96 B/clk of operands from the shared
+//             memory that TMA is filling at the same rate: the 128 B/clk port is the limit
+//             (measured: tensor pipe 50-60 % active).
+//   CTAS = 2  cta_group::2 (CTA pair on one TPC), tile 256 x 256: each CTA stages its 128 rows
+//             of A and its 128 columns of B (32 KB, 6 stages); the pair's tensor cores share
+//             the B halves, so each SM's shared memory serves 64 B/clk of operand reads and
+//             takes 64 B/clk of fills.  The leader CTA issues the MMAs for both; all TMA
+//             completions land on the leader's "full" barrier, tcgen05.commit multicasts the
+//             "empty" and "accumulator ready" signals to both CTAs, and the epilogue warps of
+//             both CTAs release the accumulator on the leader's barrier.
 // Operands may be K-major (contraction index contiguous in memory) or MN-major (row / column
 // index contiguous); both are staged by TMA in the canonical 128-byte-swizzled UMMA layouts,
 // so H^T dS (both operands MN-major) needs no transposed copy of anything.
@@ -30,13 +42,21 @@ constexpr int kBM = 128;           // tile rows  (UMMA M)
 constexpr int kBN = 256;           // tile cols  (UMMA N)
 constexpr int kBK = 64;            // contraction elements per stage (= one 128-byte swizzle row)
 constexpr int kUmmaK = 16;         // contraction elements per tcgen05.mma (bf16)
-constexpr int kStages = 4;
 constexpr int kThreads = 256;
-constexpr int kABytes = kBM * kBK * 2;      // 16 KB
-constexpr int kBBytes = kBN * kBK * 2;      // 32 KB
-constexpr int kStageBytes = kABytes + kBBytes;
-constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment */ + 256 /* barriers */;
+constexpr int kABytes = kBM * kBK * 2;      // 16 KB: 128 rows of A per CTA in both shapes
 constexpr int kTmemCols = 512;
+constexpr int kMaxStages = 8;
+
+template <int CTAS>
+struct Geo {
+    static constexpr int kTileM = kBM * CTAS;            // tile rows per CTA / CTA pair
+    static constexpr int kLoadN = kBN / CTAS;            // B columns staged by one CTA
+    static constexpr int kBBytes = kLoadN * kBK * 2;     // 32 KB / 16 KB
+    static constexpr int kStageBytes = kABytes + kBBytes;
+    static constexpr int kStages = CTAS == 1 ? 4 : 6;
+    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment */ + 256 /* barriers */;
+};
+static_assert(Geo<2>::kStages <= kMaxStages && Geo<2>::kSmemBytes <= 232448, "shared memory");
 
 enum { kMajorK = 0, kMajorMN = 1 };
 enum { kEpiLse = 0,      // a2 on the tile: per-row (max, sum exp) partials + target gather
@@ -109,12 +129,50 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "}\n" ::"r"(bar), "r"(parity)
         : "memory");
 }
+// CTAS = 2: `bar` is the shared::cluster address of the LEADER's barrier (map_to_cta(.., 0));
+// the data still lands in the executing CTA's shared memory.
+template <int CTAS>
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1,
                                             uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes "
-        "[%0], [%1, {%2, %3}], [%4];" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
-        : "memory");
+    if constexpr (CTAS == 1) {
+        asm volatile(
+            "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes "
+            "[%0], [%1, {%2, %3}], [%4];" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
+            : "memory");
+    } else {
+        asm volatile(
+            "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes "
+            "[%0], [%1, {%2, %3}], [%4];" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
+            : "memory");
+    }
+}
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t local_addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
+                 : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_rank() {
+    uint32_t r;
+    asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t cluster_id() {
+    uint32_t r;
+    asm("mov.u32 %0, %%clusterid.x;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t num_clusters() {
+    uint32_t r;
+    asm("mov.u32 %0, %%nclusterid.x;" : "=r"(r));
+    return r;
 }
 __device__ __forceinline__ void tc_fence_before() {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -122,19 +180,39 @@ __device__ __forceinline__ void tc_fence_before() {
 __device__ __forceinline__ void tc_fence_after() {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 }
+// CTAS = 2: the arrive is multicast to the barrier at the same offset in both CTAs of the pair.
+template <int CTAS>
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
-                 : "memory");
+    if constexpr (CTAS == 1) {
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
+                     : "memory");
+    } else {
+        asm volatile(
+            "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 "
+            "[%0], %1;" ::"r"(bar), "h"((uint16_t)3)
+            : "memory");
+    }
 }
+template <int CTAS>
 __device__ __forceinline__ void tc_mma(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc,
                                        uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
-        "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
+    if constexpr (CTAS == 1) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "setp.ne.b32 p, %4, 0;\n"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+            "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+            : "memory");
+    } else {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "setp.ne.b32 p, %4, 0;\n"
+            "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n"
+            "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+            : "memory");
+    }
 }
 // 32 lanes x 32 consecutive columns -> 32 registers per thread (thread = TMEM lane = tile row)
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {

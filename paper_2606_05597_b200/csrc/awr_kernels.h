@@ -33,7 +33,7 @@ cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, int cluster_size, cuda
 
 // a5: fused LM head (awr_head.cu).  `rows` carries the per-token inputs / outputs of a3
 // (its logits / dlogits members are unused); `ws` is head_ws_bytes() of device memory.
-constexpr int64_t kHeadPanelRows = 4736;   // 37 row tiles: dhidden panels are 2 full waves of 148
+constexpr int64_t kHeadPanelRows = 4736;   // 37 row tiles of 128; doubled for CTA pairs (awr_head.cu)
 struct HeadCall {
     const void* hidden;
     const void* w_head;
@@ -43,14 +43,15 @@ struct HeadCall {
     void* dhidden;
     void* dw_head;
     void* ws;
+    int ctas;        // 1: cta_group::1 tiles of 128 rows; anything else: CTA pairs, 256-row tiles
 };
 size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K);
-int head_launches(int64_t n_tok, int64_t V, int64_t K);
+int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas);
 cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st);
 // C[M, N] (bf16, row-major, ldc) = A B on the tcgen05 engine; majors: 0 = contraction index
 // contiguous, 1 = row (A) / column (B) index contiguous.
 cudaError_t launch_gemm_bf16(const void* A, int a_major, int64_t lda, const void* B, int b_major,
                              int64_t ldb, int64_t M, int64_t N, int64_t Kc, void* C, int64_t ldc,
-                             int num_sms, cudaStream_t st);
+                             int num_sms, int ctas, cudaStream_t st);
 
 }  // namespace awr

@@ -30,11 +30,15 @@ def _f64(t):
     return t.float().cpu().numpy().astype(np.float64)
 
 
+HEAD_KERNELS = [A.KERNEL_HEAD_1CTA, A.KERNEL_HEAD_2CTA]
+
+
 # ------------------------------------------------------------------ the GEMM engine alone
+@pytest.mark.parametrize("kernel", HEAD_KERNELS)
 @pytest.mark.parametrize("a_major,b_major", [(0, 0), (0, 1), (1, 0), (1, 1)])
 @pytest.mark.parametrize("M,N,Kc", [(128, 256, 64), (256, 512, 256), (300, 1000, 200),
-                                    (131, 264, 72), (1000, 2048, 1096)])
-def test_gemm_engine_matches_fp64_matmul(a_major, b_major, M, N, Kc):
+                                    (131, 264, 72), (1000, 2048, 1096), (2304, 1280, 520)])
+def test_gemm_engine_matches_fp64_matmul(a_major, b_major, M, N, Kc, kernel):
     """C = A B for K-major and MN-major operands; sizes span one tile, several tiles, ragged
     row / column / contraction tails (TMA zero fill).  The expected value is the float64
     product of the same bf16 inputs; the result is rounded once to bf16."""
@@ -47,7 +51,7 @@ def test_gemm_engine_matches_fp64_matmul(a_major, b_major, M, N, Kc):
     b = torch.randn(Kc, N, generator=g, device=DEV).to(torch.bfloat16)
     a_st = a if a_major == 0 else a.t().contiguous()          # stored [Kc, M]
     b_st = b.t().contiguous() if b_major == 0 else b          # stored [N, Kc] / [Kc, N]
-    c = A.awr_gemm_bf16(a_st, b_st, a_major, b_major)
+    c = A.awr_gemm_bf16(a_st, b_st, a_major, b_major, kernel=kernel)
     torch.cuda.synchronize()
     ref = _f64(a) @ _f64(b)
     got = _f64(c)
@@ -110,26 +114,42 @@ def _check_head(gpu, ora, w_layout):
         assert not gpu["dhidden"][torch.from_numpy(zero_rows).to(DEV)].any()
 
 
+@pytest.mark.parametrize("kernel", HEAD_KERNELS)
 @pytest.mark.parametrize("w_layout", [A.W_K_BY_V, A.W_V_BY_K])
 @pytest.mark.parametrize("n_tok,K,V", [(300, 128, 1000), (128, 64, 256), (517, 192, 2056)])
-def test_head_vs_oracle(n_tok, K, V, w_layout):
+def test_head_vs_oracle(n_tok, K, V, w_layout, kernel):
     """Ragged row tile, ragged vocabulary tile, several contraction blocks; masked tokens; the
     config-3 drift law so that clips and zero-advantage rows occur."""
     batch = _head_batch(n_tok, K, V, seed=11, masked_frac=0.03, lp_mode="drift")
-    gpu = _run_head(batch, w_layout, stale_cap=2.0)
+    gpu = _run_head(batch, w_layout, stale_cap=2.0, kernel=kernel)
     ora = _oracle_head(batch, stale_cap=2.0)
     assert ora["clip_count"] > 0
     _check_head(gpu, ora, w_layout)
 
 
+@pytest.mark.parametrize("kernel,n_tok,panels", [(A.KERNEL_HEAD_1CTA, 9700, 3),
+                                                 (A.KERNEL_HEAD_2CTA, 19300, 3)])
 @pytest.mark.parametrize("norm", [A.NORM_CONST_K, A.NORM_PER_TRAJ])
-def test_head_several_panels(norm):
-    """More rows than one dS panel (4,736): dw_head accumulates across panels in fp32."""
-    batch = _head_batch(9700, 64, 512, seed=3, n_groups=8, group_size=8)
-    gpu = _run_head(batch, A.W_K_BY_V, normalizer=norm)
+def test_head_several_panels(norm, kernel, n_tok, panels):
+    """More rows than one dS panel (4,736 rows, 9,472 for CTA pairs): dw_head accumulates
+    across panels in fp32."""
+    batch = _head_batch(n_tok, 64, 512, seed=3, n_groups=8, group_size=8)
+    gpu = _run_head(batch, A.W_K_BY_V, normalizer=norm, kernel=kernel)
     ora = _oracle_head(batch, normalizer=norm)
     _check_head(gpu, ora, A.W_K_BY_V)
-    assert A.head_launches_per_call(9700, 512, 64) == 3 + 2 + 3 * 3
+    assert A.head_launches_per_call(n_tok, 512, 64, kernel) == 3 + 2 + 3 * panels
+
+
+def test_head_shapes_agree_bitwise_on_integers():
+    """Both tcgen05 shapes see the same inputs: same integers, values within rounding."""
+    batch = _head_batch(700, 128, 1512, seed=8, lp_mode="drift")
+    a = _run_head(batch, kernel=A.KERNEL_HEAD_1CTA)
+    b = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA)
+    assert (a["token_lp"] - b["token_lp"]).abs().max().item() <= 2e-6
+    assert int(a["clip_count"][0]) == int(b["clip_count"][0])
+    assert torch.equal(a["tok_coef"] == 0, b["tok_coef"] == 0)
+    d = (a["dhidden"].float() - b["dhidden"].float()).abs().max().item()
+    assert d <= 2.0 ** -7 * a["dhidden"].float().abs().max().item()
 
 
 def test_head_matches_logits_path():
