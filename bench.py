@@ -363,8 +363,9 @@ def run_cuda(args):
 def run_head(args):
     """--config 4: the fused LM-head variant (a5).  A step = one awr_loss_fwd_bwd_fused_head call
     (hidden [32,768, 2048] and W_head [2048, 151,936] in, loss / dhidden / dw_head out).  The
-    roofline is the tensor pipe: algorithmic flops 6 K V per token (logits, dH, dW); the path
-    executes 8 K V (the logits tile is recomputed for the backward), shown beside it."""
+    roofline is the tensor pipe: algorithmic flops 6 K V per token (logits, dH, dW).  The default
+    mode executes exactly those (the fp32 logits of one row panel are kept for a streaming dS
+    pass); --head-kernel 1cta / 2cta recompute the logits tile instead (8 K V executed)."""
     import torch
 
     import paper_2606_05597_b200 as A
@@ -385,7 +386,10 @@ def run_head(args):
     call = A.HeadLossCall(batch["hidden"], batch["w_head"], batch["target_ids"],
                           batch["behave_lp"], batch["prox_lp"], batch["step_off"],
                           batch["traj_off"], batch["group_off"], batch["rewards"],
-                          want=("err_word",), **batch["params"])
+                          want=("err_word",),
+                          **dict(batch["params"], kernel={"auto": A.KERNEL_AUTO, "1cta": A.KERNEL_HEAD_1CTA,
+                                                          "2cta": A.KERNEL_HEAD_2CTA,
+                                                          "stored": A.KERNEL_HEAD_2CTA_STORED}[args.head_kernel]))
     stream = torch.cuda.current_stream(dev)
     for _ in range(args.warmup):
         call.run()
@@ -411,6 +415,7 @@ def run_head(args):
     else:
         peak, peak_src = 1400.0, "B200_PROFILING.md fallback (of fallback)"
     alg_flops = 6.0 * K * V * n_tok
+    exe_ratio = 1.0 if args.head_kernel in ("auto", "stored") else 8.0 / 6.0
     achieved = alg_flops / (local_ms / args.steps / 1e3) / 1e12
     if rank == 0:
         line = {"metric": METRIC + " (fused LM-head variant)", "value": total_tok / (total_ms / 1e3),
@@ -420,13 +425,16 @@ def run_head(args):
                 "config": {"workload": "BASELINE.json configs[4] (%s)" % w.name,
                            "n_tok_per_gpu": n_tok, "V": V, "K": K, "w_layout": "K_BY_V",
                            "parallelism": "replicas only x%d" % world,
-                           "l2": "W_head (622 MB) + dS panels (1.4 GB) larger than L2, no flush"},
+                           "l2": "W_head (622 MB) + dS panels (1.4-2.9 GB) larger than L2, no flush"},
                 "roofline": {"bound": "tensor", "achieved": achieved, "peak": peak,
                              "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
-                             "kernel": "head_gemm_kernel (4 epilogues), whole step",
+                             "kernel": "head_gemm_kernel<epi, %s> (%s), whole step" % (
+                                 "1" if args.head_kernel == "1cta" else "2",
+                                 "3 GEMMs + dS streaming pass per panel" if exe_ratio == 1.0
+                                 else "4 GEMMs, logits recomputed"),
                              "algorithmic_flops_per_step": alg_flops,
-                             "executed_flops_per_step": alg_flops * 8 / 6,
-                             "executed_tflops": achieved * 8 / 6, "peak_source": peak_src},
+                             "executed_flops_per_step": alg_flops * exe_ratio,
+                             "executed_tflops": achieved * exe_ratio, "peak_source": peak_src},
                 "cpu_baseline": None, "e2e": None, "gpu_launches": call.launches * args.steps,
                 "clocks": clk.summary(), "loss": float(call.out["loss"][0]),
                 "clip_count": int(call.out["clip_count"][0])}
@@ -458,6 +466,9 @@ def main(argv=None):
     ap.add_argument("--n-tok", type=int, default=0, help="override the config's token count")
     ap.add_argument("--normalizer", type=int, default=None, choices=[0, 1])
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4"])
+    ap.add_argument("--head-kernel", default="auto", choices=["auto", "1cta", "2cta", "stored"],
+                    help="config 4: tcgen05 shape / backward mode (auto = stored: CTA pairs, fp32 "
+                         "logits of one row panel kept for the dS pass; 1cta / 2cta recompute)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: --steps")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

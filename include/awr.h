@@ -78,9 +78,13 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     16K <= V <= 163,840); shared memory is a TMA load FIFO */
        AWR_KERNEL_CLUSTER_RF4 = 4, /* the same with a row quarter per CTA of a 4-CTA cluster and
                                     two CTAs (of different rows) resident per SM */
-       /* fused-head entry points only (AUTO = AWR_KERNEL_HEAD_2CTA): */
-       AWR_KERNEL_HEAD_1CTA = 5, /* tcgen05 cta_group::1, 128 x 256 tiles, one CTA per SM */
-       AWR_KERNEL_HEAD_2CTA = 6  /* tcgen05 cta_group::2, 256 x 256 tiles on CTA pairs */ };
+       /* fused-head entry points only (AUTO = AWR_KERNEL_HEAD_2CTA_STORED): */
+       AWR_KERNEL_HEAD_1CTA = 5, /* tcgen05 cta_group::1, 128 x 256 tiles, one CTA per SM; the
+                                    logits tile is recomputed for the backward (8 K V flops/token) */
+       AWR_KERNEL_HEAD_2CTA = 6, /* tcgen05 cta_group::2, 256 x 256 tiles on CTA pairs; recompute */
+       AWR_KERNEL_HEAD_2CTA_STORED = 7 /* CTA pairs; the fp32 logits of ONE row panel (<= 9,472
+                                    rows, workspace) are kept between the forward GEMM and a
+                                    streaming dS pass: 6 K V flops/token, same bits as recompute */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u };
 

@@ -21,7 +21,7 @@ NORM_CONST_K, NORM_PER_TRAJ = 0, 1
 FLAG_SAMPLE_STD = 1
 W_K_BY_V, W_V_BY_K = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_CLUSTER, KERNEL_CLUSTER_RF, KERNEL_CLUSTER_RF4 = 0, 1, 2, 3, 4
-KERNEL_HEAD_1CTA, KERNEL_HEAD_2CTA = 5, 6
+KERNEL_HEAD_1CTA, KERNEL_HEAD_2CTA, KERNEL_HEAD_2CTA_STORED = 5, 6, 7
 ERRBIT_STEP_OFF, ERRBIT_TRAJ_OFF, ERRBIT_GROUP_OFF, ERRBIT_TARGET_RANGE = 1, 2, 4, 8
 
 _vp = C.c_void_p

@@ -66,7 +66,7 @@ static int check_params(const awr_params* p) {
     if (p->dual_clip_c > 1.f) return AWR_ERR_PARAM;          // Eq. (2) reserved
     if (p->normalizer != AWR_NORM_CONST_K && p->normalizer != AWR_NORM_PER_TRAJ) return AWR_ERR_PARAM;
     if (p->flags & ~(uint32_t)AWR_FLAG_SAMPLE_STD) return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_STORED) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -78,9 +78,13 @@ static int check_segments(int64_t n_tok, int32_t n_steps, int32_t n_traj, int32_
 
 // fused-head entry points: which tcgen05 shape (CTAs per tile) a kernel request means, or -1
 static int resolve_head_ctas(int requested) {
-    if (requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA) return 2;
+    if (requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA ||
+        requested == AWR_KERNEL_HEAD_2CTA_STORED) return 2;
     if (requested == AWR_KERNEL_HEAD_1CTA) return 1;
     return -1;
+}
+static int resolve_head_stored(int requested) {
+    return requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA_STORED;
 }
 
 static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype) {
@@ -257,7 +261,7 @@ size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_s
 int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K, int32_t kernel) {
     const int ctas = resolve_head_ctas(kernel);
     if (ctas < 0) return AWR_ERR_PARAM;
-    return 3 + head_launches(n_tok, V, K, ctas);     // a0, a1, [F, scalars, 3 per panel], final sum
+    return 3 + head_launches(n_tok, V, K, ctas, resolve_head_stored(kernel));     // a0, a1, [F, scalars, 3 per panel], final sum
 }
 
 int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
@@ -316,6 +320,7 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     c.dhidden = o->dhidden; c.dw_head = o->dw_head;
     c.ws = reinterpret_cast<uint8_t*>(ws_ptr) + w.total;
     c.ctas = resolve_head_ctas(p->kernel);
+    c.store_logits = resolve_head_stored(p->kernel);
     if (e == cudaSuccess) e = launch_head(c, info.num_sms, st);
     if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count, st);
     if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }

@@ -170,6 +170,15 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 for (int c = 0; c < kBN / 32; ++c) {
                     tmem_ld32(t_addr + c * 32, v);
                     const int c0 = n0 + c * 32;
+                    if (g.e.zout != nullptr && row_ok) {
+                        // keep the fp32 logits of this row panel for the dS pass (no recompute)
+                        float* zp = g.e.zout + (int64_t)row * g.e.zout_ld + c0;
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if (c0 + 4 * j < g.N)
+                                *reinterpret_cast<float4*>(zp + 4 * j) =
+                                    make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+                    }
                     if (c0 + 32 > g.N) {
 #pragma unroll
                         for (int j = 0; j < 32; ++j) if (c0 + j >= g.N) v[j] = -INFINITY;
@@ -309,10 +318,11 @@ namespace head {
 __global__ void __launch_bounds__(256)
 head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld, int n_tiles,
                     const float* __restrict__ zy, float* __restrict__ row_lse,
-                    float* __restrict__ row_coef, float* __restrict__ row_gy) {
+                    float* __restrict__ row_coef, float* __restrict__ row_gy, int64_t row0,
+                    int64_t row1) {
     const int lane = threadIdx.x & 31;
-    const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (row >= a.n_tok) return;
+    const int64_t row = row0 + (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= row1) return;
     MaxSum st{-INFINITY, 0.f};
     for (int j = lane; j < n_tiles; j += 32) {
         const float2 p = part[(int64_t)j * part_ld + row];
@@ -336,6 +346,44 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
         row_lse[row] = ts.lse;
         row_coef[row] = ts.coef;
         row_gy[row] = ts.gy;
+    }
+}
+
+// a4 for the stored-logits mode: dS = c_t (exp(z - lse) - onehot) from the fp32 logits panel the
+// forward GEMM kept, rounded to bf16.  The same arithmetic, instruction for instruction, as the
+// kEpiDs epilogue of the recompute mode, so both modes produce the same bits.  HBM-bound:
+// 4 B read + 2 B written per element; rows with c_t = 0 are written as zeros without a read.
+__global__ void __launch_bounds__(512)
+head_ds_kernel(const float* __restrict__ z, int64_t z_ld, int64_t rows, int64_t V,
+               const int32_t* __restrict__ target_ids, const float* __restrict__ row_lse,
+               const float* __restrict__ row_coef, const float* __restrict__ row_gy,
+               __nv_bfloat16* __restrict__ ds, int64_t ds_ld) {
+    const int nq = (int)(V >> 2);                       // V is a multiple of 8
+    for (int64_t row = blockIdx.x; row < rows; row += gridDim.x) {
+        const float coef = row_coef[row];
+        uint2* dst = reinterpret_cast<uint2*>(ds + row * ds_ld);
+        if (coef == 0.f) {
+            for (int i = threadIdx.x; i < nq; i += blockDim.x) dst[i] = make_uint2(0u, 0u);
+            continue;
+        }
+        const int y = target_ids[row];
+        const float gy = row_gy[row];
+        const float nref = -row_lse[row] * kLog2e;
+        const float4* src = reinterpret_cast<const float4*>(z + row * z_ld);
+#pragma unroll 4
+        for (int i = threadIdx.x; i < nq; i += blockDim.x) {
+            const float4 a = __ldcs(src + i);
+            float v0 = coef * ex2_approx(fmaf(a.x, kLog2e, nref));
+            float v1 = coef * ex2_approx(fmaf(a.y, kLog2e, nref));
+            float v2 = coef * ex2_approx(fmaf(a.z, kLog2e, nref));
+            float v3 = coef * ex2_approx(fmaf(a.w, kLog2e, nref));
+            if ((y >> 2) == i) {
+                const int w = y & 3;
+                v0 = w == 0 ? gy : v0; v1 = w == 1 ? gy : v1;
+                v2 = w == 2 ? gy : v2; v3 = w == 3 ? gy : v3;
+            }
+            dst[i] = make_uint2(pack_bf16x2(v0, v1), pack_bf16x2(v2, v3));
+        }
     }
 }
 
@@ -466,7 +514,8 @@ struct HeadWs {
     float2* part;
     __nv_bfloat16* ds;
     float* dw_acc;
-    int64_t part_ld, ds_ld, panel_rows;
+    float* zpanel;           // stored-logits mode: fp32 [panel_rows, z_ld]
+    int64_t part_ld, ds_ld, z_ld, panel_rows;
     int n_vtiles, n_panels;
     size_t total;
 };
@@ -476,7 +525,7 @@ struct HeadWs {
 // 37 x 8 = 296 tiles = 2 x 148 CTAs (ctas = 1) or 4 x 74 CTA pairs (ctas = 2).
 static int64_t head_panel_rows(int ctas) { return ctas == 2 ? 2 * kHeadPanelRows : kHeadPanelRows; }
 
-static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ctas) {
+static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ctas, bool store_z) {
     HeadWs w;
     uint8_t* p = reinterpret_cast<uint8_t*>(base);
     size_t off = 0;
@@ -494,13 +543,15 @@ static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ct
     w.part = (float2*)take((size_t)w.n_vtiles * n_pad * 8);
     w.ds = (__nv_bfloat16*)take((size_t)w.panel_rows * w.ds_ld * 2);
     w.dw_acc = (float*)take(w.n_panels > 1 ? (size_t)K * V * 4 : 0);
+    w.z_ld = w.ds_ld;
+    w.zpanel = (float*)take(store_z ? (size_t)w.panel_rows * w.z_ld * 4 : 0);
     w.total = off;
     return w;
 }
 
 size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K) {
-    const size_t a = head_carve(nullptr, n_tok, V, K, 1).total;
-    const size_t b = head_carve(nullptr, n_tok, V, K, 2).total;
+    const size_t a = head_carve(nullptr, n_tok, V, K, 1, false).total;
+    const size_t b = head_carve(nullptr, n_tok, V, K, 2, true).total;
     return a > b ? a : b;
 }
 
@@ -511,7 +562,8 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     }
     const int ctas = c.ctas == 1 ? 1 : 2;
     const int gm = 4096 / (kBM * ctas);               // raster groups of 4096 rows
-    const HeadWs w = head_carve(c.ws, c.n_tok, c.V, c.K, ctas);
+    const bool store_z = c.store_logits != 0;
+    const HeadWs w = head_carve(c.ws, c.n_tok, c.V, c.K, ctas, store_z);
     const bool kv = c.w_layout == AWR_W_K_BY_V;
     const __nv_bfloat16* H = reinterpret_cast<const __nv_bfloat16*>(c.hidden);
     // W as the B operand of Z = H W (n = v, contraction = k) and of dH = dS W^T (n = k, contraction = v)
@@ -520,19 +572,25 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(w.zy, 0, (size_t)w.part_ld * 4, st);
     if (e != cudaSuccess) return e;
 
-    // ---- pass F: log-sum-exp partials + gather over all rows
-    EpiArgs ea = {};
-    ea.part = w.part; ea.part_ld = w.part_ld; ea.zy = w.zy; ea.target_ids = c.rows->target_ids;
-    e = launch_gemm(kEpiLse, OperandView{H, c.n_tok, c.K, c.K, kMajorK}, w_fwd, 0, gm, ea, num_sms, ctas, st);
-    if (e != cudaSuccess) return e;
-
-    // ---- a3
-    {
+    // pass F + a3 over rows [r0, r0 + rows): log-sum-exp partials + gather, then the scalars.
+    // Partials / gathered logits are indexed by global row (pointers pre-offset by r0).
+    auto forward = [&](int64_t r0, int64_t rows, float* zout) -> cudaError_t {
+        EpiArgs ea = {};
+        ea.part = w.part + r0; ea.part_ld = w.part_ld; ea.zy = w.zy + r0;
+        ea.target_ids = c.rows->target_ids + r0;
+        ea.zout = zout; ea.zout_ld = w.z_ld;
+        cudaError_t err = launch_gemm(kEpiLse, OperandView{H + r0 * c.K, rows, c.K, c.K, kMajorK}, w_fwd,
+                                      0, gm, ea, num_sms, ctas, st);
+        if (err != cudaSuccess) return err;
         const int warps = 8;
-        const unsigned blocks = (unsigned)((c.n_tok + warps - 1) / warps);
+        const unsigned blocks = (unsigned)((rows + warps - 1) / warps);
         head_scalars_kernel<<<blocks, warps * 32, 0, st>>>(*c.rows, w.part, w.part_ld, w.n_vtiles,
-                                                           w.zy, w.row_lse, w.row_coef, w.row_gy);
-        e = cudaGetLastError();
+                                                           w.zy, w.row_lse, w.row_coef, w.row_gy,
+                                                           r0, r0 + rows);
+        return cudaGetLastError();
+    };
+    if (!store_z) {
+        e = forward(0, c.n_tok, nullptr);
         if (e != cudaSuccess) return e;
     }
 
@@ -541,11 +599,22 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         const int64_t r0 = (int64_t)p * w.panel_rows;
         const int64_t rows = (c.n_tok - r0 < w.panel_rows) ? (c.n_tok - r0) : w.panel_rows;
         const __nv_bfloat16* Hp = H + r0 * c.K;
-        EpiArgs e1 = {};
-        e1.target_ids = c.rows->target_ids + r0; e1.row_lse = w.row_lse + r0;
-        e1.row_coef = w.row_coef + r0; e1.row_gy = w.row_gy + r0;
-        e1.ds = w.ds; e1.ds_ld = w.ds_ld;
-        e = launch_gemm(kEpiDs, OperandView{Hp, rows, c.K, c.K, kMajorK}, w_fwd, 0, gm, e1, num_sms, ctas, st);
+        if (store_z) {
+            // forward of this panel keeps its fp32 logits; dS is then one streaming pass
+            e = forward(r0, rows, w.zpanel);
+            if (e != cudaSuccess) return e;
+            const unsigned blocks = (unsigned)(rows < 4 * (int64_t)num_sms ? rows : 4 * (int64_t)num_sms);
+            head_ds_kernel<<<blocks, 512, 0, st>>>(w.zpanel, w.z_ld, rows, c.V,
+                                                   c.rows->target_ids + r0, w.row_lse + r0,
+                                                   w.row_coef + r0, w.row_gy + r0, w.ds, w.ds_ld);
+            e = cudaGetLastError();
+        } else {
+            EpiArgs e1 = {};
+            e1.target_ids = c.rows->target_ids + r0; e1.row_lse = w.row_lse + r0;
+            e1.row_coef = w.row_coef + r0; e1.row_gy = w.row_gy + r0;
+            e1.ds = w.ds; e1.ds_ld = w.ds_ld;
+            e = launch_gemm(kEpiDs, OperandView{Hp, rows, c.K, c.K, kMajorK}, w_fwd, 0, gm, e1, num_sms, ctas, st);
+        }
         if (e != cudaSuccess) return e;
 
         EpiArgs e2 = {};
@@ -571,9 +640,10 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     return cudaSuccess;
 }
 
-int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas) {
-    const HeadWs w = head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2);
-    return 2 + 3 * w.n_panels;
+int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int store_logits) {
+    const HeadWs w = head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2, store_logits != 0);
+    // recompute: F, scalars, then (dS GEMM, dH, dW) per panel; stored: (F, scalars, dS pass, dH, dW) per panel
+    return store_logits ? 5 * w.n_panels : 2 + 3 * w.n_panels;
 }
 
 cudaError_t launch_gemm_bf16(const void* A, int a_major, int64_t lda, const void* B, int b_major,

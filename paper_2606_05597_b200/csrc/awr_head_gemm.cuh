@@ -80,6 +80,8 @@ struct EpiArgs {
     int64_t part_ld;
     float* zy;                 // [M] gathered target logit (fp32 accumulator value)
     const int32_t* target_ids; // [M] (kEpiLse, kEpiDs), already offset to row 0 of this GEMM
+    float* zout;               // optional [M, zout_ld]: the fp32 logits tile, kept for the dS pass
+    int64_t zout_ld;
     // kEpiDs
     const float* row_lse;      // [M] log-sum-exp of the whole row
     const float* row_coef;     // [M] c_t

@@ -44,9 +44,11 @@ struct HeadCall {
     void* dw_head;
     void* ws;
     int ctas;        // 1: cta_group::1 tiles of 128 rows; anything else: CTA pairs, 256-row tiles
+    int store_logits;  // 0: recompute the logits tile for dS (8 K V flops / token); 1: keep the fp32
+                       // logits of one row panel and form dS in a streaming pass (6 K V)
 };
 size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K);
-int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas);
+int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int store_logits);
 cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st);
 // C[M, N] (bf16, row-major, ldc) = A B on the tcgen05 engine; majors: 0 = contraction index
 // contiguous, 1 = row (A) / column (B) index contiguous.

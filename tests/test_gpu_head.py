@@ -114,7 +114,7 @@ def _check_head(gpu, ora, w_layout):
         assert not gpu["dhidden"][torch.from_numpy(zero_rows).to(DEV)].any()
 
 
-@pytest.mark.parametrize("kernel", HEAD_KERNELS)
+@pytest.mark.parametrize("kernel", HEAD_KERNELS + [A.KERNEL_HEAD_2CTA_STORED])
 @pytest.mark.parametrize("w_layout", [A.W_K_BY_V, A.W_V_BY_K])
 @pytest.mark.parametrize("n_tok,K,V", [(300, 128, 1000), (128, 64, 256), (517, 192, 2056)])
 def test_head_vs_oracle(n_tok, K, V, w_layout, kernel):
@@ -128,7 +128,8 @@ def test_head_vs_oracle(n_tok, K, V, w_layout, kernel):
 
 
 @pytest.mark.parametrize("kernel,n_tok,panels", [(A.KERNEL_HEAD_1CTA, 9700, 3),
-                                                 (A.KERNEL_HEAD_2CTA, 19300, 3)])
+                                                 (A.KERNEL_HEAD_2CTA, 19300, 3),
+                                                 (A.KERNEL_HEAD_2CTA_STORED, 19300, 3)])
 @pytest.mark.parametrize("norm", [A.NORM_CONST_K, A.NORM_PER_TRAJ])
 def test_head_several_panels(norm, kernel, n_tok, panels):
     """More rows than one dS panel (4,736 rows, 9,472 for CTA pairs): dw_head accumulates
@@ -137,7 +138,20 @@ def test_head_several_panels(norm, kernel, n_tok, panels):
     gpu = _run_head(batch, A.W_K_BY_V, normalizer=norm, kernel=kernel)
     ora = _oracle_head(batch, normalizer=norm)
     _check_head(gpu, ora, A.W_K_BY_V)
-    assert A.head_launches_per_call(n_tok, 512, 64, kernel) == 3 + 2 + 3 * panels
+    per_call = 5 * panels if kernel == A.KERNEL_HEAD_2CTA_STORED else 2 + 3 * panels
+    assert A.head_launches_per_call(n_tok, 512, 64, kernel) == 3 + per_call
+    assert A.head_launches_per_call(n_tok, 512, 64) == A.head_launches_per_call(
+        n_tok, 512, 64, A.KERNEL_HEAD_2CTA_STORED)          # AUTO resolves to the stored mode
+
+
+def test_head_stored_logits_same_bits_as_recompute():
+    """The stored-logits mode keeps the fp32 accumulators of the forward GEMM and applies the
+    same dS arithmetic as the recompute epilogue: every output is bit-identical."""
+    batch = _head_batch(1111, 128, 3000, seed=21, lp_mode="drift", masked_frac=0.02)
+    a = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA, stale_cap=2.0)
+    b = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA_STORED, stale_cap=2.0)
+    for k in ("loss", "token_lp", "clip_count", "tok_coef", "tok_term", "dhidden", "dw_head"):
+        assert torch.equal(a[k], b[k]), k
 
 
 def test_head_shapes_agree_bitwise_on_integers():
