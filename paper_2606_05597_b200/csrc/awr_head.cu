@@ -157,6 +157,23 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
             const int row = m_blk * G::kTileM + (int)rank * kBM + q * 32 + lane;
             const int n0 = n_blk * kBN;
             const bool row_ok = row < g.M;
+            // kEpiAccum: the running fp32 sum of this thread's row is fetched one 32-column chunk
+            // ahead (chunk 0 before the accumulator is even complete), so the global-memory
+            // latency overlaps the MMAs / the previous chunk instead of serialising 8 round trips
+            float4 pre[8];
+            auto fetch_acc = [&](int c) {
+                if constexpr (EPI == kEpiAccum) {
+                    const int c0 = n0 + c * 32;
+                    if (!g.e.first_panel && row_ok && c < kBN / 32) {
+                        const float* ap = g.e.acc + (int64_t)row * g.e.out_ld + c0;
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            pre[j] = (c0 + 4 * j < g.N) ? __ldcs(reinterpret_cast<const float4*>(ap + 4 * j))
+                                                        : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                }
+            };
+            fetch_acc(0);
             mbar_wait(tfull_bar(as), aphase);
             tc_fence_after();
             const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)as * kBN;
@@ -253,12 +270,10 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                         if (!g.e.first_panel) {
 #pragma unroll
                             for (int j = 0; j < 8; ++j) {
-                                if (c0 + 4 * j < g.N) {
-                                    const float4 p = *reinterpret_cast<const float4*>(ap + 4 * j);
-                                    v[4 * j] += p.x; v[4 * j + 1] += p.y;
-                                    v[4 * j + 2] += p.z; v[4 * j + 3] += p.w;
-                                }
+                                v[4 * j] += pre[j].x; v[4 * j + 1] += pre[j].y;
+                                v[4 * j + 2] += pre[j].z; v[4 * j + 3] += pre[j].w;
                             }
+                            fetch_acc(c + 1);
                         }
                         to_bf16 = g.e.last_panel != 0;
                         if (!to_bf16) {
@@ -579,8 +594,11 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         ea.part = w.part + r0; ea.part_ld = w.part_ld; ea.zy = w.zy + r0;
         ea.target_ids = c.rows->target_ids + r0;
         ea.zout = zout; ea.zout_ld = w.z_ld;
+        // raster: when the H rows of this call fit in L2 (a panel: 39 MB at K = 2048) walk all of
+        // its row tiles before the next W column tile, so W_head streams from HBM exactly once
+        const int fgm = rows * c.K * 2 <= (48ll << 20) ? (int)((rows + kBM * ctas - 1) / (kBM * ctas)) : gm;
         cudaError_t err = launch_gemm(kEpiLse, OperandView{H + r0 * c.K, rows, c.K, c.K, kMajorK}, w_fwd,
-                                      0, gm, ea, num_sms, ctas, st);
+                                      0, fgm, ea, num_sms, ctas, st);
         if (err != cudaSuccess) return err;
         const int warps = 8;
         const unsigned blocks = (unsigned)((rows + warps - 1) / warps);
