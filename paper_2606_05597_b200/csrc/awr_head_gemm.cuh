@@ -53,7 +53,7 @@ struct Geo {
     static constexpr int kLoadN = kBN / CTAS;            // B columns staged by one CTA
     static constexpr int kBBytes = kLoadN * kBK * 2;     // 32 KB / 16 KB
     static constexpr int kStageBytes = kABytes + kBBytes;
-    static constexpr int kStages = CTAS == 1 ? 4 : 6;
+    static constexpr int kStages = CTAS == 1 ? 4 : 7;
     static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment */ + 256 /* barriers */;
 };
 static_assert(Geo<2>::kStages <= kMaxStages && Geo<2>::kSmemBytes <= 232448, "shared memory");
