@@ -23,7 +23,11 @@ this file fixes: A1 (mean over groups: kappa_g = 1/(NG G_g)), A2 (population std
 in the denominator, zero-variance group -> A = 0 exactly; sample std by flag), A3
 (k_norm is its own scalar), A4 (stale_cap truncates w_t; <= 0 or inf = off), A5/A6
 (trigger = clipped branch strictly smaller), A10 (empty steps count toward |tau_i|),
-A13 (negative target id = masked token), A14 (thresholds are 1 -/+ float64(float32(eps))).
+A13 (negative target id = masked token), A14 (thresholds are 1 -/+ float64(float32(eps))),
+A7 (Eq. (2), PAPER.md:270-275, is dimensionally garbled - "max[f(rho), c A]" with f a ratio;
+read as the dual clip of Ye et al. 2020 that the text cites: with s_t the inner min of Eq. (1)
+and rho = r_t, a token with A < 0 contributes max(s_t, c A); a *dual-clip hit* is c A > s_t
+strictly, i.e. A < 0 and r_t > c; its gradient is zero.  c <= 1 = off = Eq. (1)).
 
 Pins (tests/test_oracle_pins.py, ``-m "not gpu"``): P1..P12 of SURVEY.md 8(c) - closed
 forms, a library softmax-cross-entropy gradient, finite differences, a literal
@@ -134,7 +138,8 @@ def token_logprob(logits_rows, target_ids):
 
 
 # ----------------------------------------------------------------------------- O4..O6, O8 scalar part
-def token_terms(lp, prox_lp, behave_lp, adv_tok, scale_tok, clip_eps, stale_cap, valid):
+def token_terms(lp, prox_lp, behave_lp, adv_tok, scale_tok, clip_eps, stale_cap, valid,
+                dual_clip_c=0.0, want_dual=False):
     """O4, O5 and the scalar part of O7/O8 for a set of tokens.
 
     lp = l_t, prox_lp = q_t, behave_lp = b_t, adv_tok = A_i of the token's trajectory,
@@ -142,7 +147,10 @@ def token_terms(lp, prox_lp, behave_lp, adv_tok, scale_tok, clip_eps, stale_cap,
     range.  Returns (term_t, c_t, trig_t, r_t, w_t) with
        term_t = scale * w_t * min(r_t A, clip(r_t) A)
        c_t    = scale * w_t * r_t * A   if the unclipped branch is active, else 0
-       trig_t = clipped branch strictly smaller (A5, A6)."""
+       trig_t = clipped branch strictly smaller (A5, A6).
+    dual_clip_c > 1 (Eq. (2), reading A7): for A < 0 the inner min s_t is
+    capped from below, s_t <- max(s_t, c A); dual_t = (c A > s_t) strictly; such a token's
+    term is constant in theta, so c_t = 0.  ``want_dual`` appends dual_t to the result."""
     lp = np.asarray(lp, dtype=np.float64)
     q = np.asarray(prox_lp, dtype=np.float64)
     b = np.asarray(behave_lp, dtype=np.float64)
@@ -158,12 +166,21 @@ def token_terms(lp, prox_lp, behave_lp, adv_tok, scale_tok, clip_eps, stale_cap,
     v = np.minimum(np.maximum(r, 1.0 - eps), 1.0 + eps) * A  # O5  clipped branch
     s = np.minimum(u, v)
     trig = v < u                                            # A5 / A6: strict
+    dual = np.zeros(s.shape, dtype=bool)
+    cdual = float(np.float32(dual_clip_c))
+    if cdual > 1.0:                                         # Eq. (2), A7
+        floor = cdual * A
+        dual = (A < 0.0) & (floor > s)
+        s = np.where(A < 0.0, np.maximum(s, floor), s)
     term = scale * w * s
-    coef = np.where(trig, 0.0, scale * w * r * A)           # O8
+    coef = np.where(trig | dual, 0.0, scale * w * r * A)    # O8
     valid = np.asarray(valid, dtype=bool)
     term = np.where(valid, term, 0.0)
     coef = np.where(valid, coef, 0.0)
     trig = trig & valid
+    dual = dual & valid
+    if want_dual:
+        return term, coef, trig, r, w, dual
     return term, coef, trig, r, w
 
 
@@ -206,7 +223,7 @@ def traj_scale(step_off, traj_off, group_off, k_norm, normalizer, loss_scale):
 
 def awr_loss_fwd_bwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off,
                      rewards, *, k_norm, clip_eps, stale_cap, normalizer, flags=0,
-                     loss_scale=1.0, want_dlogits=True, grad_rows=None):
+                     loss_scale=1.0, dual_clip_c=0.0, want_dlogits=True, grad_rows=None):
     """The whole hot path a0..a4 for one batch.
 
     logits: [n_tok, V] array of the *exact* input values (bf16 widened exactly by the
@@ -231,14 +248,16 @@ def awr_loss_fwd_bwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off,
     for lo in range(0, n_tok, step):
         hi = min(n_tok, lo + step)
         lse[lo:hi], lp[lo:hi], zy[lo:hi] = token_logprob(z[lo:hi], y[lo:hi])    # O3
-    term, coef, trig, r, w = token_terms(lp, prox_lp, behave_lp, adv[tok_traj],
-                                         scale[tok_traj], clip_eps, stale_cap, valid)  # O4..O6
+    term, coef, trig, r, w, dual = token_terms(lp, prox_lp, behave_lp, adv[tok_traj],
+                                               scale[tok_traj], clip_eps, stale_cap, valid,
+                                               dual_clip_c, want_dual=True)       # O4..O6, Eq. (2)
     loss = 0.0
     for t in range(n_tok):                                                        # O7: token order
         loss -= term[t]
     out = dict(loss=loss, token_lp=lp, clip_count=int(trig.sum()), adv=adv,       # O9
                tok_traj=tok_traj, target_logit=zy, lse=lse, term=term, coef=coef,
-               trig=trig, ratio=r, stale_w=w, err_word=err, traj_scale=scale)
+               trig=trig, ratio=r, stale_w=w, err_word=err, traj_scale=scale,
+               dual=dual, dual_clip_count=int(dual.sum()))
     if want_dlogits:
         rows = np.arange(n_tok) if grad_rows is None else np.asarray(grad_rows, dtype=np.int64)
         g = np.empty((rows.size, V), dtype=np.float64)

@@ -378,3 +378,95 @@ def test_fused_head_miniature_against_plain_loops():
     assert np.allclose(out["dhidden"], dH, atol=1e-15)
     assert np.allclose(out["dw_head"], dW, atol=1e-15)
     assert out["loss"] == tok["loss"]
+
+
+# ------------------------------------------------------------------------------------ P13: Eq. (2)
+def _with_exploded_ratios(host, every=5, shift=1.5):
+    """Lower prox_lp on every 5th token so that r_t = pi_theta/pi_prox grows by e^1.5 = 4.5 > c."""
+    host = dict(host)
+    q = host["prox_lp"].copy()
+    q[::every] -= shift
+    host["prox_lp"] = q
+    return host
+
+
+def test_p13_dual_clip_worked_example():
+    """PAPER.md:270-275 with c = 3 (:461), eps = 0.2, one trajectory pair so that A = -1/+1:
+    r = 5, A = -1: min(5(-1), 1.2(-1)) = -5, capped to c A = -3 (hit, zero gradient);
+    r = 2, A = -1: min(-2, -1.2) = -2 > -3 (no hit);  r = 5, A = +1: min(5, 1.2) = 1.2 (eps-clip)."""
+    lp = np.log(np.array([0.5, 0.2, 0.5]))
+    q = lp - np.log(np.array([5.0, 2.0, 5.0]))
+    A = np.array([-1.0, -1.0, 1.0])
+    one = np.ones(3)
+    term, coef, trig, r, w, dual = O.token_terms(lp, q, q, A, one, 0.2, 0.0, one.astype(bool),
+                                                 dual_clip_c=3.0, want_dual=True)
+    assert np.allclose(r, [5.0, 2.0, 5.0]) and np.allclose(w, 1.0)
+    assert np.allclose(term, [-3.0, -2.0, 1.0 + float(np.float32(0.2))])
+    assert dual.tolist() == [True, False, False] and trig.tolist() == [False, False, True]
+    assert coef[0] == 0.0 and coef[2] == 0.0 and coef[1] == pytest.approx(-2.0)
+
+
+@pytest.mark.parametrize("norm", [O.NORM_CONST_K, O.NORM_PER_TRAJ])
+def test_p13_dual_clip_matches_a_literal_loop_and_bounds_the_term(norm):
+    """Ye et al. 2020 as cited by PAPER.md:270: max(min(rho A, clip(rho) A), c A) for A < 0, times
+    the staleness weight; literal loop with math.exp.  Also the paper's claim (:275): c A is an
+    absolute lower bound of the per-token contribution (before the weights)."""
+    host = _with_exploded_ratios(small_batch(seed=13, V=24, n_tok=80, lp_mode="drift",
+                                             normalizer=norm, stale_cap=2.0))
+    c = 3.0
+    out = run(host, dual_clip_c=c)
+    eps = float(np.float32(host["params"]["clip_eps"]))
+    loss, hits = 0.0, 0
+    for t in range(host["logits"].shape[0]):
+        A = float(out["adv"][out["tok_traj"][t]])
+        scale = float(out["traj_scale"][out["tok_traj"][t]])
+        r = math.exp(out["token_lp"][t] - float(host["prox_lp"][t]))
+        w = min(math.exp(float(host["prox_lp"][t]) - float(host["behave_lp"][t])), 2.0)
+        s = min(r * A, min(max(r, 1 - eps), 1 + eps) * A)
+        if A < 0 and c * A > s:
+            s = c * A
+            hits += 1
+        loss -= scale * w * s
+        if A < 0:
+            assert out["term"][t] >= scale * w * c * A * (1 + 1e-12)
+    assert hits > 0 and out["dual_clip_count"] == hits
+    assert out["loss"] == pytest.approx(loss, rel=1e-12, abs=1e-15)
+    # hit tokens: A < 0 and r > c exactly; they carry no gradient and are not eps-triggers
+    hit = out["dual"]
+    assert np.array_equal(hit, (out["adv"][out["tok_traj"]] < 0) & (out["ratio"] > c))
+    assert not np.any(out["trig"] & hit)
+    assert np.all(out["coef"][hit] == 0) and np.all(out["dlogits"][hit] == 0)
+
+
+def test_p13_dual_clip_off_and_limit_cases():
+    host = _with_exploded_ratios(small_batch(seed=14, lp_mode="drift"))
+    base = run(host)
+    for c in (0.0, 1.0):                               # c <= 1: off = Eq. (1)
+        o = run(host, dual_clip_c=c)
+        assert o["loss"] == base["loss"] and o["dual_clip_count"] == 0
+    big = run(host, dual_clip_c=1e30)                  # c -> inf: the floor is never reached
+    assert big["loss"] == base["loss"] and big["dual_clip_count"] == 0
+    assert np.array_equal(big["dlogits"], base["dlogits"])
+    on = run(host, dual_clip_c=3.0)
+    pos = base["adv"][base["tok_traj"]] >= 0           # A >= 0 tokens are untouched
+    assert np.array_equal(on["term"][pos], base["term"][pos])
+    assert np.array_equal(on["coef"][pos], base["coef"][pos])
+    assert on["dual_clip_count"] > 0 and on["loss"] < base["loss"]   # -J with a raised floor
+
+
+def test_p13_dual_clip_finite_differences():
+    host = _with_exploded_ratios(small_batch(seed=15, V=16, n_groups=2, group_size=3, n_tok=24,
+                                             lp_mode="drift", normalizer=O.NORM_PER_TRAJ))
+    host["logits"] = host["logits"].astype(np.float64)
+    out = run(host, dual_clip_c=3.0)
+    assert out["dual_clip_count"] > 0
+    lr = out["token_lp"] - host["prox_lp"]
+    assert np.all(np.abs(lr - math.log(3.0)) > 1e-3)   # away from the new kink
+    h = 1e-6
+    for t in range(host["logits"].shape[0]):
+        for v in (0, 7, int(host["target_ids"][t])):
+            zp = host["logits"].copy(); zp[t, v] += h
+            zm = host["logits"].copy(); zm[t, v] -= h
+            fd = (run(dict(host, logits=zp), dual_clip_c=3.0, want_dlogits=False)["loss"] -
+                  run(dict(host, logits=zm), dual_clip_c=3.0, want_dlogits=False)["loss"]) / (2 * h)
+            assert out["dlogits"][t, v] == pytest.approx(fd, abs=1e-7)
