@@ -115,7 +115,9 @@ typedef struct awr_params {
     float clip_eps;     /* eps of the decoupled clip (:57), in [0, 1); paper: 0.2 (:437) */
     float stale_cap;    /* A4: w_t <- min(w_t, cap); <= 0 or +inf = off (Eq. 1 exactly) */
     float loss_scale;   /* multiplies loss and gradient (micro-batching); 1 = Eq. 1 */
-    float dual_clip_c;  /* reserved for Eq. (2) (:270); must be <= 1 (= off) in this version */
+    float dual_clip_c;  /* Eq. (2) (:270-275, c = 3.0 in every GRPO run of the paper, :461): > 1 caps
+                           the per-token min from below by c * A when A < 0; <= 1 = off = Eq. (1).
+                           A hit (A < 0 and pi_theta/pi_prox > c) has zero gradient. */
     int32_t normalizer; /* AWR_NORM_* */
     uint32_t flags;     /* AWR_FLAG_*; unknown bits -> AWR_ERR_PARAM */
     int32_t kernel;     /* AWR_KERNEL_*; CLUSTER on an unsupported shape -> AWR_ERR_PARAM */
@@ -133,6 +135,7 @@ typedef struct awr_outputs {
     float* tok_term;        /* [n_tok] per-token contribution to J (loss = -sum) */
     float* tok_coef;        /* [n_tok] c_t */
     uint32_t* err_word;     /* [1] OR of AWR_ERRBIT_* (0 = clean) */
+    int64_t* dual_clip_count; /* [1] number of tokens hit by the dual clip (:128); 0 when off */
 } awr_outputs;
 
 /* a0..a4 fused: segment expansion, group advantage (:61), online log-sum-exp + target gather,
@@ -198,6 +201,7 @@ typedef struct awr_head_outputs {
     float* tok_term;        /* optional */
     float* tok_coef;        /* optional */
     uint32_t* err_word;     /* optional */
+    int64_t* dual_clip_count; /* optional */
 } awr_head_outputs;
 
 AWR_API int awr_loss_fwd_bwd_fused_head(const awr_head_batch* batch, const awr_params* params,

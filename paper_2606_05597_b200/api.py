@@ -57,7 +57,8 @@ def alloc_outputs(n_tok, n_traj, device, like_logits=None, want=OPTIONAL_OUTPUTS
     """Output tensors of awr_loss_fwd_bwd (dlogits only if like_logits is given)."""
     o = dict(loss=torch.empty(1, dtype=torch.float32, device=device),
              token_lp=torch.empty(n_tok, dtype=torch.float32, device=device),
-             clip_count=torch.empty(1, dtype=torch.int64, device=device))
+             clip_count=torch.empty(1, dtype=torch.int64, device=device),
+             dual_clip_count=torch.empty(1, dtype=torch.int64, device=device))
     if like_logits is not None:
         o["dlogits"] = torch.empty_like(like_logits)
     spec = dict(adv=(n_traj, torch.float32), tok_traj=(n_tok, torch.int32),
@@ -102,7 +103,7 @@ def _out_struct(o):
     return awr_outputs(_ptr(g("loss")), _ptr(g("dlogits")), _ptr(g("token_lp")),
                        _ptr(g("clip_count")), _ptr(g("adv")), _ptr(g("tok_traj")),
                        _ptr(g("target_logit")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
-                       _ptr(g("err_word")))
+                       _ptr(g("err_word")), _ptr(g("dual_clip_count")))
 
 
 class LossCall:
@@ -230,7 +231,7 @@ class HostLossCall:
         small_in = 12 * n_tok + 4 * (self.batch.n_steps + self.batch.n_traj +
                                      self.batch.n_groups + 3) + 4 * n_traj
         self.h2d_bytes = n_tok * self.batch.ld * esz + small_in
-        small_out = 4 * n_tok + 12 + sum(self.out[k].numel() * self.out[k].element_size()
+        small_out = 4 * n_tok + 20 + sum(self.out[k].numel() * self.out[k].element_size()
                                          for k in want)
         self.d2h_bytes = n_tok * self.batch.ld * esz + small_out
 
@@ -302,7 +303,8 @@ class HeadLossCall:
         o = dict(loss=torch.empty(1, dtype=torch.float32, device=dev),
                  dhidden=torch.empty_like(hidden), dw_head=torch.empty_like(w_head),
                  token_lp=torch.empty(n_tok, dtype=torch.float32, device=dev),
-                 clip_count=torch.empty(1, dtype=torch.int64, device=dev))
+                 clip_count=torch.empty(1, dtype=torch.int64, device=dev),
+                 dual_clip_count=torch.empty(1, dtype=torch.int64, device=dev))
         spec = dict(adv=(n_traj, torch.float32), tok_traj=(n_tok, torch.int32),
                     tok_term=(n_tok, torch.float32), tok_coef=(n_tok, torch.float32),
                     err_word=(1, torch.int32))
@@ -314,7 +316,7 @@ class HeadLossCall:
         self.outs = awr_head_outputs(_ptr(g("loss")), _ptr(g("dhidden")), _ptr(g("dw_head")),
                                      _ptr(g("token_lp")), _ptr(g("clip_count")), _ptr(g("adv")),
                                      _ptr(g("tok_traj")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
-                                     _ptr(g("err_word")))
+                                     _ptr(g("err_word")), _ptr(g("dual_clip_count")))
         need = head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups)
         self.workspace = workspace if workspace is not None else torch.empty(
             max(need, 256), dtype=torch.uint8, device=dev)

@@ -63,7 +63,7 @@ static int check_params(const awr_params* p) {
     if (!(p->clip_eps >= 0.f && p->clip_eps < 1.f)) return AWR_ERR_PARAM;
     if (isnan(p->stale_cap)) return AWR_ERR_PARAM;
     if (!isfinite(p->loss_scale)) return AWR_ERR_PARAM;
-    if (p->dual_clip_c > 1.f) return AWR_ERR_PARAM;          // Eq. (2) reserved
+    if (isnan(p->dual_clip_c)) return AWR_ERR_PARAM;          // Eq. (2): > 1 = on, <= 1 = off
     if (p->normalizer != AWR_NORM_CONST_K && p->normalizer != AWR_NORM_PER_TRAJ) return AWR_ERR_PARAM;
     if (p->flags & ~(uint32_t)AWR_FLAG_SAMPLE_STD) return AWR_ERR_PARAM;
     if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_STORED) return AWR_ERR_PARAM;
@@ -165,7 +165,7 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     a.tok_traj = tok_traj; a.adv = adv; a.traj_scale = w.traj_scale;
     a.token_lp = o->token_lp; a.tok_term = tok_term; a.tok_coef = o->tok_coef;
     a.target_logit = o->target_logit; a.tok_flag = w.tok_flag; a.err_word = err;
-    a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap;
+    a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap; a.dual_c = p->dual_clip_c;
     cudaEvent_t ev0 = g_prof_before, ev1 = g_prof_after;
     g_prof_before = g_prof_after = nullptr;
     if (e == cudaSuccess && ev0) e = cudaEventRecord(ev0, st);
@@ -174,7 +174,8 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     }
     if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, st);
     // a3 final reduction
-    if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count, st);
+    if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count,
+                                                    o->dual_clip_count, st);
     if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
     return AWR_OK;
 }
@@ -313,7 +314,7 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     a.tok_traj = tok_traj; a.adv = adv; a.traj_scale = w.traj_scale;
     a.token_lp = o->token_lp; a.tok_term = tok_term; a.tok_coef = o->tok_coef;
     a.target_logit = nullptr; a.tok_flag = w.tok_flag; a.err_word = err;
-    a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap;
+    a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap; a.dual_c = p->dual_clip_c;
     HeadCall c;
     c.hidden = b->hidden; c.w_head = b->w_head; c.w_layout = b->w_layout;
     c.n_tok = b->n_tok; c.V = b->V; c.K = b->K; c.rows = &a;
@@ -322,7 +323,8 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     c.ctas = resolve_head_ctas(p->kernel);
     c.store_logits = resolve_head_stored(p->kernel);
     if (e == cudaSuccess) e = launch_head(c, info.num_sms, st);
-    if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count, st);
+    if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count,
+                                                    o->dual_clip_count, st);
     if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
     return AWR_OK;
 }
@@ -438,6 +440,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
     float* d_loss = (float*)d_scal;
     int64_t* d_cnt = (int64_t*)(d_scal + 8);
     uint32_t* d_err = (uint32_t*)(d_scal + 16);
+    int64_t* d_dual = (int64_t*)(d_scal + 24);
 
     cudaStream_t user = reinterpret_cast<cudaStream_t>(stream);
     cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;
@@ -494,7 +497,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
         a.tok_traj = d_tt + r0; a.adv = d_adv; a.traj_scale = w.traj_scale;
         a.token_lp = d_lp + r0; a.tok_term = d_term + r0; a.tok_coef = d_coef + r0;
         a.target_logit = d_tl + r0; a.tok_flag = w.tok_flag + r0; a.err_word = d_err;
-        a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap;
+        a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap; a.dual_c = p->dual_clip_c;
         AWR_TRY(launch_rows(kernel, a, hb->logits_dtype, info.num_sms, s_k));
         AWR_TRY(cudaEventRecord(ev_k[bi], s_k));
         AWR_TRY(cudaStreamWaitEvent(s_out, ev_k[bi], 0));
@@ -502,9 +505,10 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
                                 (size_t)rows * row_bytes, D2H, s_out));
         AWR_TRY(cudaEventRecord(ev_out[bi], s_out));
     }
-    AWR_TRY(launch_final_reduce(d_term, w.tok_flag, n, d_loss, d_cnt, s_k));
+    AWR_TRY(launch_final_reduce(d_term, w.tok_flag, n, d_loss, d_cnt, d_dual, s_k));
     AWR_TRY(cudaMemcpyAsync(ho->loss, d_loss, 4, D2H, s_k));
     AWR_TRY(cudaMemcpyAsync(ho->clip_count, d_cnt, 8, D2H, s_k));
+    if (ho->dual_clip_count) AWR_TRY(cudaMemcpyAsync(ho->dual_clip_count, d_dual, 8, D2H, s_k));
     if (ho->err_word) AWR_TRY(cudaMemcpyAsync(ho->err_word, d_err, 4, D2H, s_k));
     if (n > 0) {
         AWR_TRY(cudaMemcpyAsync(ho->token_lp, d_lp, (size_t)n * 4, D2H, s_k));

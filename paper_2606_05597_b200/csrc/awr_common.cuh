@@ -17,6 +17,7 @@ constexpr unsigned kFull = 0xffffffffu;
 
 // per-token flag byte written by the row kernels, read by the final reduction
 constexpr uint8_t kFlagTrig = 1;
+constexpr uint8_t kFlagDual = 2;   // Eq. (2) dual-clip hit
 
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
@@ -63,9 +64,13 @@ struct TokenScalars {
     float coef;  // c_t
     float gy;    // c_t (p_y - 1): the target entry of the gradient row
     bool trig;
+    bool dual;   // Eq. (2): A < 0 and the floor c A is the active term
 };
 
 // a3: ratio, clip, normalizer (Eq. 1), fp32.
+//
+// dual_c > 1 adds Eq. (2) (reading A7): for A < 0 the inner min is
+// capped from below by dual_c * A; a hit (floor strictly larger) has zero gradient.
 //
 // lse_rest is the log-sum-exp of the row WITHOUT its target entry (of the whole row when the
 // token is not valid).  With d = lse_rest - z_y:  l_t = -softplus(d),  1 - p_y = sigmoid(d).
@@ -73,8 +78,9 @@ struct TokenScalars {
 // (DESIGN.md "Numerics").
 __device__ __forceinline__ TokenScalars token_scalars(const RowHeader& h, float lse_rest,
                                                       bool valid, float clip_eps,
-                                                      float stale_cap) {
+                                                      float stale_cap, float dual_c) {
     TokenScalars t;
+    t.dual = false;
     if (!valid) {
         t.lp = 0.f; t.lse = lse_rest; t.term = 0.f; t.coef = 0.f; t.gy = 0.f; t.trig = false;
         return t;
@@ -92,8 +98,14 @@ __device__ __forceinline__ TokenScalars token_scalars(const RowHeader& h, float 
     float v = fminf(fmaxf(r, 1.0f - clip_eps), 1.0f + clip_eps) * h.A;
     t.trig = v < u;
     float sw = h.scale * w;
-    t.term = sw * fminf(u, v);
-    t.coef = t.trig ? 0.f : sw * u;
+    float s = fminf(u, v);
+    if (dual_c > 1.0f && h.A < 0.f) {
+        const float floor_ = dual_c * h.A;
+        t.dual = floor_ > s;
+        s = fmaxf(s, floor_);
+    }
+    t.term = sw * s;
+    t.coef = (t.trig || t.dual) ? 0.f : sw * u;
     t.gy = -t.coef * one_minus_p;
     return t;
 }
@@ -131,6 +143,7 @@ struct RowArgs {
     uint8_t* tok_flag;
     uint32_t* err_word;
     float clip_eps, stale_cap;
+    float dual_c;         // Eq. (2) constant; <= 1 = off
 };
 
 // Loads the row header for token t (one thread).  Sets the error bit for y >= V.
@@ -164,7 +177,7 @@ __device__ __forceinline__ void store_token_outputs(const RowArgs& a, int64_t t,
                                                     bool valid) {
     a.token_lp[t] = ts.lp;
     a.tok_term[t] = ts.term;
-    a.tok_flag[t] = ts.trig ? kFlagTrig : 0;
+    a.tok_flag[t] = (ts.trig ? kFlagTrig : 0) | (ts.dual ? kFlagDual : 0);
     if (a.tok_coef) a.tok_coef[t] = ts.coef;
     if (a.target_logit) a.target_logit[t] = valid ? h.zy : 0.f;
 }

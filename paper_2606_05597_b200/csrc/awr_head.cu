@@ -354,7 +354,7 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
     h.A = traj >= 0 ? a.adv[traj] : 0.f;
     h.scale = traj >= 0 ? a.traj_scale[traj] : 0.f;
     h.zy = valid ? zy[row] : 0.f;
-    const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap);
+    const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
     if (lane == 0) {
         if (h.y >= a.V) atomicOr(a.err_word, AWR_ERRBIT_TARGET_RANGE);
         store_token_outputs(a, row, h, ts, valid);

@@ -17,7 +17,8 @@ cudaError_t launch_group_advantage(const float* rewards, const int32_t* group_of
                                    float loss_scale, float* adv, float* traj_scale,
                                    cudaStream_t st);
 cudaError_t launch_final_reduce(const float* tok_term, const uint8_t* tok_flag, int64_t n_tok,
-                                float* loss, int64_t* clip_count, cudaStream_t st);
+                                float* loss, int64_t* clip_count, int64_t* dual_count,
+                                cudaStream_t st);
 
 // a2 + a3 + a4, one CTA per row, any V / dtype (second pass re-reads the row through L2).
 cudaError_t launch_rows_generic(const RowArgs& a, int dtype, int num_sms, cudaStream_t st);

@@ -311,7 +311,7 @@ rows_cluster_kernel(RowArgs a, ClusterPlan p) {
         const bool valid = ctrl->hdr_valid[par] != 0;
 
         // ---- a3: per-token scalars (every thread, identical arithmetic)
-        const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap);
+        const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
         const float lse = ts.lse;
         if (tid == 0 && rank == 0) store_token_outputs(a, row, h, ts, valid);
 

@@ -110,7 +110,7 @@ rows_generic_kernel(RowArgs a) {
             for (int w = 1; w < kGenericThreads / 32; ++w) tot = combine(tot, s_red[w]);
             float lse_rest = tot.m + logf(tot.s);   // -inf when the row has no other entry
             // ---- a3
-            TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap);
+            TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
             store_token_outputs(a, row, h, ts, valid);
             s_coef = ts.coef;
             s_lse = ts.lse;

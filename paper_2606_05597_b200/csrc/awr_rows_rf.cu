@@ -297,7 +297,7 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
         const float lse_rest = M + logf(S);                   // -inf if nothing but the target
 
         // ---- a3: per-token scalars (every thread, identical arithmetic)
-        const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap);
+        const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
         if (tid == 0 && rank == 0) {
             if (h.y >= a.V) atomicOr(a.err_word, AWR_ERRBIT_TARGET_RANGE);
             store_token_outputs(a, row, h, ts, valid);

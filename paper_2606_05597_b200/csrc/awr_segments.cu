@@ -108,14 +108,16 @@ group_advantage_kernel(const float* __restrict__ rewards, const int32_t* __restr
 // then a fixed tree), clip_count = number of trigger flags.  One block: n_tok <= a few 10^5.
 __global__ void __launch_bounds__(1024)
 final_reduce_kernel(const float* __restrict__ tok_term, const uint8_t* __restrict__ tok_flag,
-                    int64_t n_tok, float* __restrict__ loss, int64_t* __restrict__ clip_count) {
+                    int64_t n_tok, float* __restrict__ loss, int64_t* __restrict__ clip_count,
+                    int64_t* __restrict__ dual_count) {
     __shared__ double s_sum[1024];
-    __shared__ unsigned long long s_cnt[1024];
+    __shared__ unsigned long long s_cnt[1024];   // trigger count in the low, dual hits in the high 32 bits
     double acc = 0.0;
     unsigned long long cnt = 0;
     for (int64_t t = threadIdx.x; t < n_tok; t += 1024) {
         acc += (double)tok_term[t];
-        cnt += (tok_flag[t] & kFlagTrig) ? 1ull : 0ull;
+        const uint8_t f = tok_flag[t];
+        cnt += ((f & kFlagTrig) ? 1ull : 0ull) + ((f & kFlagDual) ? (1ull << 32) : 0ull);
     }
     s_sum[threadIdx.x] = acc;
     s_cnt[threadIdx.x] = cnt;
@@ -129,7 +131,8 @@ final_reduce_kernel(const float* __restrict__ tok_term, const uint8_t* __restric
     }
     if (threadIdx.x == 0) {
         *loss = (float)(-s_sum[0]);
-        *clip_count = (int64_t)s_cnt[0];
+        *clip_count = (int64_t)(s_cnt[0] & 0xffffffffull);
+        if (dual_count) *dual_count = (int64_t)(s_cnt[0] >> 32);
     }
 }
 
@@ -160,8 +163,9 @@ cudaError_t launch_group_advantage(const float* rewards, const int32_t* group_of
 }
 
 cudaError_t launch_final_reduce(const float* tok_term, const uint8_t* tok_flag, int64_t n_tok,
-                                float* loss, int64_t* clip_count, cudaStream_t st) {
-    final_reduce_kernel<<<1, 1024, 0, st>>>(tok_term, tok_flag, n_tok, loss, clip_count);
+                                float* loss, int64_t* clip_count, int64_t* dual_count,
+                                cudaStream_t st) {
+    final_reduce_kernel<<<1, 1024, 0, st>>>(tok_term, tok_flag, n_tok, loss, clip_count, dual_count);
     return cudaGetLastError();
 }
 

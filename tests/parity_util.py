@@ -2,7 +2,7 @@
 (C ABI) and the fp64 oracle on the same seeded bytes and compares element by element.
 
 Bars (BASELINE.json north_star):
-  bit-exact   tok_traj, target_logit, clip_count, err_word, the zero pattern of c_t
+  bit-exact   tok_traj, target_logit, clip_count, dual_clip_count, err_word, the zero pattern of c_t
   token_lp    |d| <= 1e-4 absolute
   loss        |d| <= 1e-5 |loss| + 1e-6 sum_t |term_t|   (second term: conditioning floor, the
               advantages sum to zero per group so the loss is a difference of large sums)
@@ -77,6 +77,10 @@ def check_scalars(gpu, ora, rows=None):
             "clip_count %d != oracle %d" % (int(g["clip_count"][0]), ora["clip_count"])
         if "err_word" in g:
             assert int(g["err_word"][0]) == ora["err_word"]
+        if "dual_clip_count" in g:
+            assert int(g["dual_clip_count"][0]) == ora["dual_clip_count"], \
+                "dual_clip_count %d != oracle %d" % (int(g["dual_clip_count"][0]),
+                                                     ora["dual_clip_count"])
         tol = LOSS_RTOL * abs(ora["loss"]) + LOSS_COND_FLOOR * np.abs(ora["term"]).sum()
         assert abs(float(g["loss"][0]) - ora["loss"]) <= tol + 1e-30, \
             "loss %r vs oracle %r (tol %g)" % (float(g["loss"][0]), ora["loss"], tol)

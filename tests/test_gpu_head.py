@@ -95,6 +95,7 @@ def _check_head(gpu, ora, w_layout):
     lp = gpu["token_lp"].cpu().numpy().astype(np.float64)
     assert np.abs(lp - ora["token_lp"]).max() <= P.LP_ATOL
     assert int(gpu["clip_count"][0]) == ora["clip_count"]
+    assert int(gpu["dual_clip_count"][0]) == ora["dual_clip_count"]
     tol = P.LOSS_RTOL * abs(ora["loss"]) + P.LOSS_COND_FLOOR * np.abs(ora["term"]).sum()
     assert abs(float(gpu["loss"][0]) - ora["loss"]) <= tol
     coef = gpu["tok_coef"].cpu().numpy()
@@ -164,6 +165,19 @@ def test_head_shapes_agree_bitwise_on_integers():
     assert torch.equal(a["tok_coef"] == 0, b["tok_coef"] == 0)
     d = (a["dhidden"].float() - b["dhidden"].float()).abs().max().item()
     assert d <= 2.0 ** -7 * a["dhidden"].float().abs().max().item()
+
+
+def test_head_dual_clip():
+    """Eq. (2) through the fused head: same scalars code as the logits path."""
+    batch = _head_batch(400, 128, 1000, seed=17, lp_mode="drift")
+    q = batch["prox_lp"].clone()
+    q[::5] -= 1.5
+    batch["prox_lp"] = q
+    gpu = _run_head(batch, dual_clip_c=3.0)
+    ora = _oracle_head(batch, dual_clip_c=3.0)
+    assert ora["dual_clip_count"] > 5
+    assert np.abs(np.log(ora["ratio"][ora["ratio"] > 0]) - np.log(3.0)).min() > 1e-4
+    _check_head(gpu, ora, A.W_K_BY_V)
 
 
 def test_head_matches_logits_path():

@@ -115,6 +115,29 @@ def test_cluster_matches_generic_bitwise_on_integers(kernel):
 
 
 @pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC] + CLUSTER_KERNELS)
+@pytest.mark.parametrize("norm", [A.NORM_CONST_K, A.NORM_PER_TRAJ])
+def test_dual_clip(kernel, norm):
+    """Eq. (2) (PAPER.md:270-275, c = 3.0 as in every GRPO run of the paper, :461): tokens with
+    A < 0 whose ratio exploded past c are floored at c A, counted, and carry no gradient.  Every
+    5th token gets its prox log-prob lowered by 1.5 (r x 4.5), keeping the generator's guard
+    band around 1 +- eps and adding one around c."""
+    w = W.workload(3, n_groups=6, group_size=4, n_tok=420, V=40_000, normalizer=norm)
+    batch = W.make_batch(w, seed=31, device=DEV)
+    q = batch["prox_lp"].clone()
+    q[::5] -= 1.5
+    batch["prox_lp"] = q
+    batch["params"]["kernel"] = kernel
+    lp = P.run_gpu(batch, backward=False)["token_lp"]
+    near = ((lp - q) - float(np.log(3.0))).abs() < 1e-4          # keep log r away from log c
+    batch["prox_lp"] = torch.where(near, q - 0.01, q)
+    gpu, ora = P.full_check(batch, dual_clip_c=3.0)
+    assert ora["dual_clip_count"] > 5 and ora["clip_count"] > 0
+    off, _ = P.full_check(batch, dual_clip_c=0.0)
+    assert int(off["dual_clip_count"][0]) == 0
+    P.full_check(batch, backward=False, dual_clip_c=3.0)
+
+
+@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC] + CLUSTER_KERNELS)
 def test_in_place(kernel):
     """dlogits may alias logits exactly (include/awr.h)."""
     w = W.workload(3, n_groups=4, group_size=4, n_tok=300, V=40_000)
