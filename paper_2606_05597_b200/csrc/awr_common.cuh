@@ -25,6 +25,21 @@ __device__ __forceinline__ float ex2_approx(float x) {
     return y;
 }
 
+__device__ __forceinline__ float lg2_approx(float x) {
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// exp / log on the special-function unit (2 ulp ex2 / lg2 + one rounding of the scaled argument):
+// a3 runs redundantly in every thread between the passes of a row, so its latency is on the
+// critical path of every row; libm's expf / logf / log1pf cost ~1.2 k clocks there (measured).
+__device__ __forceinline__ float fast_exp(float x) { return ex2_approx(x * kLog2e); }
+__device__ __forceinline__ float fast_log(float x) { return lg2_approx(x) * kLn2; }
+// log(1 + e) for e in [0, 1]: the series below 2^-12 (where 1 + e would round e away)
+__device__ __forceinline__ float fast_log1p01(float e) {
+    return e < 2.44140625e-4f ? e * (1.0f - 0.5f * e) : fast_log(1.0f + e);
+}
+
 // (max, sum of exp(x - max)) pairs: the online log-sum-exp state.  m = -inf, s = 0 is the
 // identity.  Combination is written so that the identity never produces NaN.
 struct MaxSum {
@@ -86,13 +101,13 @@ __device__ __forceinline__ TokenScalars token_scalars(const RowHeader& h, float 
         return t;
     }
     const float d = lse_rest - h.zy;                  // -inf if the row has no other entry
-    const float e = expf(-fabsf(d));                  // in [0, 1]
-    const float sp = fmaxf(d, 0.f) + log1pf(e);       // softplus(d) = -l_t
+    const float e = fast_exp(-fabsf(d));              // in [0, 1]
+    const float sp = fmaxf(d, 0.f) + fast_log1p01(e); // softplus(d) = -l_t
     const float one_minus_p = (d >= 0.f ? 1.0f : e) / (1.0f + e);   // sigmoid(d) = 1 - p_y
     t.lp = -sp;
     t.lse = h.zy + sp;
-    float r = expf(t.lp - h.q);                       // pi_theta / pi_prox
-    float w = expf(h.q - h.b);                        // pi_prox / pi_behave (staleness weight)
+    float r = fast_exp(t.lp - h.q);                   // pi_theta / pi_prox
+    float w = fast_exp(h.q - h.b);                    // pi_prox / pi_behave (staleness weight)
     if (stale_cap > 0.f && stale_cap < INFINITY) w = fminf(w, stale_cap);
     float u = r * h.A;
     float v = fminf(fmaxf(r, 1.0f - clip_eps), 1.0f + clip_eps) * h.A;

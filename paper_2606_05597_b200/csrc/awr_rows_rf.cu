@@ -202,8 +202,9 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
     if (cluster < a.n_tok) { y_next = a.target_ids[cluster]; traj_next = a.tok_traj[cluster]; }
     int par = 0;
     for (int64_t row = cluster; row < a.n_tok; row += p.num_clusters, par ^= 1) {
-        // ---- row header: every thread loads the same words (one sector each); the values are
-        // not needed before the cluster barrier, so their latency hides behind passes 0 and 1
+        // ---- row header: every thread loads the same words (one sector each).  Only the raw
+        // loads are issued here; nothing consumes them before the cluster barrier (the selects
+        // and the bf16 widening sit after it), so their latency hides behind passes 0 and 1.
         RowHeader h;
         h.y = y_next;
         const int traj = traj_next;
@@ -212,12 +213,12 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
             if (nrow < a.n_tok) { y_next = a.target_ids[nrow]; traj_next = a.tok_traj[nrow]; }
         }
         const bool valid = (h.y >= 0) && (h.y < a.V);
-        h.q = a.prox_lp[row];
-        h.b = a.behave_lp[row];
-        h.A = traj >= 0 ? a.adv[traj] : 0.f;
-        h.scale = traj >= 0 ? a.traj_scale[traj] : 0.f;
-        h.zy = valid ? __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(a.logits)[row * a.ld + h.y])
-                     : 0.f;
+        const float q_raw = a.prox_lp[row];
+        const float b_raw = a.behave_lp[row];
+        float A_raw = 0.f, scale_raw = 0.f;
+        if (traj >= 0) { A_raw = a.adv[traj]; scale_raw = a.traj_scale[traj]; }
+        unsigned short zy_raw = 0;
+        if (valid) zy_raw = reinterpret_cast<const unsigned short*>(a.logits)[row * a.ld + h.y];
         // The target entry is left out of the (max, sum) state (token_scalars works from
         // lse_rest): the warp whose part holds it masks it to -inf on the way to registers.
         const int y_unit = valid ? (h.y >> 3) - part0 : -1;
@@ -294,7 +295,9 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
         float S = (M == -INFINITY) ? 0.f : st.y * ex2_approx((st.x - M) * kLog2e);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) S += __shfl_xor_sync(kFull, S, o);
-        const float lse_rest = M + logf(S);                   // -inf if nothing but the target
+        const float lse_rest = M + fast_log(S);               // -inf if nothing but the target
+        h.q = q_raw; h.b = b_raw; h.A = A_raw; h.scale = scale_raw;
+        h.zy = __uint_as_float((uint32_t)zy_raw << 16);
 
         // ---- a3: per-token scalars (every thread, identical arithmetic)
         const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
