@@ -7,9 +7,9 @@
 //     2-CTA thread-block cluster and each half (148 KB) lives in the REGISTER FILE of its SM:
 //     16 warps x 32 lanes x up to 20 packed 16-byte units per lane.
 //   * Shared memory is a pure FIFO between HBM and the registers: every warp owns a ring of
-//     2 KB slots that TMA bulk copies (cp.async.bulk + mbarrier complete_tx) fill with its part
+//     5 KB slots that TMA bulk copies (cp.async.bulk + mbarrier complete_tx) fill with its part
 //     of the rows to come; a slot is refilled the moment the warp has moved it into registers,
-//     so up to 224 KB of loads per SM are in flight while the current row is being worked on.
+//     so the whole next row (148 KB per SM) is in flight while the current row is being worked on.
 //   * Pass 0 moves the warp's part to registers and takes its max with packed bf16x2 max.
 //     Pass 1 replaces every logit, in registers, by e = exp2((z - m_w) log2 e) rounded to bf16
 //     and sums the unrounded values in f32.  The 32 warps of the cluster exchange (m_w, s_w)
@@ -26,7 +26,12 @@
 namespace awr {
 
 constexpr int kRfParts = 32;                // warps per row (over the whole cluster)
-constexpr int kRfChunkRounds = 4;           // rounds (32 units each) per slot / per TMA copy
+// A bulk copy holds its issuing thread for ~450 clocks (measured with clock()), and a warp issues
+// the copies of its ring one after the other: with 2 KB chunks (5 per row part) the refills were
+// 2.2-2.7 k of the 5.4 k clocks of pass 0.  So chunks are as large as the ring allows: two slots of
+// 10 rounds (5 KB), i.e. two copies per row part, issued while the part is moved to registers;
+// they have the rest of the row's time to land.
+constexpr int kRfChunkRounds = 10;          // rounds (32 units each) per slot / per TMA copy
 constexpr int kRfChunkUnits = 32 * kRfChunkRounds;
 constexpr int kRfSlotBytes = kRfChunkUnits * 16;
 constexpr int kRfCtrlBytes = 2048;
@@ -34,15 +39,15 @@ constexpr int kRfMinNU = 3, kRfMaxNU = 20;
 constexpr uint32_t kNegInf2 = 0xff80ff80u;  // bf16x2 (-inf, -inf)
 
 // Two shapes of the same kernel (CL CTAs per cluster x WARPS warps per CTA = 32 parts per row):
-//   CL = 2, WARPS = 16: one CTA per SM, a row half per SM, 7 ring slots per warp (224 KB).
-//   CL = 4, WARPS = 8 : two CTAs per SM (of different rows), a row quarter per CTA, 6 ring slots
-//                       per warp (96 KB per CTA).  The two co-resident CTAs drift out of phase,
+//   CL = 2, WARPS = 16: one CTA per SM, a row half per SM, 2 ring slots of 5 KB per warp (160 KB).
+//   CL = 4, WARPS = 8 : two CTAs per SM (of different rows), a row quarter per CTA, 2 ring slots
+//                       per warp (80 KB per CTA).  The two co-resident CTAs drift out of phase,
 //                       so one's exp pass overlaps the other's load / store passes.
 template <int CL>
 struct RfShape {
     static constexpr int kWarps = kRfParts / CL;
     static constexpr int kThreads = kWarps * 32;
-    static constexpr int kSlots = CL == 2 ? 7 : 6;
+    static constexpr int kSlots = 2;
     static constexpr int kCtasPerSm = CL == 2 ? 1 : 2;
     static constexpr int kSmemBytes = kRfCtrlBytes + kWarps * kSlots * kRfSlotBytes;
 };
