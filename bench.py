@@ -41,6 +41,7 @@ METRIC = "loss+grad tokens/s at V=151,936 bf16"
 UNIT = "tokens/s"
 CPU_SAMPLE_TOK = 3072      # rows of the bounded oracle sample (about 10-30 s of CPU work)
 REF_STEP_TOK = 256         # rows per step of the --impl reference arm
+HEAD_CPU_SAMPLE_TOK = 2048  # rows of the fused-head oracle sample (three fp64 GEMMs of 2048 x 151,936)
 
 
 def algorithmic_bytes_per_token(V: int, esz: int) -> int:
@@ -414,6 +415,58 @@ def run_head(args):
         peak_src = "MEASURED_PEAKS.json bf16_tflops_sustained (of measured)"
     else:
         peak, peak_src = 1400.0, "B200_PROFILING.md fallback (of fallback)"
+    # ---- end-to-end leg: pinned host hidden / W_head in, dhidden / dw_head / loss out, through
+    # the public binding; copies inside the timed region, every step
+    e2e = None
+    if not args.no_e2e:
+        e2e_steps = args.e2e_steps or args.steps
+        hin = {k: torch.empty(batch[k].shape, dtype=batch[k].dtype, pin_memory=True).copy_(batch[k])
+               for k in ("hidden", "w_head", "target_ids", "behave_lp", "prox_lp")}
+        hout = {k: torch.empty(call.out[k].shape, dtype=call.out[k].dtype, pin_memory=True)
+                for k in ("dhidden", "dw_head", "loss", "token_lp", "clip_count")}
+        h2d = sum(t.numel() * t.element_size() for t in hin.values())
+        d2h = sum(t.numel() * t.element_size() for t in hout.values())
+
+        def e2e_step():
+            for k, t in hin.items():
+                batch[k].copy_(t, non_blocking=True)
+            call.run()
+            for k, t in hout.items():
+                t.copy_(call.out[k], non_blocking=True)
+
+        e2e_step()
+        torch.cuda.synchronize(dev)
+        barrier(world)
+        e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e_beg.record(stream)
+        for _ in range(e2e_steps):
+            e2e_step()
+        e_end.record(stream)
+        torch.cuda.synchronize(dev)
+        barrier(world)
+        e_ms, e_tok = aggregate(e_beg.elapsed_time(e_end), n_tok * e2e_steps, world, dev)
+        e2e = {"value": e_tok / (e_ms / 1e3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": e2e_steps, "ms_per_step": e_ms / e2e_steps,
+               "api": "awr_loss_fwd_bwd_fused_head on device buffers refilled from pinned host "
+                      "memory each step; dhidden, dw_head, loss, token_lp copied back",
+               "loss_matches_device_leg": float(hout["loss"][0]) == float(call.out["loss"][0])}
+
+    # ---- CPU baseline: the fused-head oracle on a bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        from oracle import awr_oracle as O
+        ws = W.workload(4, n_groups=2, group_size=8, n_tok=HEAD_CPU_SAMPLE_TOK)
+        host = W.to_host(W.make_batch(ws, seed=1234, device="cpu"))
+        oargs, okw = W.oracle_args(host)
+        t0 = time.perf_counter()
+        O.awr_loss_fwd_bwd_fused_head(*oargs, **okw)
+        dt = time.perf_counter() - t0
+        cpu = {"value": host["n_tok"] / dt, "unit": UNIT, "cores": len(os.sched_getaffinity(0)),
+               "kind": "oracle", "seconds": dt,
+               "sample": "config-4 laws cut to %d tokens, K=%d, V=%d, one pass of "
+                         "oracle.awr_loss_fwd_bwd_fused_head (fp64 numpy; its three matmuls use "
+                         "the BLAS threads numpy was built with)" % (host["n_tok"], K, V)}
+
     alg_flops = 6.0 * K * V * n_tok
     exe_ratio = 1.0 if args.head_kernel in ("auto", "stored") else 8.0 / 6.0
     achieved = alg_flops / (local_ms / args.steps / 1e3) / 1e12
@@ -435,7 +488,7 @@ def run_head(args):
                              "algorithmic_flops_per_step": alg_flops,
                              "executed_flops_per_step": alg_flops * exe_ratio,
                              "executed_tflops": achieved * exe_ratio, "peak_source": peak_src},
-                "cpu_baseline": None, "e2e": None, "gpu_launches": call.launches * args.steps,
+                "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": call.launches * args.steps,
                 "clocks": clk.summary(), "loss": float(call.out["loss"][0]),
                 "clip_count": int(call.out["clip_count"][0])}
         print(json.dumps(line), flush=True)
