@@ -137,6 +137,18 @@ def token_logprob(logits_rows, target_ids):
     return lse, lp, zy
 
 
+def token_entropy(logits_rows):
+    """Per-token entropy of the policy over the vocabulary, the paper's training diagnostic
+    ("per-token entropy"): H_t = -sum_v p_v log p_v with p = softmax(z_t),
+    evaluated as lse - sum_v p_v z_v; entries with z_v = -inf have p_v = 0 and contribute 0
+    (the limit of p log p).  SURVEY.md 8(f) rank 2."""
+    z = np.asarray(logits_rows, dtype=np.float64)
+    lse = row_logsumexp(z)
+    p = np.exp(z - lse[:, None])
+    zp = np.where(p > 0.0, z, 0.0)
+    return lse - (p * zp).sum(axis=1)
+
+
 # ----------------------------------------------------------------------------- O4..O6, O8 scalar part
 def token_terms(lp, prox_lp, behave_lp, adv_tok, scale_tok, clip_eps, stale_cap, valid,
                 dual_clip_c=0.0, want_dual=False):
@@ -223,7 +235,8 @@ def traj_scale(step_off, traj_off, group_off, k_norm, normalizer, loss_scale):
 
 def awr_loss_fwd_bwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off,
                      rewards, *, k_norm, clip_eps, stale_cap, normalizer, flags=0,
-                     loss_scale=1.0, dual_clip_c=0.0, want_dlogits=True, grad_rows=None):
+                     loss_scale=1.0, dual_clip_c=0.0, want_dlogits=True, grad_rows=None,
+                     want_entropy=False):
     """The whole hot path a0..a4 for one batch.
 
     logits: [n_tok, V] array of the *exact* input values (bf16 widened exactly by the
@@ -244,10 +257,13 @@ def awr_loss_fwd_bwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off,
     lse = np.empty(n_tok, dtype=np.float64)
     lp = np.empty(n_tok, dtype=np.float64)
     zy = np.empty(n_tok, dtype=np.float64)
+    ent = np.zeros(n_tok, dtype=np.float64)
     step = max(1, (1 << 24) // max(V, 1))             # row panels: memory only, same arithmetic
     for lo in range(0, n_tok, step):
         hi = min(n_tok, lo + step)
         lse[lo:hi], lp[lo:hi], zy[lo:hi] = token_logprob(z[lo:hi], y[lo:hi])    # O3
+        if want_entropy:
+            ent[lo:hi] = np.where(valid[lo:hi], token_entropy(z[lo:hi]), 0.0)    # 0 for masked tokens
     term, coef, trig, r, w, dual = token_terms(lp, prox_lp, behave_lp, adv[tok_traj],
                                                scale[tok_traj], clip_eps, stale_cap, valid,
                                                dual_clip_c, want_dual=True)       # O4..O6, Eq. (2)
@@ -258,6 +274,8 @@ def awr_loss_fwd_bwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off,
                tok_traj=tok_traj, target_logit=zy, lse=lse, term=term, coef=coef,
                trig=trig, ratio=r, stale_w=w, err_word=err, traj_scale=scale,
                dual=dual, dual_clip_count=int(dual.sum()))
+    if want_entropy:
+        out["token_entropy"] = ent
     if want_dlogits:
         rows = np.arange(n_tok) if grad_rows is None else np.asarray(grad_rows, dtype=np.int64)
         g = np.empty((rows.size, V), dtype=np.float64)

@@ -470,3 +470,39 @@ def test_p13_dual_clip_finite_differences():
             fd = (run(dict(host, logits=zp), dual_clip_c=3.0, want_dlogits=False)["loss"] -
                   run(dict(host, logits=zm), dual_clip_c=3.0, want_dlogits=False)["loss"]) / (2 * h)
             assert out["dlogits"][t, v] == pytest.approx(fd, abs=1e-7)
+
+
+# ------------------------------------------------------------------------------------ P14: entropy
+def test_p14_entropy_closed_forms_and_library():
+    """PAPER.md:232 / :341 per-token entropy.  Uniform logits give log V exactly; a two-point
+    distribution gives the binary entropy; a near one-hot row gives ~0; -inf entries count as
+    p = 0; a constant shift changes nothing; and the whole thing agrees with the library
+    Categorical entropy."""
+    V = 1000
+    assert O.token_entropy(np.full((1, V), 3.25))[0] == pytest.approx(math.log(V), abs=1e-12)
+    p = 0.3
+    z = np.array([[math.log(p), math.log(1 - p)]])
+    assert O.token_entropy(z)[0] == pytest.approx(-(p * math.log(p) + (1 - p) * math.log(1 - p)), abs=1e-14)
+    one_hot = np.full((1, 50), -60.0); one_hot[0, 7] = 40.0
+    assert 0.0 <= O.token_entropy(one_hot)[0] < 1e-40
+    zi = np.array([[0.5, -np.inf, 1.5, -np.inf]])
+    assert O.token_entropy(zi)[0] == pytest.approx(O.token_entropy(zi[:, [0, 2]])[0], abs=1e-15)
+    rng = np.random.default_rng(3)
+    z = rng.normal(0, 3, size=(7, 333))
+    H = O.token_entropy(z)
+    assert np.allclose(O.token_entropy(z + 11.0), H, atol=1e-12)
+    ref = torch.distributions.Categorical(logits=torch.from_numpy(z)).entropy().numpy()
+    assert np.allclose(H, ref, atol=1e-12)
+    assert np.all(H > 0) and np.all(H <= math.log(333) + 1e-12)
+
+
+def test_p14_entropy_in_the_path_and_masked_tokens():
+    host = small_batch(seed=16)
+    host["target_ids"] = host["target_ids"].copy()
+    host["target_ids"][::7] = -1
+    out = run(host, want_entropy=True)
+    H = O.token_entropy(host["logits"])
+    masked = host["target_ids"] < 0
+    assert np.all(out["token_entropy"][masked] == 0.0)
+    assert np.array_equal(out["token_entropy"][~masked], H[~masked])
+    assert "token_entropy" not in run(host)
