@@ -136,6 +136,11 @@ typedef struct awr_outputs {
     float* tok_coef;        /* [n_tok] c_t */
     uint32_t* err_word;     /* [1] OR of AWR_ERRBIT_* (0 = clean) */
     int64_t* dual_clip_count; /* [1] number of tokens hit by the dual clip (:128); 0 when off */
+    float* token_entropy;   /* [n_tok] optional: H_t = -sum_v p_v log p_v of softmax(z_t), the paper's
+                               per-token entropy diagnostic (:232, :341), from the same streaming
+                               pass; 0 for masked tokens.  Generic and register-file kernels (an
+                               explicit AWR_KERNEL_CLUSTER with it -> AWR_ERR_PARAM); ignored by
+                               awr_loss_fwd_bwd_host */
 } awr_outputs;
 
 /* a0..a4 fused: segment expansion, group advantage (:61), online log-sum-exp + target gather,

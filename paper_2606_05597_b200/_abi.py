@@ -44,7 +44,8 @@ class awr_params(C.Structure):
 class awr_outputs(C.Structure):
     _fields_ = [("loss", _vp), ("dlogits", _vp), ("token_lp", _vp), ("clip_count", _vp),
                 ("adv", _vp), ("tok_traj", _vp), ("target_logit", _vp), ("tok_term", _vp),
-                ("tok_coef", _vp), ("err_word", _vp), ("dual_clip_count", _vp)]
+                ("tok_coef", _vp), ("err_word", _vp), ("dual_clip_count", _vp),
+                ("token_entropy", _vp)]
 
 
 class awr_head_batch(C.Structure):

@@ -63,7 +63,8 @@ def alloc_outputs(n_tok, n_traj, device, like_logits=None, want=OPTIONAL_OUTPUTS
         o["dlogits"] = torch.empty_like(like_logits)
     spec = dict(adv=(n_traj, torch.float32), tok_traj=(n_tok, torch.int32),
                 target_logit=(n_tok, torch.float32), tok_term=(n_tok, torch.float32),
-                tok_coef=(n_tok, torch.float32), err_word=(1, torch.int32))
+                tok_coef=(n_tok, torch.float32), err_word=(1, torch.int32),
+                token_entropy=(n_tok, torch.float32))
     for k in want:
         n, dt = spec[k]
         o[k] = torch.empty(n, dtype=dt, device=device)
@@ -103,7 +104,7 @@ def _out_struct(o):
     return awr_outputs(_ptr(g("loss")), _ptr(g("dlogits")), _ptr(g("token_lp")),
                        _ptr(g("clip_count")), _ptr(g("adv")), _ptr(g("tok_traj")),
                        _ptr(g("target_logit")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
-                       _ptr(g("err_word")), _ptr(g("dual_clip_count")))
+                       _ptr(g("err_word")), _ptr(g("dual_clip_count")), _ptr(g("token_entropy")))
 
 
 class LossCall:

@@ -87,8 +87,12 @@ static int resolve_head_stored(int requested) {
     return requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA_STORED;
 }
 
-static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype) {
+static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool want_entropy = false) {
     if (requested > AWR_KERNEL_CLUSTER_RF4) return -1;        // a fused-head kernel id
+    // token_entropy is produced by the generic and the register-file kernels
+    if (want_entropy && requested == AWR_KERNEL_CLUSTER) return -1;
+    if (want_entropy && requested == AWR_KERNEL_AUTO && V * 2 >= 65536 && !rows_rf_supported(V, ld, dtype))
+        return AWR_KERNEL_GENERIC;
     const bool ok = rows_cluster_supported(V, ld, dtype);
     const bool ok_rf = rows_rf_supported(V, ld, dtype);
     if (requested == AWR_KERNEL_CLUSTER) return ok ? AWR_KERNEL_CLUSTER : -1;
@@ -130,7 +134,7 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     if (backward && (reinterpret_cast<uintptr_t>(o->dlogits) & 15)) return AWR_ERR_ALIGN;
     const size_t need = awr_workspace_bytes(b->n_tok, b->V, b->n_steps, b->n_traj, b->n_groups);
     if (!ws_ptr || (reinterpret_cast<uintptr_t>(ws_ptr) & 255) || ws_bytes < need) return AWR_ERR_WORKSPACE;
-    const int kernel = resolve_kernel(p->kernel, b->V, b->ld, b->logits_dtype);
+    const int kernel = resolve_kernel(p->kernel, b->V, b->ld, b->logits_dtype, o->token_entropy != nullptr);
     if (kernel < 0) return AWR_ERR_PARAM;
 
     DeviceInfo info;
@@ -165,6 +169,7 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     a.tok_traj = tok_traj; a.adv = adv; a.traj_scale = w.traj_scale;
     a.token_lp = o->token_lp; a.tok_term = tok_term; a.tok_coef = o->tok_coef;
     a.target_logit = o->target_logit; a.tok_flag = w.tok_flag; a.err_word = err;
+    a.token_entropy = o->token_entropy;
     a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap; a.dual_c = p->dual_clip_c;
     cudaEvent_t ev0 = g_prof_before, ev1 = g_prof_after;
     g_prof_before = g_prof_after = nullptr;
@@ -497,6 +502,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
         a.tok_traj = d_tt + r0; a.adv = d_adv; a.traj_scale = w.traj_scale;
         a.token_lp = d_lp + r0; a.tok_term = d_term + r0; a.tok_coef = d_coef + r0;
         a.target_logit = d_tl + r0; a.tok_flag = w.tok_flag + r0; a.err_word = d_err;
+        a.token_entropy = nullptr;                       // not offered by the host-buffer entry
         a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap; a.dual_c = p->dual_clip_c;
         AWR_TRY(launch_rows(kernel, a, hb->logits_dtype, info.num_sms, s_k));
         AWR_TRY(cudaEventRecord(ev_k[bi], s_k));

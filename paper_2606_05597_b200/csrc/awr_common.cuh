@@ -63,6 +63,17 @@ __device__ __forceinline__ MaxSum warp_combine(MaxSum v) {
     return v;
 }
 
+// Entropy of the row from the state of its non-target entries: sz_rest = sum_{v != y} e^{z_v - m}
+// max(z_v, -FLT_MAX) relative to the same m as lse_rest's sum (entries at -inf contribute 0).
+//   H = lse - sum_v p_v z_v = lse - (sz_rest e^{m - lse} + p_y z_y)
+__device__ __forceinline__ float row_entropy(float lse, float m_rest, float sz_rest, float lp,
+                                             float zy) {
+    const float rest = (m_rest == -INFINITY) ? 0.f : sz_rest * ex2_approx((m_rest - lse) * kLog2e);
+    const float py = ex2_approx(lp * kLog2e);
+    return lse - (rest + (py > 0.f ? py * zy : 0.f));
+}
+constexpr float kZFloor = -3.0e38f;     // stands in for -inf in e * z (e is 0 there)
+
 // Everything the path needs to know about a row besides the row itself.
 struct RowHeader {
     int y;        // target id (already range-checked: valid <=> 0 <= y < V)
@@ -155,6 +166,7 @@ struct RowArgs {
     float* tok_term;
     float* tok_coef;      // nullable
     float* target_logit;  // nullable
+    float* token_entropy; // nullable: H_t = lse - sum_v p_v z_v (0 for masked tokens)
     uint8_t* tok_flag;
     uint32_t* err_word;
     float clip_eps, stale_cap;

@@ -51,6 +51,8 @@ rows_generic_kernel(RowArgs a) {
     using E = Elem<T>;
     constexpr int EPV = E::kPerVec;
     __shared__ MaxSum s_red[kGenericThreads / 32];
+    __shared__ float s_redz[kGenericThreads / 32];
+    const bool want_ent = a.token_entropy != nullptr;
     __shared__ float s_coef, s_lse, s_gy;
     __shared__ int s_y;
     const int tid = threadIdx.x;
@@ -70,6 +72,7 @@ rows_generic_kernel(RowArgs a) {
 
         // ---- a2: one streaming pass, per-thread online (max, sum)
         MaxSum ms{-INFINITY, 0.f};
+        float sz = 0.f;                    // sum e^{x - m} x alongside ms (entropy, optional)
         const uint4* zv = reinterpret_cast<const uint4*>(z);
         for (int64_t i = tid; i < nvec; i += kGenericThreads) {
             uint4 v = zv[i];
@@ -84,25 +87,51 @@ rows_generic_kernel(RowArgs a) {
 #pragma unroll
             for (int k = 1; k < EPV; ++k) cm = fmaxf(cm, x[k]);
             if (cm > ms.m) {
-                ms.s *= ex2_approx((ms.m - cm) * kLog2e);
+                const float sc = ex2_approx((ms.m - cm) * kLog2e);
+                ms.s *= sc;
+                sz *= sc;
                 ms.m = cm;
             }
             float ml = (ms.m == -INFINITY) ? 0.f : ms.m * kLog2e;   // all -inf so far: no NaN
             float acc = 0.f;
+            if (want_ent) {
 #pragma unroll
-            for (int k = 0; k < EPV; ++k) acc += ex2_approx(fmaf(x[k], kLog2e, -ml));
+                for (int k = 0; k < EPV; ++k) {
+                    const float e = ex2_approx(fmaf(x[k], kLog2e, -ml));
+                    acc += e;
+                    sz = fmaf(e, fmaxf(x[k], kZFloor), sz);
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < EPV; ++k) acc += ex2_approx(fmaf(x[k], kLog2e, -ml));
+            }
             ms.s += acc;
         }
         for (int64_t i = tail0 + tid; i < a.V; i += kGenericThreads) {
             float x = (i == ycol) ? -INFINITY : E::load(z + i);
             if (x > ms.m) {
-                ms.s *= ex2_approx((ms.m - x) * kLog2e);
+                const float sc = ex2_approx((ms.m - x) * kLog2e);
+                ms.s *= sc;
+                sz *= sc;
                 ms.m = x;
             }
-            if (ms.m != -INFINITY) ms.s += ex2_approx((x - ms.m) * kLog2e);
+            if (ms.m != -INFINITY) {
+                const float e = ex2_approx((x - ms.m) * kLog2e);
+                ms.s += e;
+                sz = fmaf(e, fmaxf(x, kZFloor), sz);
+            }
+        }
+        {
+            // bring this thread's sz to the warp's max before the (max, sum) state is merged
+            float wm = ms.m;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) wm = fmaxf(wm, __shfl_xor_sync(kFull, wm, o));
+            sz = (ms.m == -INFINITY) ? 0.f : sz * ex2_approx((ms.m - wm) * kLog2e);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) sz += __shfl_xor_sync(kFull, sz, o);
         }
         ms = warp_combine(ms);
-        if ((tid & 31) == 0) s_red[tid >> 5] = ms;
+        if ((tid & 31) == 0) { s_red[tid >> 5] = ms; s_redz[tid >> 5] = sz; }
         __syncthreads();
         if (tid == 0) {
             MaxSum tot = s_red[0];
@@ -112,6 +141,13 @@ rows_generic_kernel(RowArgs a) {
             // ---- a3
             TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
             store_token_outputs(a, row, h, ts, valid);
+            if (want_ent) {
+                float szt = 0.f;
+#pragma unroll
+                for (int w = 0; w < kGenericThreads / 32; ++w)
+                    if (s_red[w].m != -INFINITY) szt += s_redz[w] * ex2_approx((s_red[w].m - tot.m) * kLog2e);
+                a.token_entropy[row] = valid ? row_entropy(ts.lse, tot.m, szt, ts.lp, h.zy) : 0.f;
+            }
             s_coef = ts.coef;
             s_lse = ts.lse;
             s_y = valid ? h.y : -1;

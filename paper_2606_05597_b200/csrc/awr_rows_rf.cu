@@ -62,6 +62,7 @@ struct RfPlan {
 struct RfCtrl {
     uint64_t full[16 * 8];         // one mbarrier per ring slot per warp (8 >= slots)
     float2 stats[2][kRfParts];     // [row parity][part] (max, sum) of every warp of the cluster
+    float statz[2][kRfParts];      // [row parity][part] sum e z of the part (entropy output only)
 };
 static_assert(sizeof(RfCtrl) <= kRfCtrlBytes, "control block");
 
@@ -118,6 +119,11 @@ __device__ __forceinline__ void st_cluster_f32x2(uint32_t local_addr, uint32_t r
     asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(remote), "f"(a), "f"(b)
                  : "memory");
 }
+__device__ __forceinline__ void st_cluster_f32(uint32_t local_addr, uint32_t rank, float a) {
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(rank));
+    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(remote), "f"(a) : "memory");
+}
 __device__ __forceinline__ void lds128(uint32_t (&v)[4], uint32_t addr) {
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
                  : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
@@ -143,7 +149,7 @@ __device__ __forceinline__ uint32_t fma_bf16x2(uint32_t a, uint32_t b, uint32_t 
 // ---------------------------------------------------------------- the kernel
 // NU = rounds per warp part = ceil(max part units / 32); every round but the last is full for
 // every warp (parts differ by at most one unit and NU is exact, see make_rf_plan).
-template <int NU, int CL>
+template <int NU, int CL, bool ENT>
 __global__ void __launch_bounds__(RfShape<CL>::kThreads, RfShape<CL>::kCtasPerSm)
 rows_rf_kernel(RowArgs a, RfPlan p) {
     using namespace rf;
@@ -170,6 +176,8 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
     const int my_rows = (int)((a.n_tok - cluster + p.num_clusters - 1) / p.num_clusters);
     const int total_seq = my_rows * nch;
     const bool backward = a.dlogits != nullptr;
+    constexpr bool want_ent = ENT;        // token_entropy output (its own instantiation: the extra
+                                          // accumulator must not cost the default path anything)
     const uint8_t* lbase = reinterpret_cast<const uint8_t*>(a.logits) + (int64_t)part0 * 16;
     uint8_t* gbase = reinterpret_cast<uint8_t*>(a.dlogits) + (int64_t)part0 * 16 + lane * 16;
     const int64_t row_bytes = a.ld * 2;
@@ -273,14 +281,20 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
         // ---- pass 1: z -> e = exp2((z - m) log2 e) as bf16, in registers; f32 sum
         const float nref = (m == -INFINITY) ? 0.f : -m * kLog2e;
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
+        float accz = 0.f;                          // sum e z (entropy output; the pass is MUFU-bound)
 #pragma unroll
         for (int k = 0; k < NU; ++k) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                const float e0 = ex2_approx(fmaf(bf16_lo(v[k][j]), kLog2e, nref));
-                const float e1 = ex2_approx(fmaf(bf16_hi(v[k][j]), kLog2e, nref));
+                const float z0 = bf16_lo(v[k][j]), z1 = bf16_hi(v[k][j]);
+                const float e0 = ex2_approx(fmaf(z0, kLog2e, nref));
+                const float e1 = ex2_approx(fmaf(z1, kLog2e, nref));
                 acc[j] += e0;
                 acc[j] += e1;
+                if (want_ent) {
+                    accz = fmaf(e0, fmaxf(z0, kZFloor), accz);
+                    accz = fmaf(e1, fmaxf(z1, kZFloor), accz);
+                }
                 v[k][j] = pack_bf16x2(e0, e1);
             }
         }
@@ -290,6 +304,11 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
 
         // ---- exchange: every warp of the cluster publishes (m_w, s_w) to both CTAs
         if (lane < CL) st_cluster_f32x2(smem_u32(&ctrl->stats[par][part_idx]), (uint32_t)lane, m, s);
+        if (want_ent) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) accz += __shfl_xor_sync(kFull, accz, o);
+            if (lane < CL) st_cluster_f32(smem_u32(&ctrl->statz[par][part_idx]), (uint32_t)lane, accz);
+        }
         __syncwarp();
         cluster_arrive();
         cluster_wait();
@@ -306,6 +325,13 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
 
         // ---- a3: per-token scalars (every thread, identical arithmetic)
         const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
+        if (want_ent) {
+            float SZ = (st.x == -INFINITY) ? 0.f : ctrl->statz[par][lane] * ex2_approx((st.x - M) * kLog2e);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) SZ += __shfl_xor_sync(kFull, SZ, o);
+            if (tid == 0 && rank == 0)
+                a.token_entropy[row] = valid ? row_entropy(ts.lse, M, SZ, ts.lp, h.zy) : 0.f;
+        }
         if (tid == 0 && rank == 0) {
             if (h.y >= a.V) atomicOr(a.err_word, AWR_ERRBIT_TARGET_RANGE);
             store_token_outputs(a, row, h, ts, valid);
@@ -368,7 +394,7 @@ bool rows_rf_supported(int64_t V, int64_t ld, int dtype) {
     return make_rf_plan(V, ld, dtype, p, nu);
 }
 
-template <int NU, int CL>
+template <int NU, int CL, bool ENT>
 static cudaError_t launch_nu(const RowArgs& a, RfPlan p, int num_sms, cudaStream_t st) {
     using S = RfShape<CL>;
     static int max_clusters = -1;            // co-resident clusters (device query, cached)
@@ -384,13 +410,13 @@ static cudaError_t launch_nu(const RowArgs& a, RfPlan p, int num_sms, cudaStream
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     if (max_clusters < 0) {
-        cudaError_t e = cudaFuncSetAttribute(rows_rf_kernel<NU, CL>,
+        cudaError_t e = cudaFuncSetAttribute(rows_rf_kernel<NU, CL, ENT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              S::kSmemBytes);
         if (e != cudaSuccess) return e;
         cfg.gridDim = dim3(CL * num_sms, 1, 1);
         int n = 0;
-        e = cudaOccupancyMaxActiveClusters(&n, rows_rf_kernel<NU, CL>, &cfg);
+        e = cudaOccupancyMaxActiveClusters(&n, rows_rf_kernel<NU, CL, ENT>, &cfg);
         if (e != cudaSuccess) return e;
         const int want = num_sms * S::kCtasPerSm / CL;
         max_clusters = n < 1 ? 1 : (n > want ? want : n);
@@ -399,7 +425,7 @@ static cudaError_t launch_nu(const RowArgs& a, RfPlan p, int num_sms, cudaStream
     if ((int64_t)nc > a.n_tok) nc = (int)a.n_tok;
     p.num_clusters = nc;
     cfg.gridDim = dim3(CL * nc, 1, 1);
-    return cudaLaunchKernelEx(&cfg, rows_rf_kernel<NU, CL>, a, p);
+    return cudaLaunchKernelEx(&cfg, rows_rf_kernel<NU, CL, ENT>, a, p);
 }
 
 cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, int cluster_size, cudaStream_t st) {
@@ -409,10 +435,13 @@ cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, int cluster_size, cuda
     if (!make_rf_plan(a.V, a.ld, AWR_DTYPE_BF16, p, nu)) return cudaErrorInvalidValue;
     if (cluster_size != 2 && cluster_size != 4) return cudaErrorInvalidValue;
     switch (nu) {
-#define AWR_RF_CASE(N)                                                       \
-    case N:                                                                  \
-        return cluster_size == 2 ? launch_nu<N, 2>(a, p, num_sms, st)        \
-                                 : launch_nu<N, 4>(a, p, num_sms, st);
+#define AWR_RF_CASE(N)                                                                   \
+    case N:                                                                              \
+        if (a.token_entropy != nullptr)                                                  \
+            return cluster_size == 2 ? launch_nu<N, 2, true>(a, p, num_sms, st)          \
+                                     : launch_nu<N, 4, true>(a, p, num_sms, st);         \
+        return cluster_size == 2 ? launch_nu<N, 2, false>(a, p, num_sms, st)             \
+                                 : launch_nu<N, 4, false>(a, p, num_sms, st);
         AWR_RF_CASE(3) AWR_RF_CASE(4) AWR_RF_CASE(5) AWR_RF_CASE(6) AWR_RF_CASE(7) AWR_RF_CASE(8)
         AWR_RF_CASE(9) AWR_RF_CASE(10) AWR_RF_CASE(11) AWR_RF_CASE(12) AWR_RF_CASE(13)
         AWR_RF_CASE(14) AWR_RF_CASE(15) AWR_RF_CASE(16) AWR_RF_CASE(17) AWR_RF_CASE(18)

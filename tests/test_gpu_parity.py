@@ -137,6 +137,57 @@ def test_dual_clip(kernel, norm):
     P.full_check(batch, backward=False, dual_clip_c=3.0)
 
 
+@pytest.mark.parametrize("kernel,V,dtype", [(A.KERNEL_GENERIC, 1024, torch.float32),
+                                            (A.KERNEL_GENERIC, 1003, torch.bfloat16),
+                                            (A.KERNEL_GENERIC, 50_000, torch.bfloat16),
+                                            (A.KERNEL_CLUSTER_RF, 151_936, torch.bfloat16),
+                                            (A.KERNEL_CLUSTER_RF4, 151_936, torch.bfloat16),
+                                            (A.KERNEL_CLUSTER_RF, 40_000, torch.bfloat16),
+                                            (A.KERNEL_AUTO, 151_936, torch.bfloat16)])
+@pytest.mark.parametrize("backward", [True, False])
+def test_token_entropy(kernel, V, dtype, backward):
+    """per-token entropy from the same streaming pass,
+    forward-only (the proximal log-prob recomputation of :436) and with the gradient.  Some
+    logits are set to -inf (p = 0 entries contribute nothing); masked tokens give 0.
+    Bar: |dH| <= 1e-4 absolute (fp32 sums of e z next to the log-sum-exp)."""
+    ld = (V + 7) // 8 * 8
+    w = W.workload(3, n_groups=4, group_size=4, n_tok=300, V=V, dtype=dtype)
+    batch = W.make_batch(w, seed=41, device=DEV, ld=ld, masked_frac=0.05)
+    z = batch["logits"]
+    z[::3, 5:V:97] = float("-inf")
+    ids = batch["target_ids"].long().clamp(min=0)
+    z[torch.arange(z.shape[0], device=DEV), ids] = z[torch.arange(z.shape[0], device=DEV), ids].nan_to_num(neginf=0.0)
+    params = dict(batch["params"], kernel=kernel)
+    fn = A.awr_loss_fwd_bwd if backward else A.awr_loss_fwd
+    out = fn(z, batch["target_ids"], batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+             batch["traj_off"], batch["group_off"], batch["rewards"], V=V,
+             want=A.OPTIONAL_OUTPUTS + ("token_entropy",), **params)
+    torch.cuda.synchronize()
+    ora = P.run_oracle(batch, want_dlogits=False, want_entropy=True)
+    H = out["token_entropy"].cpu().numpy().astype(np.float64)
+    assert np.isfinite(H).all()
+    assert np.abs(H - ora["token_entropy"]).max() <= 1e-4
+    assert np.all(H[batch["target_ids"].cpu().numpy() < 0] == 0.0)
+    assert ora["token_entropy"].max() > 1.0
+    # the other outputs are what they are without the entropy output
+    ref = fn(z, batch["target_ids"], batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+             batch["traj_off"], batch["group_off"], batch["rewards"], V=V, **params)
+    torch.cuda.synchronize()
+    assert torch.equal(out["token_lp"], ref["token_lp"]) and float(out["loss"][0]) == float(ref["loss"][0])
+    if backward:
+        assert torch.equal(out["dlogits"][:, :V], ref["dlogits"][:, :V])
+
+
+def test_token_entropy_not_offered_by_the_shared_memory_cluster_kernel():
+    w = W.workload(1, n_groups=2, group_size=4, n_tok=64, V=40_000)
+    batch = W.make_batch(w, seed=1, device=DEV)
+    with pytest.raises(A.AwrError) as ei:
+        A.awr_loss_fwd(batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+                       batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"],
+                       want=("token_entropy",), **dict(batch["params"], kernel=A.KERNEL_CLUSTER))
+    assert ei.value.status == -5
+
+
 @pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC] + CLUSTER_KERNELS)
 def test_in_place(kernel):
     """dlogits may alias logits exactly (include/awr.h)."""
