@@ -46,6 +46,9 @@ NORM_CONST_K = 0      # n_i = 1 / k_norm           (the paper's fix
 NORM_PER_TRAJ = 1     # n_i = 1 / |tau_i| (steps)  (standard multi-step GRPO)
 
 FLAG_SAMPLE_STD = 1   # A2: divide by (G-1) instead of G
+FLAG_SUCCESS_FILTER = 2  # RAFT++ baseline: A_i = 1[R_i > 0], group normalisation off
+FLAG_COUPLED = 4      # coupled-ratio ablation: one pi_theta/pi_behave ratio, clip
+                      # centred on it, no staleness weight (= Eq. (1) with pi_prox := pi_behave)
 
 ERR_STEP_OFF = 1      # step_off not starting at 0 / decreasing / not ending at n_tok
 ERR_TRAJ_OFF = 2      # traj_off  ... n_steps
@@ -97,7 +100,11 @@ def group_advantage(rewards, group_off, flags=0):
     """O2: A_i = (r_i - mean(r)) / std(r) within each task group.
 
     Reading A2: population std; if every reward of the group has the same value (tested
-    on the values, -0 == +0) or the group has one member, A_i = 0 exactly; no eps."""
+    on the values, -0 == +0) or the group has one member, A_i = 0 exactly; no eps.
+    FLAG_SUCCESS_FILTER (RAFT++): "group normalization disabled and the
+    group-relative advantage replaced by a success filter (r > 0)": A_i = 1 if R_i > 0 else 0."""
+    if flags & FLAG_SUCCESS_FILTER:
+        return (np.asarray(rewards, dtype=np.float64) > 0.0).astype(np.float64)
     rewards = np.asarray(rewards, dtype=np.float64)
     group_off = np.asarray(group_off, dtype=np.int64)
     adv = np.zeros(rewards.size, dtype=np.float64)
@@ -264,6 +271,8 @@ def awr_loss_fwd_bwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off,
         lse[lo:hi], lp[lo:hi], zy[lo:hi] = token_logprob(z[lo:hi], y[lo:hi])    # O3
         if want_entropy:
             ent[lo:hi] = np.where(valid[lo:hi], token_entropy(z[lo:hi]), 0.0)    # 0 for masked tokens
+    if flags & FLAG_COUPLED:                  # the single ratio pi_theta / pi_behave
+        prox_lp = behave_lp
     term, coef, trig, r, w, dual = token_terms(lp, prox_lp, behave_lp, adv[tok_traj],
                                                scale[tok_traj], clip_eps, stale_cap, valid,
                                                dual_clip_c, want_dual=True)       # O4..O6, Eq. (2)

@@ -506,3 +506,47 @@ def test_p14_entropy_in_the_path_and_masked_tokens():
     assert np.all(out["token_entropy"][masked] == 0.0)
     assert np.array_equal(out["token_entropy"][~masked], H[~masked])
     assert "token_entropy" not in run(host)
+
+
+# ------------------------------------------------------------------------------------ P15: baselines
+def test_p15_raft_success_filter():
+    """RAFT++ (PAPER.md:65): advantage = 1[R > 0], no group normalisation, decoupled ratio kept.
+    Only successful trajectories carry gradient; with all ratios 1 the gradient is behaviour
+    cloning on the positives: scale_i (softmax - onehot) on their tokens, 0 elsewhere."""
+    assert O.group_advantage(np.array([1, 0, 0, 1, 0.5, 0, -1], dtype=np.float32), np.array([0, 4, 7]),
+                             O.FLAG_SUCCESS_FILTER).tolist() == [1, 0, 0, 1, 1, 0, 0]
+    # a single-member group (the paper runs RAFT++ with G = 1, :462) still gets A = 1[R > 0]
+    assert O.group_advantage(np.array([1.0], dtype=np.float32), np.array([0, 1]), O.FLAG_SUCCESS_FILTER)[0] == 1.0
+    host = small_batch(seed=17, normalizer=O.NORM_PER_TRAJ)
+    lp = run(host)["token_lp"]
+    host = dict(host, prox_lp=lp.astype(np.float32), behave_lp=lp.astype(np.float32))
+    out = run(host, flags=O.FLAG_SUCCESS_FILTER)
+    succ = host["rewards"][out["tok_traj"]] > 0
+    assert succ.any() and (~succ).any()
+    assert np.all(out["dlogits"][~succ] == 0)
+    z = torch.from_numpy(host["logits"].astype(np.float64))
+    p = torch.softmax(z, dim=1).numpy()
+    p[np.arange(p.shape[0]), host["target_ids"]] -= 1.0
+    r = np.exp(lp - host["prox_lp"])                      # ~1, not exactly (f32 rounding of lp)
+    expect = (out["traj_scale"][out["tok_traj"]] * r)[:, None] * p
+    assert np.allclose(out["dlogits"][succ], expect[succ], rtol=1e-9, atol=1e-15)
+
+
+def test_p15_coupled_ratio_is_eq1_with_prox_equal_behave():
+    """the coupled baseline folds staleness and update movement into one
+    pi_theta/pi_behave ratio with the clip centred on it: Eq. (1) with pi_prox := pi_behave
+    (w_t = 1), whatever prox log-probs are passed.  Literal loop as the second check."""
+    host = small_batch(seed=18, lp_mode="drift")
+    a = run(host, flags=O.FLAG_COUPLED)
+    b = run(dict(host, prox_lp=host["behave_lp"]))
+    for k in ("loss", "clip_count"):
+        assert a[k] == b[k]
+    assert np.array_equal(a["dlogits"], b["dlogits"]) and np.all(a["stale_w"] == 1.0)
+    eps = float(np.float32(host["params"]["clip_eps"]))
+    loss = 0.0
+    for t in range(host["logits"].shape[0]):
+        A = float(a["adv"][a["tok_traj"][t]])
+        rho = math.exp(a["token_lp"][t] - float(host["behave_lp"][t]))
+        loss -= float(a["traj_scale"][a["tok_traj"][t]]) * min(rho * A, min(max(rho, 1 - eps), 1 + eps) * A)
+    assert a["loss"] == pytest.approx(loss, rel=1e-12, abs=1e-15)
+    assert a["clip_count"] != run(host)["clip_count"]     # the decoupled clip is centred elsewhere
