@@ -69,7 +69,11 @@ typedef enum awr_status {
 enum { AWR_DTYPE_BF16 = 0, AWR_DTYPE_F32 = 1 };
 enum { AWR_NORM_CONST_K = 0,   /* n_i = 1 / k_norm   (:59) */
        AWR_NORM_PER_TRAJ = 1   /* n_i = 1 / |tau_i|  (:55) */ };
-enum { AWR_FLAG_SAMPLE_STD = 1u /* A2: std with 1/(G-1) instead of the default 1/G */ };
+enum { AWR_FLAG_SAMPLE_STD = 1u,     /* A2: std with 1/(G-1) instead of the default 1/G */
+       AWR_FLAG_SUCCESS_FILTER = 2u, /* RAFT++ baseline (:65): A_i = 1[R_i > 0], no group mean/std */
+       AWR_FLAG_COUPLED = 4u         /* coupled-ratio ablation (:114): one pi_theta/pi_behave ratio
+                                        with the clip centred on it, no staleness weight; prox_lp
+                                        is not read */ };
 enum { AWR_W_K_BY_V = 0 /* w_head[k * V + v] */, AWR_W_V_BY_K = 1 /* w_head[v * K + k] */ };
 enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_GENERIC = 1,  /* one CTA per row, second pass re-reads the row through L2 */

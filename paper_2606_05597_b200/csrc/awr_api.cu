@@ -65,7 +65,8 @@ static int check_params(const awr_params* p) {
     if (!isfinite(p->loss_scale)) return AWR_ERR_PARAM;
     if (isnan(p->dual_clip_c)) return AWR_ERR_PARAM;          // Eq. (2): > 1 = on, <= 1 = off
     if (p->normalizer != AWR_NORM_CONST_K && p->normalizer != AWR_NORM_PER_TRAJ) return AWR_ERR_PARAM;
-    if (p->flags & ~(uint32_t)AWR_FLAG_SAMPLE_STD) return AWR_ERR_PARAM;
+    if (p->flags & ~(uint32_t)(AWR_FLAG_SAMPLE_STD | AWR_FLAG_SUCCESS_FILTER | AWR_FLAG_COUPLED))
+        return AWR_ERR_PARAM;
     if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_STORED) return AWR_ERR_PARAM;
     return AWR_OK;
 }
@@ -165,7 +166,8 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     a.logits = b->logits;
     a.dlogits = backward ? o->dlogits : nullptr;
     a.n_tok = b->n_tok; a.V = b->V; a.ld = b->ld;
-    a.target_ids = b->target_ids; a.behave_lp = b->behave_lp; a.prox_lp = b->prox_lp;
+    a.target_ids = b->target_ids; a.behave_lp = b->behave_lp;
+    a.prox_lp = (p->flags & AWR_FLAG_COUPLED) ? b->behave_lp : b->prox_lp;
     a.tok_traj = tok_traj; a.adv = adv; a.traj_scale = w.traj_scale;
     a.token_lp = o->token_lp; a.tok_term = tok_term; a.tok_coef = o->tok_coef;
     a.target_logit = o->target_logit; a.tok_flag = w.tok_flag; a.err_word = err;
@@ -315,7 +317,8 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
                                    w.traj_scale, st);
     RowArgs a = {};
     a.n_tok = b->n_tok; a.V = b->V; a.ld = b->V;
-    a.target_ids = b->target_ids; a.behave_lp = b->behave_lp; a.prox_lp = b->prox_lp;
+    a.target_ids = b->target_ids; a.behave_lp = b->behave_lp;
+    a.prox_lp = (p->flags & AWR_FLAG_COUPLED) ? b->behave_lp : b->prox_lp;
     a.tok_traj = tok_traj; a.adv = adv; a.traj_scale = w.traj_scale;
     a.token_lp = o->token_lp; a.tok_term = tok_term; a.tok_coef = o->tok_coef;
     a.target_logit = nullptr; a.tok_flag = w.tok_flag; a.err_word = err;
@@ -498,7 +501,8 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
         RowArgs a;
         a.logits = buf; a.dlogits = buf;                 // in place on the panel
         a.n_tok = rows; a.V = hb->V; a.ld = hb->ld;
-        a.target_ids = d_ids + r0; a.behave_lp = d_b + r0; a.prox_lp = d_q + r0;
+        a.target_ids = d_ids + r0; a.behave_lp = d_b + r0;
+        a.prox_lp = ((p->flags & AWR_FLAG_COUPLED) ? d_b : d_q) + r0;
         a.tok_traj = d_tt + r0; a.adv = d_adv; a.traj_scale = w.traj_scale;
         a.token_lp = d_lp + r0; a.tok_term = d_term + r0; a.tok_coef = d_coef + r0;
         a.target_logit = d_tl + r0; a.tok_flag = w.tok_flag + r0; a.err_word = d_err;

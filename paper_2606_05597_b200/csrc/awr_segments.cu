@@ -85,12 +85,13 @@ group_advantage_kernel(const float* __restrict__ rewards, const int32_t* __restr
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(kFull, ss, o);
+    const bool filter = (flags & AWR_FLAG_SUCCESS_FILTER) != 0;   // RAFT++ (:65): A = 1[R > 0]
     bool zero = !differs || G == 1;                       // A2: exact zero, no eps
     float denom = (flags & AWR_FLAG_SAMPLE_STD) ? (float)(G - 1) : (float)G;
     float inv_sigma = zero ? 0.f : 1.0f / sqrtf(ss / denom);
     float kappa = 1.0f / ((float)n_groups * (float)G);    // A1
     for (int i = lo + lane; i < hi; i += 32) {
-        adv[i] = zero ? 0.f : (rewards[i] - mu) * inv_sigma;
+        adv[i] = filter ? (rewards[i] > 0.f ? 1.f : 0.f) : (zero ? 0.f : (rewards[i] - mu) * inv_sigma);
         if (traj_scale) {
             float n_i;
             if (normalizer == AWR_NORM_CONST_K) {

@@ -114,6 +114,31 @@ def test_cluster_matches_generic_bitwise_on_integers(kernel):
     assert float((a["token_lp"] - b["token_lp"]).abs().max()) < 2e-5
 
 
+@pytest.mark.parametrize("flags", [A.FLAG_SUCCESS_FILTER, A.FLAG_COUPLED,
+                                   A.FLAG_SUCCESS_FILTER | A.FLAG_COUPLED])
+@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER_RF])
+def test_baseline_variants(flags, kernel):
+    """the paper's two comparison losses by flag - RAFT++ (advantage =
+    1[R > 0]; run at group size 1 as in :462 and at 4) and the coupled-ratio
+    ablation.  The generator's guard band is around the decoupled ratio, so for
+    the coupled runs tokens whose coupled ratio sits within 1e-4 of 1 +- eps get a nudge."""
+    for gs in (1, 4):
+        w = W.workload(3, n_groups=24 // gs, group_size=gs, n_tok=400, V=40_000,
+                       normalizer=A.NORM_PER_TRAJ)
+        batch = W.make_batch(w, seed=51 + gs, device=DEV)
+        batch["params"]["kernel"] = kernel
+        if flags & A.FLAG_COUPLED:
+            lp = P.run_gpu(batch, backward=False)["token_lp"]
+            lr = lp - batch["behave_lp"]
+            near = ((lr - float(np.log1p(0.2))).abs() < 1e-4) | ((lr - float(np.log1p(-0.2))).abs() < 1e-4)
+            batch["behave_lp"] = torch.where(near, batch["behave_lp"] - 0.01, batch["behave_lp"])
+        gpu, ora = P.full_check(batch, flags=flags)
+        if flags & A.FLAG_SUCCESS_FILTER:
+            assert set(np.unique(ora["adv"]).tolist()) <= {0.0, 1.0} and ora["adv"].sum() > 0
+        if gs > 1 or (flags & A.FLAG_SUCCESS_FILTER):     # single-member groups: A = 0 without the filter
+            assert (ora["coef"] != 0).any()
+
+
 @pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC] + CLUSTER_KERNELS)
 @pytest.mark.parametrize("norm", [A.NORM_CONST_K, A.NORM_PER_TRAJ])
 def test_dual_clip(kernel, norm):
