@@ -47,6 +47,8 @@ NORM_PER_TRAJ = 1     # n_i = 1 / |tau_i| (steps)  (standard multi-
 
 FLAG_SAMPLE_STD = 1   # A2: divide by (G-1) instead of G
 FLAG_SUCCESS_FILTER = 2  # RAFT++ baseline: A_i = 1[R_i > 0], group normalisation off
+FLAG_SKIP_UNIFORM = 8  # dynamic sampling (DAPO): all-success / all-failure groups are
+                       # skipped - zero advantage AND left out of the mean over groups
 FLAG_COUPLED = 4      # coupled-ratio ablation: one pi_theta/pi_behave ratio, clip
                       # centred on it, no staleness weight (= Eq. (1) with pi_prox := pi_behave)
 
@@ -95,6 +97,15 @@ def segment_expand(step_off, traj_off, group_off):
                 traj_steps=traj_steps, group_size=group_size)
 
 
+def mixed_groups(rewards, group_off):
+    """PAPER.md:63 dynamic sampling: a group is *mixed* if its rewards are not all equal
+    (neither all-success nor all-failure); single-member and empty groups are not."""
+    R = np.asarray(rewards)
+    go = np.asarray(group_off)
+    return np.array([bool(np.any(R[int(go[g]):int(go[g + 1])] != R[int(go[g])]))
+                     if go[g + 1] > go[g] else False for g in range(go.size - 1)], dtype=bool)
+
+
 # ----------------------------------------------------------------------------- O2
 def group_advantage(rewards, group_off, flags=0):
     """O2: A_i = (r_i - mean(r)) / std(r) within each task group.
@@ -104,7 +115,13 @@ def group_advantage(rewards, group_off, flags=0):
     FLAG_SUCCESS_FILTER (RAFT++): "group normalization disabled and the
     group-relative advantage replaced by a success filter (r > 0)": A_i = 1 if R_i > 0 else 0."""
     if flags & FLAG_SUCCESS_FILTER:
-        return (np.asarray(rewards, dtype=np.float64) > 0.0).astype(np.float64)
+        adv = (np.asarray(rewards, dtype=np.float64) > 0.0).astype(np.float64)
+        if flags & FLAG_SKIP_UNIFORM:
+            mixed = mixed_groups(rewards, group_off)
+            for g in range(np.asarray(group_off).size - 1):
+                if not mixed[g]:
+                    adv[int(group_off[g]):int(group_off[g + 1])] = 0.0
+        return adv
     rewards = np.asarray(rewards, dtype=np.float64)
     group_off = np.asarray(group_off, dtype=np.int64)
     adv = np.zeros(rewards.size, dtype=np.float64)
@@ -223,12 +240,17 @@ def dlogits_rows(logits_rows, target_ids, lse, coef):
 
 
 # ----------------------------------------------------------------------------- the whole path
-def traj_scale(step_off, traj_off, group_off, k_norm, normalizer, loss_scale):
+def traj_scale(step_off, traj_off, group_off, k_norm, normalizer, loss_scale, rewards=None,
+               flags=0):
     """O6: scale_i = loss_scale * kappa_g * n_i with kappa_g = 1/(NG G_g) (A1) and
     n_i = 1/k_norm (PAPER.md:59) or 1/|tau_i| (PAPER.md:55)."""
     seg = segment_expand(step_off, traj_off, group_off)
     n_groups = np.asarray(group_off).size - 1
     G = seg["group_size"][seg["traj_group"]].astype(np.float64)
+    if flags & FLAG_SKIP_UNIFORM:             # the batch is the mixed groups only (PAPER.md:63)
+        n_groups = int(mixed_groups(rewards, group_off).sum())
+        if n_groups == 0:
+            return np.zeros(G.size, dtype=np.float64)
     kappa = 1.0 / (n_groups * G)
     if normalizer == NORM_CONST_K:
         n_i = np.full(G.size, 1.0 / float(np.float32(k_norm)))
@@ -258,7 +280,8 @@ def awr_loss_fwd_bwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off,
         err |= ERR_TARGET_RANGE
     seg = segment_expand(step_off, traj_off, group_off)                          # a0
     adv = group_advantage(rewards, group_off, flags)                              # O2
-    scale = traj_scale(step_off, traj_off, group_off, k_norm, normalizer, loss_scale)  # O6
+    scale = traj_scale(step_off, traj_off, group_off, k_norm, normalizer, loss_scale,
+                       rewards, flags)                                            # O6
     tok_traj = seg["tok_traj"]
     valid = (y >= 0) & (y < V)
     lse = np.empty(n_tok, dtype=np.float64)

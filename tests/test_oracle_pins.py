@@ -550,3 +550,44 @@ def test_p15_coupled_ratio_is_eq1_with_prox_equal_behave():
         loss -= float(a["traj_scale"][a["tok_traj"][t]]) * min(rho * A, min(max(rho, 1 - eps), 1 + eps) * A)
     assert a["loss"] == pytest.approx(loss, rel=1e-12, abs=1e-15)
     assert a["clip_count"] != run(host)["clip_count"]     # the decoupled clip is centred elsewhere
+
+
+# ------------------------------------------------------------------------------------ P16
+def test_p16_dynamic_sampling_skips_uniform_groups():
+    """PAPER.md:63 (DAPO dynamic sampling): all-success / all-failure groups are skipped.  The
+    result must equal the loss of the batch that physically contains only the mixed groups."""
+    w = W.workload(3, n_groups=8, group_size=4, n_tok=160, V=32, dtype=torch.float32,
+                   p_equal_groups=0.5)
+    host = W.to_host(W.make_batch(w, seed=19))
+    mixed = O.mixed_groups(host["rewards"], host["group_off"])
+    assert 0 < mixed.sum() < mixed.size
+    out = run(host, flags=O.FLAG_SKIP_UNIFORM)
+    # rebuild the batch from the mixed groups only
+    so, to, go = host["step_off"], host["traj_off"], host["group_off"]
+    keep_traj = np.concatenate([np.arange(go[g], go[g + 1]) for g in np.nonzero(mixed)[0]])
+    keep_steps = np.concatenate([np.arange(to[i], to[i + 1]) for i in keep_traj])
+    keep_tok = np.concatenate([np.arange(so[j], so[j + 1]) for j in keep_steps])
+    sub = dict(host)
+    sub["logits"] = host["logits"][keep_tok]
+    for k in ("target_ids", "behave_lp", "prox_lp"):
+        sub[k] = host[k][keep_tok]
+    sub["rewards"] = host["rewards"][keep_traj]
+    sub["step_off"] = np.concatenate([[0], np.cumsum(np.diff(so)[keep_steps])]).astype(np.int32)
+    sub["traj_off"] = np.concatenate([[0], np.cumsum(np.diff(to)[keep_traj])]).astype(np.int32)
+    sub["group_off"] = np.concatenate([[0], np.cumsum(np.diff(go)[mixed])]).astype(np.int32)
+    ref = run(sub)
+    assert out["loss"] == pytest.approx(ref["loss"], rel=1e-12, abs=1e-16)
+    assert out["clip_count"] == ref["clip_count"]
+    assert np.allclose(out["dlogits"][keep_tok], ref["dlogits"], rtol=1e-12, atol=1e-18)
+    gone = np.setdiff1d(np.arange(host["logits"].shape[0]), keep_tok)
+    assert np.all(out["dlogits"][gone] == 0)
+    # without the flag the same tokens carry 1/NG instead of 1/NG_mixed
+    base = run(host)
+    assert base["loss"] == pytest.approx(out["loss"] * mixed.sum() / mixed.size, rel=1e-12)
+    # nothing mixed -> nothing at all
+    allsame = dict(host, rewards=np.ones_like(host["rewards"]))
+    z = run(allsame, flags=O.FLAG_SKIP_UNIFORM)
+    assert z["loss"] == 0.0 and not z["dlogits"].any()
+    # with the RAFT++ filter, an all-success group is skipped too
+    r = run(allsame, flags=O.FLAG_SKIP_UNIFORM | O.FLAG_SUCCESS_FILTER)
+    assert r["loss"] == 0.0 and not r["adv"].any()
