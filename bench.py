@@ -343,7 +343,8 @@ def run_cuda(args):
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "bf16 in/out, f32 math" if esz == 2 else "f32",
                 "data": "synthetic",
-                "config": {"workload": "BASELINE.json configs[%d] (%s)" % (args.config, w.name),
+                "config": {"workload": ("BASELINE.json configs[%d] (%s)" if args.config < 5 else
+                                        "not in BASELINE.json: workload %d (%s)") % (args.config, w.name),
                            "n_tok_per_gpu": n_tok, "V": V, "n_groups": w.n_groups,
                            "group_size": w.group_size, "normalizer":
                                "1/k" if params["normalizer"] == A.NORM_CONST_K else "1/|tau_i|",
@@ -515,7 +516,8 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4, 5],
+                    help="BASELINE.json configs[i]; 5 = the Thinking-variant shapes (SURVEY 8(f) rank 4)")
     ap.add_argument("--n-tok", type=int, default=0, help="override the config's token count")
     ap.add_argument("--normalizer", type=int, default=None, choices=[0, 1])
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4"])

@@ -47,6 +47,9 @@ class Workload:
     lp_mode: str                 # "perturb" | "lag" | "drift"
     p_equal_groups: float = 0.0  # config 3: share of groups forced to all-equal rewards
     fixed: bool = False          # config 0: hand-written structure
+    tok_lo: int = 32             # response tokens per step ~ U{tok_lo..tok_hi}
+    tok_hi: int = 256
+    horizon: int | None = None   # step cap of a trajectory (PAPER.md:73: 10 / 20 / 30; :321-331)
     hidden: int | None = None    # config 4
     params: dict = field(default_factory=dict)
 
@@ -72,6 +75,13 @@ def workload(cfg: int, **over) -> Workload:
     elif cfg == 4:
         w = Workload("config4_fused_head", 16, 16, 32_768, V_QWEN, torch.bfloat16, 0.0, 0.0,
                      "lag", hidden=2048, params=dict(base))
+    elif cfg == 5:
+        # not a BASELINE.json config: SURVEY.md 8(f) rank 4, the Thinking-variant shapes
+        # (400-900 response tokens per step) under the long horizons (:321-331)
+        # 2 groups x 8 with uncut step lengths (~90k tokens, ~28 GB of logits): cutting 16 groups
+        # to a token budget would shrink the very step lengths this workload is about
+        w = Workload("next_thinking_shapes", 2, 8, None, V_QWEN, torch.bfloat16, 3.0, 4.0, "lag",
+                     tok_lo=400, tok_hi=900, horizon=40, params=dict(base))
     else:
         raise ValueError(cfg)
     for k, v in over.items():
@@ -102,7 +112,9 @@ def make_structure(w: Workload, seed: int):
                 rewards[g * w.group_size:(g + 1) * w.group_size] = common[g]
         lam = np.where(rewards > 0, 4.1, 11.5)          # 1 + Poisson: means 5.1 / 12.5
         steps = 1 + rng.poisson(lam).astype(np.int64)
-        tok_per_step = rng.integers(32, 257, size=int(steps.sum())).astype(np.int64)
+        if w.horizon is not None:
+            steps = np.minimum(steps, w.horizon)
+        tok_per_step = rng.integers(w.tok_lo, w.tok_hi + 1, size=int(steps.sum())).astype(np.int64)
         group_off = (np.arange(w.n_groups + 1) * w.group_size).astype(np.int32)
     if w.n_tok is not None and not w.fixed:
         # "cut to Ntok": keep every group / trajectory / step, rescale the step lengths

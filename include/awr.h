@@ -71,6 +71,9 @@ enum { AWR_NORM_CONST_K = 0,   /* n_i = 1 / k_norm   (:59) */
        AWR_NORM_PER_TRAJ = 1   /* n_i = 1 / |tau_i|  (:55) */ };
 enum { AWR_FLAG_SAMPLE_STD = 1u,     /* A2: std with 1/(G-1) instead of the default 1/G */
        AWR_FLAG_SUCCESS_FILTER = 2u, /* RAFT++ baseline (:65): A_i = 1[R_i > 0], no group mean/std */
+       AWR_FLAG_SKIP_UNIFORM = 8u,   /* dynamic sampling (:63): all-success / all-failure groups are
+                                        skipped on the device - zero advantage, and the mean over
+                                        groups runs over the mixed groups only (one extra launch) */
        AWR_FLAG_COUPLED = 4u         /* coupled-ratio ablation (:114): one pi_theta/pi_behave ratio
                                         with the clip centred on it, no staleness weight; prox_lp
                                         is not read */ };

@@ -21,6 +21,7 @@ NORM_CONST_K, NORM_PER_TRAJ = 0, 1
 FLAG_SAMPLE_STD = 1
 FLAG_SUCCESS_FILTER = 2
 FLAG_COUPLED = 4
+FLAG_SKIP_UNIFORM = 8
 W_K_BY_V, W_V_BY_K = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_CLUSTER, KERNEL_CLUSTER_RF, KERNEL_CLUSTER_RF4 = 0, 1, 2, 3, 4
 KERNEL_HEAD_1CTA, KERNEL_HEAD_2CTA, KERNEL_HEAD_2CTA_STORED = 5, 6, 7

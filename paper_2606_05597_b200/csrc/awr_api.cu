@@ -65,7 +65,8 @@ static int check_params(const awr_params* p) {
     if (!isfinite(p->loss_scale)) return AWR_ERR_PARAM;
     if (isnan(p->dual_clip_c)) return AWR_ERR_PARAM;          // Eq. (2): > 1 = on, <= 1 = off
     if (p->normalizer != AWR_NORM_CONST_K && p->normalizer != AWR_NORM_PER_TRAJ) return AWR_ERR_PARAM;
-    if (p->flags & ~(uint32_t)(AWR_FLAG_SAMPLE_STD | AWR_FLAG_SUCCESS_FILTER | AWR_FLAG_COUPLED))
+    if (p->flags & ~(uint32_t)(AWR_FLAG_SAMPLE_STD | AWR_FLAG_SUCCESS_FILTER | AWR_FLAG_COUPLED |
+                               AWR_FLAG_SKIP_UNIFORM))
         return AWR_ERR_PARAM;
     if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_STORED) return AWR_ERR_PARAM;
     return AWR_OK;
@@ -160,7 +161,7 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     if (e == cudaSuccess)
         e = launch_group_advantage(b->rewards, b->group_off, b->traj_off, b->n_groups, b->n_traj,
                                    p->flags, p->normalizer, p->k_norm, p->loss_scale, adv,
-                                   w.traj_scale, st);
+                                   w.traj_scale, w.err + 1, st);
     // a2 + a3 + a4
     RowArgs a;
     a.logits = b->logits;
@@ -253,7 +254,7 @@ int awr_group_advantage(const float* rewards, const int32_t* group_off, int32_t 
     if (n_traj > 0) e = cudaMemsetAsync(adv, 0, (size_t)n_traj * 4, st);
     if (e == cudaSuccess)
         e = launch_group_advantage(rewards, group_off, nullptr, n_groups, n_traj, flags,
-                                   AWR_NORM_CONST_K, 1.f, 1.f, adv, nullptr, st);
+                                   AWR_NORM_CONST_K, 1.f, 1.f, adv, nullptr, nullptr, st);
     if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
     return AWR_OK;
 }
@@ -314,7 +315,7 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     if (e == cudaSuccess)
         e = launch_group_advantage(b->rewards, b->group_off, b->traj_off, b->n_groups, b->n_traj,
                                    p->flags, p->normalizer, p->k_norm, p->loss_scale, adv,
-                                   w.traj_scale, st);
+                                   w.traj_scale, w.err + 1, st);
     RowArgs a = {};
     a.n_tok = b->n_tok; a.V = b->V; a.ld = b->V;
     a.target_ids = b->target_ids; a.behave_lp = b->behave_lp;
@@ -485,7 +486,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
     if (hb->n_traj > 0) AWR_TRY(cudaMemsetAsync(d_adv, 0, (size_t)hb->n_traj * 4, s_k));
     AWR_TRY(launch_segment_expand(d_so, d_to, d_go, n, hb->n_steps, hb->n_traj, hb->n_groups, d_tt, d_err, s_k));
     AWR_TRY(launch_group_advantage(d_rw, d_go, d_to, hb->n_groups, hb->n_traj, p->flags, p->normalizer,
-                                   p->k_norm, p->loss_scale, d_adv, w.traj_scale, s_k));
+                                   p->k_norm, p->loss_scale, d_adv, w.traj_scale, w.err + 1, s_k));
     // row panels: H2D -> kernel (in place) -> D2H, three buffers in flight
     const size_t row_bytes = (size_t)hb->ld * esz;
     int64_t panel = 0;

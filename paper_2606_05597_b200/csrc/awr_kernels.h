@@ -15,6 +15,7 @@ cudaError_t launch_group_advantage(const float* rewards, const int32_t* group_of
                                    const int32_t* traj_off, int n_groups, int n_traj,
                                    uint32_t flags, int normalizer, float k_norm,
                                    float loss_scale, float* adv, float* traj_scale,
+                                   uint32_t* n_mixed /* zeroed scratch word, nullable */,
                                    cudaStream_t st);
 cudaError_t launch_final_reduce(const float* tok_term, const uint8_t* tok_flag, int64_t n_tok,
                                 float* loss, int64_t* clip_count, int64_t* dual_count,

@@ -58,7 +58,8 @@ __global__ void __launch_bounds__(128)
 group_advantage_kernel(const float* __restrict__ rewards, const int32_t* __restrict__ group_off,
                        const int32_t* __restrict__ traj_off, int n_groups, int n_traj,
                        uint32_t flags, int normalizer, float k_norm, float loss_scale,
-                       float* __restrict__ adv, float* __restrict__ traj_scale) {
+                       float* __restrict__ adv, float* __restrict__ traj_scale,
+                       const uint32_t* __restrict__ n_mixed) {
     int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     int lane = threadIdx.x & 31;
     if (warp >= n_groups) return;
@@ -89,9 +90,15 @@ group_advantage_kernel(const float* __restrict__ rewards, const int32_t* __restr
     bool zero = !differs || G == 1;                       // A2: exact zero, no eps
     float denom = (flags & AWR_FLAG_SAMPLE_STD) ? (float)(G - 1) : (float)G;
     float inv_sigma = zero ? 0.f : 1.0f / sqrtf(ss / denom);
-    float kappa = 1.0f / ((float)n_groups * (float)G);    // A1
+    // A1: mean over groups; with dynamic sampling (:63) over the mixed groups only, and a
+    // uniform group contributes nothing at all
+    const bool skip = (flags & AWR_FLAG_SKIP_UNIFORM) != 0;
+    const bool dropped = skip && !differs;
+    const float ng = (skip && n_mixed) ? (float)(*n_mixed) : (float)n_groups;
+    float kappa = (ng > 0.f && !dropped) ? 1.0f / (ng * (float)G) : 0.f;
     for (int i = lo + lane; i < hi; i += 32) {
-        adv[i] = filter ? (rewards[i] > 0.f ? 1.f : 0.f) : (zero ? 0.f : (rewards[i] - mu) * inv_sigma);
+        adv[i] = dropped ? 0.f
+                         : (filter ? (rewards[i] > 0.f ? 1.f : 0.f) : (zero ? 0.f : (rewards[i] - mu) * inv_sigma));
         if (traj_scale) {
             float n_i;
             if (normalizer == AWR_NORM_CONST_K) {
@@ -150,16 +157,39 @@ cudaError_t launch_segment_expand(const int32_t* step_off, const int32_t* traj_o
     return cudaGetLastError();
 }
 
+// Dynamic sampling: number of groups whose rewards are not all equal.  One warp per
+// group, an integer atomic (order-independent, so the result is deterministic).
+__global__ void __launch_bounds__(128)
+count_mixed_groups_kernel(const float* __restrict__ rewards, const int32_t* __restrict__ group_off,
+                          int n_groups, int n_traj, uint32_t* __restrict__ n_mixed) {
+    int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (warp >= n_groups) return;
+    int lo = min(max(group_off[warp], 0), n_traj);
+    int hi = min(max(group_off[warp + 1], lo), n_traj);
+    if (hi <= lo) return;
+    const float first = rewards[lo];
+    bool differs = false;
+    for (int i = lo + lane; i < hi; i += 32) differs |= (rewards[i] != first);
+    differs = __any_sync(kFull, differs);
+    if (lane == 0 && differs) atomicAdd(n_mixed, 1u);
+}
+
 cudaError_t launch_group_advantage(const float* rewards, const int32_t* group_off,
                                    const int32_t* traj_off, int n_groups, int n_traj,
                                    uint32_t flags, int normalizer, float k_norm,
                                    float loss_scale, float* adv, float* traj_scale,
-                                   cudaStream_t st) {
+                                   uint32_t* n_mixed, cudaStream_t st) {
     if (n_groups <= 0) return cudaSuccess;
     int blocks = (n_groups + 3) / 4;
+    if ((flags & AWR_FLAG_SKIP_UNIFORM) && n_mixed) {       // *n_mixed was zeroed by the caller
+        count_mixed_groups_kernel<<<blocks, 128, 0, st>>>(rewards, group_off, n_groups, n_traj, n_mixed);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
     group_advantage_kernel<<<blocks, 128, 0, st>>>(rewards, group_off, traj_off, n_groups, n_traj,
                                                    flags, normalizer, k_norm, loss_scale, adv,
-                                                   traj_scale);
+                                                   traj_scale, n_mixed);
     return cudaGetLastError();
 }
 

@@ -114,6 +114,35 @@ def test_cluster_matches_generic_bitwise_on_integers(kernel):
     assert float((a["token_lp"] - b["token_lp"]).abs().max()) < 2e-5
 
 
+def test_thinking_shapes_workload():
+    """the Thinking-variant raggedness (400-900 tokens per step, horizon 40)
+    through the same kernels, cut to a size the oracle finishes in seconds."""
+    w = W.workload(5, n_groups=3, group_size=4, n_tok=700)
+    st = W.make_structure(W.workload(5), seed=0)
+    per_step = np.diff(st["step_off"])
+    assert 400 <= per_step.min() and per_step.max() <= 900 and np.diff(st["traj_off"]).max() <= 40
+    batch = W.make_batch(w, seed=71, device=DEV)
+    assert A.select_kernel(batch["V"], batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RF
+    P.full_check(batch, dual_clip_c=3.0)
+    P.full_check(batch, normalizer=A.NORM_PER_TRAJ, flags=A.FLAG_SKIP_UNIFORM)
+
+
+def test_dynamic_sampling_flag():
+    """SURVEY 8(f) rank 4 / PAPER.md:63: uniform groups skipped on the device, the mean over groups
+    runs over the mixed ones; also through the fused head and with no mixed group at all."""
+    w = W.workload(3, n_groups=12, group_size=4, n_tok=400, V=40_000, p_equal_groups=0.5)
+    batch = W.make_batch(w, seed=61, device=DEV)
+    gpu, ora = P.full_check(batch, flags=A.FLAG_SKIP_UNIFORM)
+    base, _ = P.full_check(batch)
+    mixed = O.mixed_groups(batch["rewards"].cpu().numpy(), batch["group_off"].cpu().numpy())
+    assert 0 < mixed.sum() < mixed.size
+    assert float(gpu["loss"][0]) == pytest.approx(float(base["loss"][0]) * mixed.size / mixed.sum(), rel=1e-5)
+    P.full_check(batch, flags=A.FLAG_SKIP_UNIFORM | A.FLAG_SUCCESS_FILTER)
+    batch["rewards"] = torch.ones_like(batch["rewards"])
+    z, _ = P.full_check(batch, flags=A.FLAG_SKIP_UNIFORM | A.FLAG_SUCCESS_FILTER)
+    assert float(z["loss"][0]) == 0.0 and not z["dlogits"].any()
+
+
 @pytest.mark.parametrize("flags", [A.FLAG_SUCCESS_FILTER, A.FLAG_COUPLED,
                                    A.FLAG_SUCCESS_FILTER | A.FLAG_COUPLED])
 @pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER_RF])
