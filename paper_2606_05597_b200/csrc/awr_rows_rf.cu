@@ -129,8 +129,10 @@ __device__ __forceinline__ void lds128(uint32_t (&v)[4], uint32_t addr) {
                  : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
                  : "r"(addr));
 }
+// Streaming (evict-first) stores: the gradient is written once and not read back by this kernel;
+// measured 4.61 ms against 4.74 ms with default stores on config 1 (.wt: 4.77 ms).
 __device__ __forceinline__ void stg128(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-    asm volatile("st.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(a), "r"(b), "r"(c),
+    asm volatile("st.global.cs.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(a), "r"(b), "r"(c),
                  "r"(d)
                  : "memory");
 }
