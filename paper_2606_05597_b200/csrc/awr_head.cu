@@ -101,13 +101,21 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                     if (rank == 0) mbar_expect_tx(bar, kStageBytes * CTAS);
                     if constexpr (CTAS == 2) bar = map_to_cta(bar, 0);
                     const int k0 = kb * kBK;
-                    for (uint32_t j = 0; j < g.a.boxes; ++j) {
-                        if (g.a.major == kMajorK) tma_load_2d<CTAS>(sa, &tmap_a, k0, m0, bar);
-                        else tma_load_2d<CTAS>(sa + j * g.a.box_bytes, &tmap_a, m0 + 64 * (int)j, k0, bar);
+                    if (g.a.rank3) {
+                        tma_load_3d<CTAS>(sa, &tmap_a, 0, k0, m0 >> 6, bar);
+                    } else {
+                        for (uint32_t j = 0; j < g.a.boxes; ++j) {
+                            if (g.a.major == kMajorK) tma_load_2d<CTAS>(sa, &tmap_a, k0, m0, bar);
+                            else tma_load_2d<CTAS>(sa + j * g.a.box_bytes, &tmap_a, m0 + 64 * (int)j, k0, bar);
+                        }
                     }
-                    for (uint32_t j = 0; j < g.b.boxes; ++j) {
-                        if (g.b.major == kMajorK) tma_load_2d<CTAS>(sb, &tmap_b, k0, n0, bar);
-                        else tma_load_2d<CTAS>(sb + j * g.b.box_bytes, &tmap_b, n0 + 64 * (int)j, k0, bar);
+                    if (g.b.rank3) {
+                        tma_load_3d<CTAS>(sb, &tmap_b, 0, k0, n0 >> 6, bar);
+                    } else {
+                        for (uint32_t j = 0; j < g.b.boxes; ++j) {
+                            if (g.b.major == kMajorK) tma_load_2d<CTAS>(sb, &tmap_b, k0, n0, bar);
+                            else tma_load_2d<CTAS>(sb + j * g.b.box_bytes, &tmap_b, n0 + 64 * (int)j, k0, bar);
+                        }
                     }
                     if (++stage == kStages) { stage = 0; phase ^= 1u; }
                 }
@@ -433,9 +441,11 @@ struct OperandView {
 static bool make_operand(const OperandView& v, int tile_mn, CUtensorMap* map, Operand* op) {
     EncodeTiledFn enc = encode_fn();
     if (!enc) return false;
-    cuuint64_t dims[2], strides[1];
-    cuuint32_t box[2], estr[2] = {1, 1};
+    cuuint64_t dims[3], strides[2];
+    cuuint32_t box[3], estr[3] = {1, 1, 1};
+    cuuint32_t rank = 2;
     strides[0] = (cuuint64_t)v.ld * 2;
+    op->rank3 = 0;
     if (v.major == kMajorK) {
         dims[0] = (cuuint64_t)v.kc; dims[1] = (cuuint64_t)v.mn;
         box[0] = kBK; box[1] = (cuuint32_t)tile_mn;
@@ -448,10 +458,19 @@ static bool make_operand(const OperandView& v, int tile_mn, CUtensorMap* map, Op
         op->boxes = (uint32_t)tile_mn / 64; op->box_bytes = 64 * kBK * 2;
         op->desc_lo = (uint32_t)(op->box_bytes >> 4) << 16;   // next 64-wide MN chunk
         op->k_step = (kUmmaK * 128) >> 4;             // 16 contraction rows of 128 bytes
+        if (v.mn % 64 == 0) {
+            // the same bytes as a rank-3 tensor [mn / 64][kc][64]: one copy per stage fills all the
+            // 64-wide chunks (shared-memory order chunk, k, 64 = the layout described above)
+            rank = 3;
+            op->rank3 = 1;
+            dims[0] = 64; dims[1] = (cuuint64_t)v.kc; dims[2] = (cuuint64_t)(v.mn / 64);
+            strides[0] = (cuuint64_t)v.ld * 2; strides[1] = 128;
+            box[0] = 64; box[1] = kBK; box[2] = (cuuint32_t)tile_mn / 64;
+        }
     }
     op->major = (uint32_t)v.major;
     op->desc_hi = (1024u >> 4) | (1u << 14) | (2u << 29);     // SBO 1024 B, version 1, SWIZZLE_128B
-    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(v.base), dims,
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void*>(v.base), dims,
                      strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;

@@ -67,6 +67,10 @@ enum { kEpiLse = 0,      // a2 on the tile: per-row (max, sum exp) partials + ta
 // How one operand is staged and described to the tensor core (all runtime values).
 struct Operand {
     uint32_t major;       // kMajorK / kMajorMN
+    uint32_t rank3;       // MN-major operand described as a rank-3 tensor (64 x Kc x MN/64): the
+                          // whole stage arrives with ONE bulk-tensor copy (a copy instruction
+                          // costs its issuing thread ~250-300 clocks; with one 64-wide box per
+                          // instruction the producer, not the tensor pipe, set the pace)
     uint32_t boxes;       // TMA boxes per stage
     uint32_t box_bytes;   // shared-memory bytes per box
     uint32_t desc_lo;     // leading-byte-offset field of the smem descriptor (bits 16..29)
@@ -145,6 +149,21 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         asm volatile(
             "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes "
             "[%0], [%1, {%2, %3}], [%4];" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
+            : "memory");
+    }
+}
+template <int CTAS>
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2,
+                                            uint32_t bar) {
+    if constexpr (CTAS == 1) {
+        asm volatile(
+            "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes "
+            "[%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+            : "memory");
+    } else {
+        asm volatile(
+            "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes "
+            "[%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
             : "memory");
     }
 }
