@@ -211,3 +211,34 @@ def test_head_empty_and_status_codes():
     torch.cuda.synchronize()
     assert float(out["loss"][0]) == 0.0 and int(out["clip_count"][0]) == 0
     assert not out["dw_head"].any()
+
+
+def test_head_graph_capture_and_side_stream():
+    """The fused-head call (tensor-map encodes on the host, 20+ launches, one memset) only
+    enqueues work on the caller's stream: it runs on a side stream and replays from a CUDA graph
+    with identical results."""
+    batch = _head_batch(600, 128, 2056, seed=9, lp_mode="drift")
+    call = A.HeadLossCall(batch["hidden"], batch["w_head"], batch["target_ids"], batch["behave_lp"],
+                          batch["prox_lp"], batch["step_off"], batch["traj_off"], batch["group_off"],
+                          batch["rewards"], **batch["params"])
+    ref = {k: v.clone() for k, v in call.run().items()}
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    for v in call.out.values():
+        v.zero_()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        call.run(stream=s)
+    s.synchronize()
+    for k in ref:
+        assert torch.equal(ref[k], call.out[k]), k
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            call.run(stream=s)
+    for v in call.out.values():
+        v.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    for k in ref:
+        assert torch.equal(ref[k], call.out[k]), k
