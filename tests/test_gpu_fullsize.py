@@ -1,5 +1,6 @@
 """GPU parity at BASELINE.json's FULL sizes (configs 1-3: 40,960 / 65,536 / 131,072 rows of
-V = 151,936 bf16), in the launch configuration bench.py times (kernel = AUTO, device buffers).
+V = 151,936 bf16; config 4: the fused head at 32,768 x 2048 x 151,936), in the launch
+configuration bench.py times (kernel = AUTO, device buffers).
 
 The fp64 oracle cannot do 10^10 exps in seconds, so per config:
   * sampled rows (first, last, the rows around every cluster-schedule wrap, random ones,
@@ -143,3 +144,95 @@ def test_full_size_sampled(cfg, in_place):
             d = torch.where(ok, (lp - out["token_lp"][lo:lo + 2048]).abs(), torch.zeros_like(lp))
             worst = max(worst, float(d.max()))
         assert worst <= P.LP_ATOL
+
+
+def test_full_size_fused_head_config4():
+    """BASELINE.json configs[4] at full size (32,768 x 2048 x 151,936) in the launch configuration
+    bench.py times (AUTO = CTA pairs, stored logits panel, 4 row panels).
+
+    * sampled rows against the fp64 oracle: the oracle's own steps on H[rows] W (exact fp64
+      product of the bf16 inputs): token_lp, coefficient zero pattern, and the dhidden rows
+      dS_row W^T;
+    * every row / every element against a library computation that shares nothing with the
+      kernels (torch fp32 matmul with TF32 off + log_softmax, in row chunks): token_lp on all
+      rows, dhidden and dw_head in full (relative Frobenius error <= 5e-3, DESIGN.md tolerances);
+    * properties: loss = -(sum of per-token terms), clip_count from the per-token outputs."""
+    w = W.workload(4)
+    batch = W.make_batch(w, seed=104, device=DEV)
+    n_tok, V, K = batch["n_tok"], batch["V"], w.hidden
+    assert (n_tok, V, K) == (32_768, 151_936, 2048)
+    params = dict(batch["params"])
+    out = A.awr_loss_fwd_bwd_fused_head(batch["hidden"], batch["w_head"], batch["target_ids"],
+                                        batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+                                        batch["traj_off"], batch["group_off"], batch["rewards"],
+                                        **params)
+    torch.cuda.synchronize()
+    assert int(out["err_word"][0]) == 0
+    H, Wh = batch["hidden"], batch["w_head"]
+
+    # ---- properties on all rows
+    so, to, go = (batch[k].cpu().numpy() for k in ("step_off", "traj_off", "group_off"))
+    seg = O.segment_expand(so, to, go)
+    assert np.array_equal(out["tok_traj"].cpu().numpy(), seg["tok_traj"].astype(np.int32))
+    term = out["tok_term"].double().cpu().numpy()
+    coef = out["tok_coef"].cpu().numpy()
+    assert abs(float(out["loss"][0]) + term.sum()) <= 1e-6 * abs(term.sum()) + 1e-7 * np.abs(term).sum()
+    assert int(out["clip_count"][0]) == int(((coef == 0) & (term != 0)).sum())
+
+    # ---- library reference on all rows (fp32, TF32 off)
+    prev = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = False
+    try:
+        Wf = Wh.float()
+        dW_ref = torch.zeros(K, V, dtype=torch.float32, device=DEV)
+        dH_ref = torch.empty(n_tok, K, dtype=torch.float32, device=DEV)
+        worst_lp = 0.0
+        for lo in range(0, n_tok, 2048):
+            hi = min(n_tok, lo + 2048)
+            Hf = H[lo:hi].float()
+            z = Hf @ Wf
+            lsm = torch.log_softmax(z, dim=1)
+            y = batch["target_ids"][lo:hi].long()
+            lp = lsm.gather(1, y[:, None])[:, 0]
+            worst_lp = max(worst_lp, float((lp - out["token_lp"][lo:hi]).abs().max()))
+            dS = torch.exp(lsm)
+            dS[torch.arange(hi - lo, device=DEV), y] -= 1.0
+            dS *= out["tok_coef"][lo:hi, None]
+            dH_ref[lo:hi] = dS @ Wf.t()
+            dW_ref += Hf.t() @ dS
+            del z, lsm, dS
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = prev
+    assert worst_lp <= P.LP_ATOL
+    for name, got, ref in (("dhidden", out["dhidden"].float(), dH_ref),
+                           ("dw_head", out["dw_head"].float(), dW_ref)):
+        fro = float((got - ref).norm() / ref.norm())
+        mx = float((got - ref).abs().max() / ref.abs().max())
+        assert fro <= 5e-3, "%s relative Frobenius error %.3e" % (name, fro)
+        assert mx <= 1e-2, "%s max-abs error %.3e of max|ref|" % (name, mx)
+    del dW_ref, Wf
+
+    # ---- sampled rows against the oracle
+    rng = np.random.Generator(np.random.PCG64(4))
+    rows = np.unique(np.concatenate([[0, 1, 255, 256, 9471, 9472, 9473, 28415, 28416, n_tok - 1],
+                                     rng.integers(0, n_tok, size=38)]))
+    idx = torch.as_tensor(rows, device=DEV)
+    Hs = H[idx].float().cpu().numpy().astype(np.float64)
+    Ws = Wh.float().cpu().numpy().astype(np.float64)
+    z = Hs @ Ws                                        # exact widening, fp64 product (A17)
+    y = batch["target_ids"][idx].cpu().numpy().astype(np.int64)
+    adv = O.group_advantage(batch["rewards"].cpu().numpy(), go, params.get("flags", 0))
+    scale = O.traj_scale(so, to, go, params["k_norm"], params["normalizer"], params.get("loss_scale", 1.0))
+    tt = seg["tok_traj"][rows]
+    lse, lp, zy = O.token_logprob(z, y)
+    t_, c_, trig, r_, w_ = O.token_terms(lp, batch["prox_lp"][idx].cpu().numpy(),
+                                         batch["behave_lp"][idx].cpu().numpy(), adv[tt], scale[tt],
+                                         params["clip_eps"], params["stale_cap"], np.ones(rows.size, bool))
+    assert np.abs(out["token_lp"][idx].cpu().numpy().astype(np.float64) - lp).max() <= P.LP_ATOL
+    assert np.array_equal(coef[rows] == 0, c_ == 0)
+    np.testing.assert_allclose(coef[rows], c_, rtol=2e-4, atol=1e-6 * np.abs(c_).max() + 1e-30)
+    dS = O.dlogits_rows(z, y, lse, c_)
+    dH = dS @ Ws.T
+    got = out["dhidden"][idx].float().cpu().numpy().astype(np.float64)
+    fro = np.linalg.norm(got - dH) / max(np.linalg.norm(dH), 1e-300)
+    assert fro <= 5e-3, "sampled dhidden rows: relative Frobenius error %.3e" % fro
