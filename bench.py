@@ -157,9 +157,10 @@ def oracle_sample(cfg: int, n_tok: int, seed: int):
 def time_oracle(args_kw, repeats: int = 1):
     from oracle import awr_oracle as O
     args, kw = args_kw
+    fn = O.awr_loss_fwd_bwd_fused_head if len(args) == 9 else O.awr_loss_fwd_bwd   # config 4: hidden, W
     t0 = time.perf_counter()
     for _ in range(repeats):
-        out = O.awr_loss_fwd_bwd(*args, **kw)
+        out = fn(*args, **kw)
     dt = time.perf_counter() - t0
     return dt / repeats, out
 
