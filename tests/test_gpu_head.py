@@ -242,3 +242,22 @@ def test_head_graph_capture_and_side_stream():
     torch.cuda.synchronize()
     for k in ref:
         assert torch.equal(ref[k], call.out[k]), k
+
+
+def _random_head_shapes(n, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    return [(int(rng.integers(1, 700)), 64 * int(rng.integers(1, 5)), 8 * int(rng.integers(1, 400)),
+             int(rng.integers(0, 1000))) for _ in range(n)]
+
+
+@pytest.mark.parametrize("n_tok,K,V,seed", _random_head_shapes(8, 7))
+def test_head_random_shapes(n_tok, K, V, seed):
+    """Seeded random (rows, K, V): ragged tiles in every dimension, rank-3 and rank-2 tensor maps
+    (V a multiple of 64 or not), all three kernel modes."""
+    batch = _head_batch(max(n_tok, 16), K, V, seed=seed, lp_mode="drift", masked_frac=0.02)
+    ora = _oracle_head(batch, stale_cap=2.0)
+    for kernel in HEAD_KERNELS + [A.KERNEL_HEAD_2CTA_STORED]:
+        gpu = _run_head(batch, kernel=kernel, stale_cap=2.0)
+        _check_head(gpu, ora, A.W_K_BY_V)
+    gpu = _run_head(batch, A.W_V_BY_K, stale_cap=2.0)
+    _check_head(gpu, ora, A.W_V_BY_K)

@@ -385,3 +385,31 @@ def test_graph_capture():
     torch.cuda.synchronize()
     for k in ref:
         assert torch.equal(ref[k], call.out[k]), k
+
+
+def _random_shapes(n, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    out = []
+    for _ in range(n):
+        V = int(rng.integers(16_384 // 8, 163_840 // 8 + 1)) * 8
+        ld = V + 8 * int(rng.integers(0, 3))
+        out.append((V, ld, int(rng.integers(1, 260)), int(rng.integers(0, 1 << 30))))
+    return out
+
+
+@pytest.mark.parametrize("V,ld,n_tok,seed", _random_shapes(10, 2024))
+def test_register_file_kernels_random_shapes(V, ld, n_tok, seed):
+    """Seeded random vocabulary sizes over the whole range the register-file kernels accept
+    (every NU from 3 to 20 has its own instantiation), random row strides and row counts
+    (fewer rows than clusters included), both cluster shapes, entropy on."""
+    w = W.workload(3, n_groups=3, group_size=4, n_tok=max(n_tok, 12), V=V)
+    batch = W.make_batch(w, seed=seed % 1000, device=DEV, ld=ld, masked_frac=0.05)
+    for kernel in (A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4):
+        batch["params"]["kernel"] = kernel
+        gpu, ora = P.full_check(batch, dual_clip_c=3.0)
+    out = A.awr_loss_fwd(batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+                         batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"],
+                         V=V, want=("token_entropy",), **batch["params"])
+    torch.cuda.synchronize()
+    ref = P.run_oracle(batch, want_dlogits=False, want_entropy=True)
+    assert np.abs(out["token_entropy"].cpu().numpy() - ref["token_entropy"]).max() <= 1e-4
