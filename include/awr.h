@@ -146,8 +146,7 @@ typedef struct awr_outputs {
     float* token_entropy;   /* [n_tok] optional: H_t = -sum_v p_v log p_v of softmax(z_t), the paper's
                                per-token entropy diagnostic (:232, :341), from the same streaming
                                pass; 0 for masked tokens.  Generic and register-file kernels (an
-                               explicit AWR_KERNEL_CLUSTER with it -> AWR_ERR_PARAM); ignored by
-                               awr_loss_fwd_bwd_host */
+                               explicit AWR_KERNEL_CLUSTER with it -> AWR_ERR_PARAM) */
 } awr_outputs;
 
 /* a0..a4 fused: segment expansion, group advantage (:61), online log-sum-exp + target gather,

@@ -386,7 +386,8 @@ HostPlan host_plan(int64_t n_tok, int64_t V, int64_t ld, int32_t dtype, int32_t 
     s += align_up((size_t)(n_steps + 1) * 4, 256) + align_up((size_t)(n_traj + 1) * 4, 256) +
          align_up((size_t)(n_groups + 1) * 4, 256) + align_up((size_t)n_traj * 4, 256);
     s += 256;                                      // loss, clip_count, err
-    s += align_up((size_t)n_tok * 4, 256) * 4;     // optional tok_traj, target_logit, tok_term, tok_coef
+    s += align_up((size_t)n_tok * 4, 256) * 5;     // optional tok_traj, target_logit, tok_term, tok_coef,
+                                                   // token_entropy
     s += align_up((size_t)n_traj * 4, 256);        // optional adv
     h.small_bytes = s;
     h.ws_bytes = awr_workspace_bytes(n_tok, V, n_steps, n_traj, n_groups);
@@ -419,7 +420,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
     if (((size_t)hb->ld * esz) % 16) return AWR_ERR_ALIGN;
     HostPlan hp = host_plan(hb->n_tok, hb->V, hb->ld, hb->logits_dtype, hb->n_steps, hb->n_traj, hb->n_groups);
     if (!dev_ws || (reinterpret_cast<uintptr_t>(dev_ws) & 255) || dev_ws_bytes < hp.total) return AWR_ERR_WORKSPACE;
-    const int kernel = resolve_kernel(p->kernel, hb->V, hb->ld, hb->logits_dtype);
+    const int kernel = resolve_kernel(p->kernel, hb->V, hb->ld, hb->logits_dtype, ho->token_entropy != nullptr);
     if (kernel < 0) return AWR_ERR_PARAM;
     DeviceInfo info;
     if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
@@ -442,6 +443,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
     float* d_tl = (float*)take((size_t)n * 4);
     float* d_term = (float*)take((size_t)n * 4);
     float* d_coef = (float*)take((size_t)n * 4);
+    float* d_ent = (float*)take((size_t)n * 4);
     float* d_adv = (float*)take((size_t)hb->n_traj * 4);
     off = hp.small_bytes;
     void* d_ws = base + off; off += hp.ws_bytes;
@@ -507,7 +509,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
         a.tok_traj = d_tt + r0; a.adv = d_adv; a.traj_scale = w.traj_scale;
         a.token_lp = d_lp + r0; a.tok_term = d_term + r0; a.tok_coef = d_coef + r0;
         a.target_logit = d_tl + r0; a.tok_flag = w.tok_flag + r0; a.err_word = d_err;
-        a.token_entropy = nullptr;                       // not offered by the host-buffer entry
+        a.token_entropy = ho->token_entropy ? d_ent + r0 : nullptr;
         a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap; a.dual_c = p->dual_clip_c;
         AWR_TRY(launch_rows(kernel, a, hb->logits_dtype, info.num_sms, s_k));
         AWR_TRY(cudaEventRecord(ev_k[bi], s_k));
@@ -527,6 +529,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
         if (ho->target_logit) AWR_TRY(cudaMemcpyAsync(ho->target_logit, d_tl, (size_t)n * 4, D2H, s_k));
         if (ho->tok_term) AWR_TRY(cudaMemcpyAsync(ho->tok_term, d_term, (size_t)n * 4, D2H, s_k));
         if (ho->tok_coef) AWR_TRY(cudaMemcpyAsync(ho->tok_coef, d_coef, (size_t)n * 4, D2H, s_k));
+        if (ho->token_entropy) AWR_TRY(cudaMemcpyAsync(ho->token_entropy, d_ent, (size_t)n * 4, D2H, s_k));
     }
     if (ho->adv && hb->n_traj > 0) AWR_TRY(cudaMemcpyAsync(ho->adv, d_adv, (size_t)hb->n_traj * 4, D2H, s_k));
     if (s_in) { cudaError_t e2 = cudaStreamSynchronize(s_in); if (e == cudaSuccess) e = e2; }

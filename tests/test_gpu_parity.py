@@ -413,3 +413,32 @@ def test_register_file_kernels_random_shapes(V, ld, n_tok, seed):
     torch.cuda.synchronize()
     ref = P.run_oracle(batch, want_dlogits=False, want_entropy=True)
     assert np.abs(out["token_entropy"].cpu().numpy() - ref["token_entropy"]).max() <= 1e-4
+
+
+@pytest.mark.parametrize("n_tok,V,dtype", [(7000, 40_000, torch.bfloat16), (300, 1024, torch.float32)])
+def test_host_buffer_entry(n_tok, V, dtype):
+    """awr_loss_fwd_bwd_host (the e2e leg of bench.py): pinned host buffers, row panels over three
+    device buffers (7,000 rows of 80 KB = three 256 MB panels).  Same kernels as the device entry,
+    so every output must be bit-identical to it, and it is checked against the oracle as well."""
+    w = W.workload(3, n_groups=6, group_size=4, n_tok=n_tok, V=V, dtype=dtype)
+    batch = W.make_batch(w, seed=81, device=DEV, masked_frac=0.02)
+    want = A.OPTIONAL_OUTPUTS + ("token_entropy",)
+    dev = A.awr_loss_fwd_bwd(batch["logits"], batch["target_ids"], batch["behave_lp"],
+                             batch["prox_lp"], batch["step_off"], batch["traj_off"],
+                             batch["group_off"], batch["rewards"], want=want,
+                             **dict(batch["params"], dual_clip_c=3.0))
+    torch.cuda.synchronize()
+    host_in = {k: batch[k].cpu().pin_memory() for k in ("logits", "target_ids", "behave_lp", "prox_lp",
+                                                        "step_off", "traj_off", "group_off", "rewards")}
+    out = A.awr_loss_fwd_bwd_host(host_in["logits"], host_in["target_ids"], host_in["behave_lp"],
+                                  host_in["prox_lp"], host_in["step_off"], host_in["traj_off"],
+                                  host_in["group_off"], host_in["rewards"], device=DEV, want=want,
+                                  **dict(batch["params"], dual_clip_c=3.0))
+    for k in ("loss", "clip_count", "dual_clip_count", "token_lp", "tok_term", "tok_coef", "tok_traj",
+              "target_logit", "adv", "token_entropy", "err_word", "dlogits"):
+        assert not out[k].is_cuda
+        assert torch.equal(out[k], dev[k].cpu()), k
+    ora = P.run_oracle(batch, dual_clip_c=3.0, want_entropy=True)
+    P.check_scalars({k: v for k, v in out.items() if k != "dlogits"}, ora)
+    P.check_dlogits(out["dlogits"].to(DEV), ora, V)
+    assert np.abs(out["token_entropy"].numpy() - ora["token_entropy"]).max() <= 1e-4
