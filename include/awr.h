@@ -213,6 +213,7 @@ typedef struct awr_head_outputs {
     float* tok_coef;        /* optional */
     uint32_t* err_word;     /* optional */
     int64_t* dual_clip_count; /* optional */
+    float* token_entropy;   /* optional [n_tok], as in awr_outputs (a third per-tile partial) */
 } awr_head_outputs;
 
 AWR_API int awr_loss_fwd_bwd_fused_head(const awr_head_batch* batch, const awr_params* params,

@@ -63,7 +63,8 @@ class awr_head_batch(C.Structure):
 class awr_head_outputs(C.Structure):
     _fields_ = [("loss", _vp), ("dhidden", _vp), ("dw_head", _vp), ("token_lp", _vp),
                 ("clip_count", _vp), ("adv", _vp), ("tok_traj", _vp), ("tok_term", _vp),
-                ("tok_coef", _vp), ("err_word", _vp), ("dual_clip_count", _vp)]
+                ("tok_coef", _vp), ("err_word", _vp), ("dual_clip_count", _vp),
+                ("token_entropy", _vp)]
 
 
 # name -> (restype, argtypes): every symbol include/awr.h declares

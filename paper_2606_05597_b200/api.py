@@ -308,7 +308,7 @@ class HeadLossCall:
                  dual_clip_count=torch.empty(1, dtype=torch.int64, device=dev))
         spec = dict(adv=(n_traj, torch.float32), tok_traj=(n_tok, torch.int32),
                     tok_term=(n_tok, torch.float32), tok_coef=(n_tok, torch.float32),
-                    err_word=(1, torch.int32))
+                    err_word=(1, torch.int32), token_entropy=(n_tok, torch.float32))
         for k in want:
             n, dt = spec[k]
             o[k] = torch.empty(n, dtype=dt, device=dev)
@@ -317,7 +317,8 @@ class HeadLossCall:
         self.outs = awr_head_outputs(_ptr(g("loss")), _ptr(g("dhidden")), _ptr(g("dw_head")),
                                      _ptr(g("token_lp")), _ptr(g("clip_count")), _ptr(g("adv")),
                                      _ptr(g("tok_traj")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
-                                     _ptr(g("err_word")), _ptr(g("dual_clip_count")))
+                                     _ptr(g("err_word")), _ptr(g("dual_clip_count")),
+                                     _ptr(g("token_entropy")))
         need = head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups)
         self.workspace = workspace if workspace is not None else torch.empty(
             max(need, 256), dtype=torch.uint8, device=dev)

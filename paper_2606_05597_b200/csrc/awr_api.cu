@@ -323,6 +323,7 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     a.tok_traj = tok_traj; a.adv = adv; a.traj_scale = w.traj_scale;
     a.token_lp = o->token_lp; a.tok_term = tok_term; a.tok_coef = o->tok_coef;
     a.target_logit = nullptr; a.tok_flag = w.tok_flag; a.err_word = err;
+    a.token_entropy = o->token_entropy;
     a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap; a.dual_c = p->dual_clip_c;
     HeadCall c;
     c.hidden = b->hidden; c.w_head = b->w_head; c.w_layout = b->w_layout;

@@ -189,7 +189,8 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
 
             if constexpr (EPI == kEpiLse) {
                 const int y = row_ok ? g.e.target_ids[row] : -1;
-                float m = -INFINITY, s = 0.f, zy = 0.f;
+                float m = -INFINITY, s = 0.f, zy = 0.f, sz = 0.f;
+                const bool want_ent = g.e.partz != nullptr;
                 const bool y_here = (y >= n0) && (y < n0 + kBN) && (y < g.N);
 #pragma unroll 1
                 for (int c = 0; c < kBN / 32; ++c) {
@@ -219,15 +220,28 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                     const float mn = fmaxf(m, cm);
                     if (mn != -INFINITY) {
                         const float ref = mn * kLog2e;
+                        const float resc = ex2_approx(fmaf(m, kLog2e, -ref));
                         float acc = 0.f;
+                        if (want_ent) {
+                            float accz = 0.f;
 #pragma unroll
-                        for (int j = 0; j < 32; ++j) acc += ex2_approx(fmaf(v[j], kLog2e, -ref));
-                        s = s * ex2_approx(fmaf(m, kLog2e, -ref)) + acc;
+                            for (int j = 0; j < 32; ++j) {
+                                const float e = ex2_approx(fmaf(v[j], kLog2e, -ref));
+                                acc += e;
+                                accz = fmaf(e, fmaxf(v[j], kZFloor), accz);
+                            }
+                            sz = sz * resc + accz;
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < 32; ++j) acc += ex2_approx(fmaf(v[j], kLog2e, -ref));
+                        }
+                        s = s * resc + acc;
                         m = mn;
                     }
                 }
                 if (row_ok) {
                     g.e.part[(int64_t)n_blk * g.e.part_ld + row] = make_float2(m, s);
+                    if (want_ent) g.e.partz[(int64_t)n_blk * g.e.part_ld + row] = sz;
                     if (y_here) g.e.zy[row] = zy;
                 }
             } else if constexpr (EPI == kEpiDs) {
@@ -340,7 +354,8 @@ namespace head {
 // the row without its target entry, then the same token_scalars() as the logits path.
 __global__ void __launch_bounds__(256)
 head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld, int n_tiles,
-                    const float* __restrict__ zy, float* __restrict__ row_lse,
+                    const float* __restrict__ partz, const float* __restrict__ zy,
+                    float* __restrict__ row_lse,
                     float* __restrict__ row_coef, float* __restrict__ row_gy, int64_t row0,
                     int64_t row1) {
     const int lane = threadIdx.x & 31;
@@ -352,6 +367,16 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
         st = combine(st, MaxSum{p.x, p.y});
     }
     st = warp_combine(st);
+    float sz = 0.f;
+    if (partz != nullptr) {                      // entropy: sum e^{z - M} z over the tiles
+        for (int j = lane; j < n_tiles; j += 32) {
+            const float2 p = part[(int64_t)j * part_ld + row];
+            if (p.x != -INFINITY) sz += partz[(int64_t)j * part_ld + row] * ex2_approx((p.x - st.m) * kLog2e);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sz += __shfl_xor_sync(kFull, sz, o);
+    }
+
     const float lse_rest = st.m + logf(st.s);          // -inf when nothing but the target
     RowHeader h;
     h.y = a.target_ids[row];
@@ -366,6 +391,7 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
     if (lane == 0) {
         if (h.y >= a.V) atomicOr(a.err_word, AWR_ERRBIT_TARGET_RANGE);
         store_token_outputs(a, row, h, ts, valid);
+        if (a.token_entropy) a.token_entropy[row] = valid ? row_entropy(ts.lse, st.m, sz, ts.lp, h.zy) : 0.f;
         row_lse[row] = ts.lse;
         row_coef[row] = ts.coef;
         row_gy[row] = ts.gy;
@@ -546,6 +572,7 @@ static inline size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 struct HeadWs {
     float *zy, *row_lse, *row_coef, *row_gy;
     float2* part;
+    float* partz;            // entropy output only
     __nv_bfloat16* ds;
     float* dw_acc;
     float* zpanel;           // stored-logits mode: fp32 [panel_rows, z_ld]
@@ -559,7 +586,8 @@ struct HeadWs {
 // 37 x 8 = 296 tiles = 2 x 148 CTAs (ctas = 1) or 4 x 74 CTA pairs (ctas = 2).
 static int64_t head_panel_rows(int ctas) { return ctas == 2 ? 2 * kHeadPanelRows : kHeadPanelRows; }
 
-static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ctas, bool store_z) {
+static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ctas, bool store_z,
+                         bool entropy = true) {
     HeadWs w;
     uint8_t* p = reinterpret_cast<uint8_t*>(base);
     size_t off = 0;
@@ -575,6 +603,7 @@ static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ct
     w.row_coef = (float*)take((size_t)n_pad * 4);
     w.row_gy = (float*)take((size_t)n_pad * 4);
     w.part = (float2*)take((size_t)w.n_vtiles * n_pad * 8);
+    w.partz = (float*)take(entropy ? (size_t)w.n_vtiles * n_pad * 4 : 0);
     w.ds = (__nv_bfloat16*)take((size_t)w.panel_rows * w.ds_ld * 2);
     w.dw_acc = (float*)take(w.n_panels > 1 ? (size_t)K * V * 4 : 0);
     w.z_ld = w.ds_ld;
@@ -611,6 +640,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     auto forward = [&](int64_t r0, int64_t rows, float* zout) -> cudaError_t {
         EpiArgs ea = {};
         ea.part = w.part + r0; ea.part_ld = w.part_ld; ea.zy = w.zy + r0;
+        ea.partz = c.rows->token_entropy ? w.partz + r0 : nullptr;
         ea.target_ids = c.rows->target_ids + r0;
         ea.zout = zout; ea.zout_ld = w.z_ld;
         // raster: when the H rows of this call fit in L2 (a panel: 39 MB at K = 2048) walk all of
@@ -622,6 +652,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         const int warps = 8;
         const unsigned blocks = (unsigned)((rows + warps - 1) / warps);
         head_scalars_kernel<<<blocks, warps * 32, 0, st>>>(*c.rows, w.part, w.part_ld, w.n_vtiles,
+                                                           c.rows->token_entropy ? w.partz : nullptr,
                                                            w.zy, w.row_lse, w.row_coef, w.row_gy,
                                                            r0, r0 + rows);
         return cudaGetLastError();

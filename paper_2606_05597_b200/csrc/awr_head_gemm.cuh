@@ -82,6 +82,7 @@ struct EpiArgs {
     // kEpiLse
     float2* part;              // [n_tiles][part_ld] (max, sum) of every row over one column tile
     int64_t part_ld;
+    float* partz;              // optional [n_tiles][part_ld]: sum e^{z - max} z of the tile (entropy)
     float* zy;                 // [M] gathered target logit (fp32 accumulator value)
     const int32_t* target_ids; // [M] (kEpiLse, kEpiDs), already offset to row 0 of this GEMM
     float* zout;               // optional [M, zout_ld]: the fp32 logits tile, kept for the dS pass

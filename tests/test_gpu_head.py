@@ -261,3 +261,23 @@ def test_head_random_shapes(n_tok, K, V, seed):
         _check_head(gpu, ora, A.W_K_BY_V)
     gpu = _run_head(batch, A.W_V_BY_K, stale_cap=2.0)
     _check_head(gpu, ora, A.W_V_BY_K)
+
+
+@pytest.mark.parametrize("kernel", HEAD_KERNELS + [A.KERNEL_HEAD_2CTA_STORED])
+def test_head_token_entropy(kernel):
+    """Per-token entropy from the fused head: a third per-tile partial (sum e^{z-m} z) merged
+    across the vocabulary tiles; |dH| <= 1e-4 against the oracle, 0 for masked tokens, and the
+    other outputs unchanged by asking for it."""
+    batch = _head_batch(700, 128, 3000, seed=33, lp_mode="drift", masked_frac=0.03)
+    params = dict(batch["params"], kernel=kernel)
+    args = (batch["hidden"], batch["w_head"], batch["target_ids"], batch["behave_lp"],
+            batch["prox_lp"], batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"])
+    out = A.awr_loss_fwd_bwd_fused_head(*args, want=A.api.HEAD_OPTIONAL_OUTPUTS + ("token_entropy",), **params)
+    ref = A.awr_loss_fwd_bwd_fused_head(*args, **params)
+    torch.cuda.synchronize()
+    ora = _oracle_head(batch, want_entropy=True)
+    H = out["token_entropy"].cpu().numpy().astype(np.float64)
+    assert np.abs(H - ora["token_entropy"]).max() <= 1e-4
+    assert np.all(H[batch["target_ids"].cpu().numpy() < 0] == 0.0) and ora["token_entropy"].max() > 1.0
+    for k in ("loss", "token_lp", "dhidden", "dw_head"):
+        assert torch.equal(out[k], ref[k]), k
