@@ -28,11 +28,12 @@ __device__ __forceinline__ void tile_coords(const GemmArgs& g, int tile, int& m_
     }
 }
 
-template <int EPI, int CTAS>
+template <int EPI, int CTAS, int NT>
 __global__ void __launch_bounds__(kThreads, 1)
 head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                  const __grid_constant__ CUtensorMap tmap_b, const GemmArgs g) {
-    using G = Geo<CTAS>;
+    using G = Geo<CTAS, NT>;
+    constexpr int kTN = G::kTileN;
     constexpr int kStages = G::kStages;
     constexpr int kStageBytes = G::kStageBytes;
     extern __shared__ uint8_t smem_raw[];
@@ -92,7 +93,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 int m_blk, n_blk;
                 tile_coords(g, tile, m_blk, n_blk);
                 const int m0 = m_blk * G::kTileM + (int)rank * kBM;
-                const int n0 = n_blk * kBN + (int)rank * G::kLoadN;
+                const int n0 = n_blk * kTN + (int)rank * G::kLoadN;
                 for (int kb = 0; kb < num_kb; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = smem_base + stage * kStageBytes;
@@ -109,12 +110,17 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                             else tma_load_2d<CTAS>(sa + j * g.a.box_bytes, &tmap_a, m0 + 64 * (int)j, k0, bar);
                         }
                     }
-                    if (g.b.rank3) {
-                        tma_load_3d<CTAS>(sb, &tmap_b, 0, k0, n0 >> 6, bar);
-                    } else {
-                        for (uint32_t j = 0; j < g.b.boxes; ++j) {
-                            if (g.b.major == kMajorK) tma_load_2d<CTAS>(sb, &tmap_b, k0, n0, bar);
-                            else tma_load_2d<CTAS>(sb + j * g.b.box_bytes, &tmap_b, n0 + 64 * (int)j, k0, bar);
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) {
+                        const uint32_t sbn = sb + nt * G::kBBytes1;
+                        const int nn = n0 + nt * kBN;
+                        if (g.b.rank3) {
+                            tma_load_3d<CTAS>(sbn, &tmap_b, 0, k0, nn >> 6, bar);
+                        } else {
+                            for (uint32_t j = 0; j < g.b.boxes; ++j) {
+                                if (g.b.major == kMajorK) tma_load_2d<CTAS>(sbn, &tmap_b, k0, nn, bar);
+                                else tma_load_2d<CTAS>(sbn + j * g.b.box_bytes, &tmap_b, nn + 64 * (int)j, k0, bar);
+                            }
                         }
                     }
                     if (++stage == kStages) { stage = 0; phase ^= 1u; }
@@ -131,7 +137,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
             for (int tile = tile0; tile < num_tiles; tile += tile_step) {
                 mbar_wait(tempty_bar(as), aphase ^ 1u);
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + (uint32_t)as * kBN;
+                const uint32_t d_tmem = tmem_base + (uint32_t)as * kBN;      // NT = 2: as is always 0
                 for (int kb = 0; kb < num_kb; ++kb) {
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
@@ -143,15 +149,18 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                     for (int k = 0; k < kBK / kUmmaK; ++k) {
                         const uint64_t adesc =
                             ((uint64_t)g.a.desc_hi << 32) | (uint64_t)(a_lo + k * g.a.k_step);
-                        const uint64_t bdesc =
-                            ((uint64_t)g.b.desc_hi << 32) | (uint64_t)(b_lo + k * g.b.k_step);
-                        tc_mma<CTAS>(d_tmem, adesc, bdesc, g.idesc, (uint32_t)((kb | k) != 0));
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) {
+                            const uint64_t bdesc = ((uint64_t)g.b.desc_hi << 32) |
+                                (uint64_t)(b_lo + nt * (G::kBBytes1 >> 4) + k * g.b.k_step);
+                            tc_mma<CTAS>(d_tmem + nt * kBN, adesc, bdesc, g.idesc, (uint32_t)((kb | k) != 0));
+                        }
                     }
                     tc_commit<CTAS>(empty_bar(stage));    // smem slot free once these MMAs retire
                     if (++stage == kStages) { stage = 0; phase ^= 1u; }
                 }
                 tc_commit<CTAS>(tfull_bar(as));           // accumulator tile complete
-                if (++as == 2) { as = 0; aphase ^= 1u; }
+                if (++as == G::kAccStages) { as = 0; aphase ^= 1u; }
             }
         }
     } else if (warp >= 4) {
@@ -163,7 +172,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
             int m_blk, n_blk;
             tile_coords(g, tile, m_blk, n_blk);
             const int row = m_blk * G::kTileM + (int)rank * kBM + q * 32 + lane;
-            const int n0 = n_blk * kBN;
+            const int n0 = n_blk * kTN;
             const bool row_ok = row < g.M;
             // kEpiAccum: the running fp32 sum of this thread's row is fetched one 32-column chunk
             // ahead (chunk 0 before the accumulator is even complete), so the global-memory
@@ -172,7 +181,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
             auto fetch_acc = [&](int c) {
                 if constexpr (EPI == kEpiAccum) {
                     const int c0 = n0 + c * 32;
-                    if (!g.e.first_panel && row_ok && c < kBN / 32) {
+                    if (!g.e.first_panel && row_ok && c < kTN / 32) {
                         const float* ap = g.e.acc + (int64_t)row * g.e.out_ld + c0;
 #pragma unroll
                         for (int j = 0; j < 8; ++j)
@@ -191,9 +200,9 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 const int y = row_ok ? g.e.target_ids[row] : -1;
                 float m = -INFINITY, s = 0.f, zy = 0.f, sz = 0.f;
                 const bool want_ent = g.e.partz != nullptr;
-                const bool y_here = (y >= n0) && (y < n0 + kBN) && (y < g.N);
+                const bool y_here = (y >= n0) && (y < n0 + kTN) && (y < g.N);
 #pragma unroll 1
-                for (int c = 0; c < kBN / 32; ++c) {
+                for (int c = 0; c < kTN / 32; ++c) {
                     tmem_ld32(t_addr + c * 32, v);
                     const int c0 = n0 + c * 32;
                     if (g.e.zout != nullptr && row_ok) {
@@ -254,7 +263,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 const float nref = -lse * kLog2e;
                 __nv_bfloat16* dst = g.e.ds + (int64_t)row * g.e.ds_ld + n0;
 #pragma unroll 1
-                for (int c = 0; c < kBN / 32; ++c) {
+                for (int c = 0; c < kTN / 32; ++c) {
                     tmem_ld32(t_addr + c * 32, v);
                     const int c0 = n0 + c * 32;
                     if (!row_ok || c0 >= g.N) continue;
@@ -282,7 +291,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
             } else {
                 const int64_t ro = (int64_t)row * g.e.out_ld + n0;
 #pragma unroll 1
-                for (int c = 0; c < kBN / 32; ++c) {
+                for (int c = 0; c < kTN / 32; ++c) {
                     tmem_ld32(t_addr + c * 32, v);
                     const int c0 = n0 + c * 32;
                     if (!row_ok || c0 >= g.N) continue;
@@ -324,7 +333,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 if constexpr (CTAS == 2) mbar_arrive_cluster(map_to_cta(tempty_bar(as), 0));
                 else mbar_arrive(tempty_bar(as));
             }
-            if (++as == 2) { as = 0; aphase ^= 1u; }
+            if (++as == G::kAccStages) { as = 0; aphase ^= 1u; }
         }
     }
 
@@ -502,14 +511,14 @@ static bool make_operand(const OperandView& v, int tile_mn, CUtensorMap* map, Op
     return r == CUDA_SUCCESS;
 }
 
-template <int EPI, int CTAS>
+template <int EPI, int CTAS, int NT>
 static cudaError_t launch_gemm_epi(const CUtensorMap& ta, const CUtensorMap& tb, const GemmArgs& g,
                                    int grid, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(head_gemm_kernel<EPI, CTAS>,
+        cudaError_t e = cudaFuncSetAttribute(head_gemm_kernel<EPI, CTAS, NT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             Geo<CTAS>::kSmemBytes);
+                                             Geo<CTAS, NT>::kSmemBytes);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -521,18 +530,21 @@ static cudaError_t launch_gemm_epi(const CUtensorMap& ta, const CUtensorMap& tb,
     attr[0].val.clusterDim.z = 1;
     cfg.gridDim = dim3(grid, 1, 1);
     cfg.blockDim = dim3(kThreads, 1, 1);
-    cfg.dynamicSmemBytes = Geo<CTAS>::kSmemBytes;
+    cfg.dynamicSmemBytes = Geo<CTAS, NT>::kSmemBytes;
     cfg.stream = st;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, head_gemm_kernel<EPI, CTAS>, ta, tb, g);
+    return cudaLaunchKernelEx(&cfg, head_gemm_kernel<EPI, CTAS, NT>, ta, tb, g);
 }
 
 // C[M, N] = A * B with epilogue `epi`; `order` / `group_m` pick the tile raster (group_m in row
 // tiles of 128 * ctas rows); ctas = 1: one CTA per tile, 2: a CTA pair per 256-row tile.
 static cudaError_t launch_gemm(int epi, const OperandView& A, const OperandView& B, int order,
-                               int group_m, const EpiArgs& e, int num_sms, int ctas, cudaStream_t st) {
+                               int group_m, const EpiArgs& e, int num_sms, int ctas, cudaStream_t st,
+                               bool wide = false) {
     if (A.mn <= 0 || B.mn <= 0 || A.kc <= 0) return cudaSuccess;
+    // wide: 256 x 512 tiles (kEpiStoreBf16 on CTA pairs, N a multiple of 512)
+    const int nt = (wide && ctas == 2 && epi == kEpiStoreBf16 && B.mn % (2 * kBN) == 0) ? 2 : 1;
     if (A.kc != B.kc) return cudaErrorInvalidValue;
     CUtensorMap ta, tb;
     GemmArgs g;
@@ -540,7 +552,7 @@ static cudaError_t launch_gemm(int epi, const OperandView& A, const OperandView&
     const int tile_m = kBM * ctas;
     g.M = (int32_t)A.mn; g.N = (int32_t)B.mn; g.Kc = (int32_t)A.kc;
     g.m_tiles = (g.M + tile_m - 1) / tile_m;
-    g.n_tiles = (g.N + kBN - 1) / kBN;
+    g.n_tiles = (g.N + kBN * nt - 1) / (kBN * nt);
     g.order = order; g.group_m = group_m < 1 ? 1 : group_m;
     g.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)A.major << 15) |
               ((uint32_t)B.major << 16) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)(tile_m >> 4) << 24);
@@ -550,8 +562,9 @@ static cudaError_t launch_gemm(int epi, const OperandView& A, const OperandView&
     const int grid = (int)(tiles < slots ? tiles : slots) * ctas;
 #define AWR_HEAD_CASE(E)                                                            \
     case E:                                                                         \
-        return ctas == 2 ? launch_gemm_epi<E, 2>(ta, tb, g, grid, st)               \
-                         : launch_gemm_epi<E, 1>(ta, tb, g, grid, st);
+        return ctas == 2 ? launch_gemm_epi<E, 2, 1>(ta, tb, g, grid, st)            \
+                         : launch_gemm_epi<E, 1, 1>(ta, tb, g, grid, st);
+    if (nt == 2) return launch_gemm_epi<kEpiStoreBf16, 2, 2>(ta, tb, g, grid, st);
     switch (epi) {
         AWR_HEAD_CASE(kEpiLse) AWR_HEAD_CASE(kEpiDs) AWR_HEAD_CASE(kEpiStoreBf16) AWR_HEAD_CASE(kEpiAccum)
         default: return cudaErrorInvalidValue;
@@ -688,7 +701,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         EpiArgs e2 = {};
         e2.out = reinterpret_cast<__nv_bfloat16*>(c.dhidden) + r0 * c.K; e2.out_ld = c.K;
         e = launch_gemm(kEpiStoreBf16, OperandView{w.ds, rows, c.V, w.ds_ld, kMajorK}, w_bwd, 1, 1, e2,
-                        num_sms, ctas, st);
+                        num_sms, ctas, st, /*wide=*/true);
         if (e != cudaSuccess) return e;
 
         EpiArgs e3 = {};

@@ -47,16 +47,25 @@ constexpr int kABytes = kBM * kBK * 2;      // 16 KB: 128 rows of A per CTA in b
 constexpr int kTmemCols = 512;
 constexpr int kMaxStages = 8;
 
-template <int CTAS>
+// NT = 256-column accumulators per tile.  NT = 2 (CTA pairs only): a 256 x 512 tile fills all 512
+// TMEM columns, so the accumulator is not double-buffered (the epilogue does not overlap the next
+// tile) but every staged A row is used for twice as many columns: for the dhidden GEMM, whose
+// contraction is 151,936 long and whose output is small, that cuts operand traffic by a quarter
+// and halves the number of CTA pairs that must stream the same dS rows in step.
+template <int CTAS, int NT = 1>
 struct Geo {
     static constexpr int kTileM = kBM * CTAS;            // tile rows per CTA / CTA pair
-    static constexpr int kLoadN = kBN / CTAS;            // B columns staged by one CTA
-    static constexpr int kBBytes = kLoadN * kBK * 2;     // 32 KB / 16 KB
+    static constexpr int kTileN = kBN * NT;              // tile columns
+    static constexpr int kLoadN = kBN / CTAS;            // B columns staged by one CTA per accumulator
+    static constexpr int kBBytes1 = kLoadN * kBK * 2;    // 32 KB / 16 KB
+    static constexpr int kBBytes = kBBytes1 * NT;
     static constexpr int kStageBytes = kABytes + kBBytes;
-    static constexpr int kStages = CTAS == 1 ? 4 : 7;
+    static constexpr int kStages = CTAS == 1 ? 4 : (NT == 1 ? 7 : 4);
+    static constexpr int kAccStages = 2 / NT;            // TMEM accumulator buffers
     static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment */ + 256 /* barriers */;
 };
 static_assert(Geo<2>::kStages <= kMaxStages && Geo<2>::kSmemBytes <= 232448, "shared memory");
+static_assert(Geo<2, 2>::kSmemBytes <= 232448, "shared memory");
 
 enum { kMajorK = 0, kMajorMN = 1 };
 enum { kEpiLse = 0,      // a2 on the tile: per-row (max, sum exp) partials + target gather

@@ -281,3 +281,18 @@ def test_head_token_entropy(kernel):
     assert np.all(H[batch["target_ids"].cpu().numpy() < 0] == 0.0) and ora["token_entropy"].max() > 1.0
     for k in ("loss", "token_lp", "dhidden", "dw_head"):
         assert torch.equal(out[k], ref[k]), k
+
+
+@pytest.mark.parametrize("K,n_tok", [(512, 700), (1024, 300)])
+def test_head_wide_dhidden_tiles(K, n_tok):
+    """K a multiple of 512: the dhidden GEMM of the CTA-pair modes runs on 256 x 512 tiles (one
+    undoubled 512-column TMEM accumulator).  Against the oracle, and equal to the one-CTA mode
+    within rounding."""
+    batch = _head_batch(n_tok, K, 1512, seed=44, lp_mode="drift", masked_frac=0.02)
+    ora = _oracle_head(batch, stale_cap=2.0)
+    outs = {}
+    for kernel in HEAD_KERNELS + [A.KERNEL_HEAD_2CTA_STORED]:
+        outs[kernel] = _run_head(batch, kernel=kernel, stale_cap=2.0)
+        _check_head(outs[kernel], ora, A.W_K_BY_V)
+    d = (outs[A.KERNEL_HEAD_1CTA]["dhidden"].float() - outs[A.KERNEL_HEAD_2CTA]["dhidden"].float()).abs().max()
+    assert float(d) <= 2.0 ** -7 * float(outs[A.KERNEL_HEAD_1CTA]["dhidden"].float().abs().max())
