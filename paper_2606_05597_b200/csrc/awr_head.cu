@@ -201,9 +201,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 float m = -INFINITY, s = 0.f, zy = 0.f, sz = 0.f;
                 const bool want_ent = g.e.partz != nullptr;
                 const bool y_here = (y >= n0) && (y < n0 + kTN) && (y < g.N);
-#pragma unroll 1
-                for (int c = 0; c < kTN / 32; ++c) {
-                    tmem_ld32(t_addr + c * 32, v);
+                auto process = [&](int c, float (&v)[32]) {
                     const int c0 = n0 + c * 32;
                     if (g.e.zout != nullptr && row_ok) {
                         // keep the fp32 logits of this row panel for the dS pass (no recompute)
@@ -247,6 +245,19 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                         s = s * resc + acc;
                         m = mn;
                     }
+                };
+                // two register buffers: the TMEM load of chunk c + 1 is in flight while chunk c is
+                // reduced (the exposed load latency was 30 % of the epilogue's stall samples)
+                float vb[32];
+                tmem_ld32_issue(t_addr, v);
+#pragma unroll 1
+                for (int c = 0; c < kTN / 32; c += 2) {
+                    tmem_ld_wait(v);
+                    tmem_ld32_issue(t_addr + (c + 1) * 32, vb);
+                    process(c, v);
+                    tmem_ld_wait(vb);
+                    if (c + 2 < kTN / 32) tmem_ld32_issue(t_addr + (c + 2) * 32, v);
+                    process(c + 1, vb);
                 }
                 if (row_ok) {
                     g.e.part[(int64_t)n_blk * g.e.part_ld + row] = make_float2(m, s);
