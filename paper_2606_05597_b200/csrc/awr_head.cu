@@ -34,7 +34,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                  const __grid_constant__ CUtensorMap tmap_b, const GemmArgs g) {
     using G = Geo<CTAS, NT>;
     constexpr int kTN = G::kTileN;
-    constexpr int kStages = G::kStages;
+    constexpr int kStages = EpiGeo<EPI, CTAS, NT>::kStages;
     constexpr int kStageBytes = G::kStageBytes;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -45,6 +45,8 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
     auto tfull_bar = [&](int s) { return bars + 8u * (2 * kStages + s); };
     auto tempty_bar = [&](int s) { return bars + 8u * (2 * kStages + 2 + s); };
     const uint32_t tmem_slot = bars + 8u * (2 * kStages + 4);
+    // staging tiles of the LSE epilogue (kEpiLse only), behind the 256-byte barrier block
+    float* zstage = reinterpret_cast<float*>(smem_raw + (bars + 256u - smem_u32(smem_raw)));
     uint32_t* tmem_slot_ptr =
         reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
@@ -203,14 +205,27 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 const bool y_here = (y >= n0) && (y < n0 + kTN) && (y < g.N);
                 auto process = [&](int c, float (&v)[32]) {
                     const int c0 = n0 + c * 32;
-                    if (g.e.zout != nullptr && row_ok) {
-                        // keep the fp32 logits of this row panel for the dS pass (no recompute)
-                        float* zp = g.e.zout + (int64_t)row * g.e.zout_ld + c0;
+                    if (g.e.zout != nullptr) {            // warp-uniform
+                        // keep the fp32 logits of this row panel for the dS pass (no recompute):
+                        // thread = row after the TMEM load; transposed through this warp's padded
+                        // shared-memory tile so that every store instruction writes 4 whole
+                        // 128-byte row segments instead of 16 bytes of 32 different rows
+                        float* stg = zstage + q * (32 * kZStageLd);
 #pragma unroll
                         for (int j = 0; j < 8; ++j)
-                            if (c0 + 4 * j < g.N)
-                                *reinterpret_cast<float4*>(zp + 4 * j) =
-                                    make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+                            *reinterpret_cast<float4*>(stg + lane * kZStageLd + 4 * j) =
+                                make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+                        __syncwarp();
+                        const int cc = (lane & 7) * 4;
+                        const int row_w = row - lane;         // tile row of this warp's TMEM lane 0
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            const int r = i * 4 + (lane >> 3);
+                            const float4 t = *reinterpret_cast<const float4*>(stg + r * kZStageLd + cc);
+                            if (row_w + r < g.M && c0 + cc < g.N)
+                                __stcs(reinterpret_cast<float4*>(g.e.zout + (int64_t)(row_w + r) * g.e.zout_ld + c0 + cc), t);
+                        }
+                        __syncwarp();
                     }
                     if (c0 + 32 > g.N) {
 #pragma unroll
@@ -529,7 +544,7 @@ static cudaError_t launch_gemm_epi(const CUtensorMap& ta, const CUtensorMap& tb,
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(head_gemm_kernel<EPI, CTAS, NT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             Geo<CTAS, NT>::kSmemBytes);
+                                             EpiGeo<EPI, CTAS, NT>::kSmemBytes);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -541,7 +556,7 @@ static cudaError_t launch_gemm_epi(const CUtensorMap& ta, const CUtensorMap& tb,
     attr[0].val.clusterDim.z = 1;
     cfg.gridDim = dim3(grid, 1, 1);
     cfg.blockDim = dim3(kThreads, 1, 1);
-    cfg.dynamicSmemBytes = Geo<CTAS, NT>::kSmemBytes;
+    cfg.dynamicSmemBytes = EpiGeo<EPI, CTAS, NT>::kSmemBytes;
     cfg.stream = st;
     cfg.attrs = attr;
     cfg.numAttrs = 1;

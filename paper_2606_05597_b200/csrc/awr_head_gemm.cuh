@@ -64,6 +64,21 @@ struct Geo {
     static constexpr int kAccStages = 2 / NT;            // TMEM accumulator buffers
     static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment */ + 256 /* barriers */;
 };
+// The LSE epilogue (kEpiLse) keeps the fp32 logits tile: a TMEM load hands every thread one ROW,
+// and 16-byte stores to 32 different rows per instruction drain so slowly that the epilogue,
+// not the tensor pipe, set the pace of the forward GEMM (ncu: its warps sat on the registers of
+// outstanding stores).  Each epilogue warp therefore transposes its 32 x 32 chunk through a
+// private padded shared-memory tile and stores whole 128-byte rows; the ring gives up one stage.
+constexpr int kZStageLd = 36;                                   // floats per staged row (144 B)
+constexpr int kZStageBytes = 4 * 32 * kZStageLd * 4;            // 4 epilogue warps: 18,432 B
+template <int EPI, int CTAS, int NT>
+struct EpiGeo {
+    using G = Geo<CTAS, NT>;
+    static constexpr bool kStaged = EPI == 0;                   // kEpiLse
+    static constexpr int kStages = (kStaged && CTAS == 2 && NT == 1) ? G::kStages - 1 : G::kStages;
+    static constexpr int kSmemBytes = kStages * G::kStageBytes + 1024 + 256 + (kStaged ? kZStageBytes : 0);
+};
+static_assert(EpiGeo<0, 2, 1>::kSmemBytes <= 232448 && EpiGeo<0, 1, 1>::kSmemBytes <= 232448, "shared memory");
 static_assert(Geo<2>::kStages <= kMaxStages && Geo<2>::kSmemBytes <= 232448, "shared memory");
 static_assert(Geo<2, 2>::kSmemBytes <= 232448, "shared memory");
 
