@@ -198,8 +198,10 @@ __device__ __forceinline__ uint32_t map_to_cta(uint32_t local_addr, uint32_t ran
     return r;
 }
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr)
-                 : "memory");
+    // default semantics (release at CTA scope), as CUTLASS's ClusterBarrier::arrive(cta_id): what
+    // is handed over is tensor memory, ordered by tcgen05.fence::before_thread_sync; an explicit
+    // .release.cluster costs a MEMBAR.ALL.CTA + ERRBAR per tile per warp
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
