@@ -222,7 +222,12 @@ AWR_API int awr_loss_fwd_bwd_fused_head(const awr_head_batch* batch, const awr_p
 AWR_API size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
                                 int32_t n_traj, int32_t n_groups);
 
-/* Kernel launches one awr_loss_fwd_bwd_fused_head call enqueues for this shape. */
+/* Note: in the stored-logits mode the call forks the dS pass of each row panel onto a library-owned
+ * side stream (created once per device) and joins it back before the panel's dhidden GEMM; from
+ * the caller's point of view all work is still ordered on `stream`, and the call can be captured
+ * into a CUDA graph.  Workspace: two fp32 logits panels.
+ *
+ * Kernel launches one awr_loss_fwd_bwd_fused_head call enqueues for this shape. */
 AWR_API int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K, int32_t kernel);
 
 /* The tensor-core engine of a5 on its own (tests, benchmarks): C[M, N] = A B, bf16 operands,

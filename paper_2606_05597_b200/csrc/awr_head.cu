@@ -8,6 +8,8 @@
 //     pass G2  dhidden[panel] = dS W_head^T                                      (GEMM, kEpiStoreBf16)
 //     pass G3  dw_head += H[panel]^T dS   (fp32 running sum, bf16 at the end)    (GEMM, kEpiAccum)
 // Every GEMM is the tcgen05 kernel below; see awr_head_gemm.cuh for the engine.
+#include <mutex>
+
 #include "awr_head_gemm.cuh"
 #include "awr_kernels.h"
 
@@ -608,6 +610,29 @@ using namespace head;
 
 static inline size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
+struct SideStream {
+    cudaStream_t stream;
+    cudaEvent_t fork, join;
+    bool ok;
+};
+// one per device, created on first use (thread-safe: guarded by a mutex)
+static const SideStream* side_stream() {
+    static SideStream cache[64] = {};
+    static std::mutex mu;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    SideStream& s = cache[dev];
+    if (!s.ok) {
+        if (cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess)
+            return nullptr;
+        s.ok = true;
+    }
+    return &s;
+}
+
 struct HeadWs {
     float *zy, *row_lse, *row_coef, *row_gy;
     float2* part;
@@ -615,6 +640,7 @@ struct HeadWs {
     __nv_bfloat16* ds;
     float* dw_acc;
     float* zpanel;           // stored-logits mode: fp32 [panel_rows, z_ld]
+    float* zpanel2;          // second buffer: the forward of panel p + 1 runs beside the dS pass of p
     int64_t part_ld, ds_ld, z_ld, panel_rows;
     int n_vtiles, n_panels;
     size_t total;
@@ -647,6 +673,7 @@ static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ct
     w.dw_acc = (float*)take(w.n_panels > 1 ? (size_t)K * V * 4 : 0);
     w.z_ld = w.ds_ld;
     w.zpanel = (float*)take(store_z ? (size_t)w.panel_rows * w.z_ld * 4 : 0);
+    w.zpanel2 = (float*)take(store_z && w.n_panels > 1 ? (size_t)w.panel_rows * w.z_ld * 4 : 0);
     w.total = off;
     return w;
 }
@@ -701,20 +728,49 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         if (e != cudaSuccess) return e;
     }
 
+    // Stored mode: the HBM-bound dS pass of panel p runs on a side stream beside the tensor-bound
+    // forward GEMM of panel p + 1 (two logits buffers); both join before the panel's dhidden GEMM.
+    // The side stream and the two fork / join events are created once per device and kept (the
+    // only state the library keeps besides function attributes); the fork / join pattern is legal
+    // inside a CUDA-graph capture of the caller's stream.
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    if (store_z) {
+        const SideStream* ss = side_stream();
+        if (!ss) return cudaErrorUnknown;
+        side = ss->stream; ev_fork = ss->fork; ev_join = ss->join;
+    }
+    float* zbuf[2] = {w.zpanel, w.zpanel2};
+    if (store_z && w.n_panels > 0) {
+        const int64_t rows0 = c.n_tok < w.panel_rows ? c.n_tok : w.panel_rows;
+        e = forward(0, rows0, zbuf[0]);
+        if (e != cudaSuccess) return e;
+    }
+
     // ---- row panels: dS, dhidden, dw_head
     for (int p = 0; p < w.n_panels; ++p) {
         const int64_t r0 = (int64_t)p * w.panel_rows;
         const int64_t rows = (c.n_tok - r0 < w.panel_rows) ? (c.n_tok - r0) : w.panel_rows;
         const __nv_bfloat16* Hp = H + r0 * c.K;
         if (store_z) {
-            // forward of this panel keeps its fp32 logits; dS is then one streaming pass
-            e = forward(r0, rows, w.zpanel);
+            // dS of this panel from its stored fp32 logits: one streaming pass, on the side stream
+            e = cudaEventRecord(ev_fork, st);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(side, ev_fork, 0);
             if (e != cudaSuccess) return e;
             const unsigned blocks = (unsigned)(rows < 4 * (int64_t)num_sms ? rows : 4 * (int64_t)num_sms);
-            head_ds_kernel<<<blocks, 512, 0, st>>>(w.zpanel, w.z_ld, rows, c.V,
-                                                   c.rows->target_ids + r0, w.row_lse + r0,
-                                                   w.row_coef + r0, w.row_gy + r0, w.ds, w.ds_ld);
+            head_ds_kernel<<<blocks, 512, 0, side>>>(zbuf[p & 1], w.z_ld, rows, c.V,
+                                                     c.rows->target_ids + r0, w.row_lse + r0,
+                                                     w.row_coef + r0, w.row_gy + r0, w.ds, w.ds_ld);
             e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaEventRecord(ev_join, side);
+            if (e != cudaSuccess) return e;
+            if (p + 1 < w.n_panels) {       // meanwhile: forward of the next panel into the other buffer
+                const int64_t r1 = r0 + w.panel_rows;
+                const int64_t rows1 = (c.n_tok - r1 < w.panel_rows) ? (c.n_tok - r1) : w.panel_rows;
+                e = forward(r1, rows1, zbuf[(p + 1) & 1]);
+                if (e != cudaSuccess) return e;
+            }
+            e = cudaStreamWaitEvent(st, ev_join, 0);
         } else {
             EpiArgs e1 = {};
             e1.target_ids = c.rows->target_ids + r0; e1.row_lse = w.row_lse + r0;
