@@ -136,7 +136,11 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     if (backward && (reinterpret_cast<uintptr_t>(o->dlogits) & 15)) return AWR_ERR_ALIGN;
     const size_t need = awr_workspace_bytes(b->n_tok, b->V, b->n_steps, b->n_traj, b->n_groups);
     if (!ws_ptr || (reinterpret_cast<uintptr_t>(ws_ptr) & 255) || ws_bytes < need) return AWR_ERR_WORKSPACE;
-    const int kernel = resolve_kernel(p->kernel, b->V, b->ld, b->logits_dtype, o->token_entropy != nullptr);
+    int kernel = resolve_kernel(p->kernel, b->V, b->ld, b->logits_dtype, o->token_entropy != nullptr);
+    // forward only (no row has to stay on chip for a second pass): the one-CTA-per-row kernel
+    // streams faster than the cluster kernels (config 1: 2.56 ms = 4.9 TB/s against 3.05 ms);
+    // with the entropy output its online rescaling of a third accumulator costs more (3.84 ms)
+    if (!backward && p->kernel == AWR_KERNEL_AUTO && !o->token_entropy) kernel = AWR_KERNEL_GENERIC;
     if (kernel < 0) return AWR_ERR_PARAM;
 
     DeviceInfo info;

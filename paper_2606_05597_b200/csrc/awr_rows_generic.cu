@@ -45,14 +45,14 @@ template <> struct Elem<__nv_bfloat16> {
     }
 };
 
-template <typename T>
+template <typename T, bool ENT>
 __global__ void __launch_bounds__(kGenericThreads)
 rows_generic_kernel(RowArgs a) {
     using E = Elem<T>;
     constexpr int EPV = E::kPerVec;
     __shared__ MaxSum s_red[kGenericThreads / 32];
     __shared__ float s_redz[kGenericThreads / 32];
-    const bool want_ent = a.token_entropy != nullptr;
+    constexpr bool want_ent = ENT;        // token_entropy output: its own instantiation
     __shared__ float s_coef, s_lse, s_gy;
     __shared__ int s_y;
     const int tid = threadIdx.x;
@@ -89,7 +89,7 @@ rows_generic_kernel(RowArgs a) {
             if (cm > ms.m) {
                 const float sc = ex2_approx((ms.m - cm) * kLog2e);
                 ms.s *= sc;
-                sz *= sc;
+                if (want_ent) sz *= sc;
                 ms.m = cm;
             }
             float ml = (ms.m == -INFINITY) ? 0.f : ms.m * kLog2e;   // all -inf so far: no NaN
@@ -112,16 +112,16 @@ rows_generic_kernel(RowArgs a) {
             if (x > ms.m) {
                 const float sc = ex2_approx((ms.m - x) * kLog2e);
                 ms.s *= sc;
-                sz *= sc;
+                if (want_ent) sz *= sc;
                 ms.m = x;
             }
             if (ms.m != -INFINITY) {
                 const float e = ex2_approx((x - ms.m) * kLog2e);
                 ms.s += e;
-                sz = fmaf(e, fmaxf(x, kZFloor), sz);
+                if (want_ent) sz = fmaf(e, fmaxf(x, kZFloor), sz);
             }
         }
-        {
+        if (want_ent) {
             // bring this thread's sz to the warp's max before the (max, sum) state is merged
             float wm = ms.m;
 #pragma unroll
@@ -194,10 +194,13 @@ cudaError_t launch_rows_generic(const RowArgs& a, int dtype, int num_sms, cudaSt
     int64_t blocks = a.n_tok;
     int64_t cap = (int64_t)num_sms * 8;
     if (blocks > cap) blocks = cap;
+    const bool ent = a.token_entropy != nullptr;
     if (dtype == AWR_DTYPE_BF16) {
-        rows_generic_kernel<__nv_bfloat16><<<(int)blocks, kGenericThreads, 0, st>>>(a);
+        if (ent) rows_generic_kernel<__nv_bfloat16, true><<<(int)blocks, kGenericThreads, 0, st>>>(a);
+        else rows_generic_kernel<__nv_bfloat16, false><<<(int)blocks, kGenericThreads, 0, st>>>(a);
     } else {
-        rows_generic_kernel<float><<<(int)blocks, kGenericThreads, 0, st>>>(a);
+        if (ent) rows_generic_kernel<float, true><<<(int)blocks, kGenericThreads, 0, st>>>(a);
+        else rows_generic_kernel<float, false><<<(int)blocks, kGenericThreads, 0, st>>>(a);
     }
     return cudaGetLastError();
 }
