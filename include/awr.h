@@ -22,8 +22,16 @@
  *     caller; inputs are read-only; outputs are overwritten (never accumulated into).
  *     Only awr_loss_fwd_bwd_host takes HOST pointers (stated there).
  *   - Calls only enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the legacy
- *     default stream).  No allocation, no host synchronisation, no hidden state; outputs are
- *     valid once the stream has been synchronised.  Graph-capturable.
+ *     default stream).  No allocation, no host synchronisation; outputs are valid once the
+ *     stream has been synchronised.  Graph-capturable.
+ *   - Thread safety / state: entry points may be called concurrently from several host threads
+ *     as long as concurrent calls use different `stream`s, different workspaces and different
+ *     outputs.  The library keeps no per-call state.  What it keeps per DEVICE: cached device
+ *     attributes, function attributes, and (fused head, stored-logits mode only) a pool of up to
+ *     8 side streams, each with one fork / join event pair, keyed by the caller's stream - calls
+ *     on different streams never share one; when all 8 are busy the call runs without the
+ *     overlap.  Two calls racing on the SAME stream are ordered by whichever enqueues first, as
+ *     with any CUDA work.
  *   - Return value: AWR_OK or a negative awr_status.  Host-side checks cover scalars, null
  *     pointers, alignment and workspace size only.  Data-dependent faults set bits in
  *     *err_word (AWR_ERRBIT_*) and the affected token contributes nothing.
@@ -46,7 +54,7 @@
 extern "C" {
 #endif
 
-#define AWR_VERSION 100
+#define AWR_VERSION 200
 
 #if defined(__GNUC__)
 #define AWR_API __attribute__((visibility("default")))
@@ -76,7 +84,7 @@ enum { AWR_FLAG_SAMPLE_STD = 1u,     /* A2: std with 1/(G-1) instead of the defa
                                         groups runs over the mixed groups only (one extra launch) */
        AWR_FLAG_COUPLED = 4u         /* coupled-ratio ablation (:114): one pi_theta/pi_behave ratio
                                         with the clip centred on it, no staleness weight; prox_lp
-                                        is not read */ };
+                                        is not read and may be NULL */ };
 enum { AWR_W_K_BY_V = 0 /* w_head[k * V + v] */, AWR_W_V_BY_K = 1 /* w_head[v * K + k] */ };
 enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_GENERIC = 1,  /* one CTA per row, second pass re-reads the row through L2 */
@@ -131,7 +139,9 @@ typedef struct awr_params {
 } awr_params;
 
 typedef struct awr_outputs {
-    float* loss;            /* [1]  -J, f32 (summed in fp64 in token order, then rounded) */
+    float* loss;            /* [1]  -J, f32: the per-token terms summed in fp64 in a FIXED order
+                               (thread-strided partial sums of 1024 threads, then a binary tree)
+                               and rounded once - bit-reproducible, not token order */
     void* dlogits;          /* [n_tok, ld] same dtype/stride as logits; NULL in awr_loss_fwd */
     float* token_lp;        /* [n_tok] l_t = log pi_theta(y_t); 0 for masked tokens */
     int64_t* clip_count;    /* [1] number of tokens with trig_t */
@@ -147,6 +157,12 @@ typedef struct awr_outputs {
                                per-token entropy diagnostic (:232, :341), from the same streaming
                                pass; 0 for masked tokens.  Generic and register-file kernels (an
                                explicit AWR_KERNEL_CLUSTER with it -> AWR_ERR_PARAM) */
+    /* optional measurement aid (both or neither; NULL = off): two cudaEvent_t created by the
+     * caller with timing enabled; THIS call records them on `stream` immediately before / after
+     * its row kernel (a2 + a3 + a4), so bench.py can report that kernel's own duration from
+     * inside the timed region.  Per call, no library state (ignored by the host-buffer entry). */
+    void* ev_row_begin;
+    void* ev_row_end;
 } awr_outputs;
 
 /* a0..a4 fused: segment expansion, group advantage (:61), online log-sum-exp + target gather,
@@ -155,7 +171,10 @@ AWR_API int awr_loss_fwd_bwd(const awr_batch* batch, const awr_params* params, c
                      void* workspace, size_t workspace_bytes, void* stream);
 
 /* Forward only: loss, token_lp, clip_count (and the optional per-token outputs); out->dlogits
- * is ignored.  Reads each row once, writes no gradient. */
+ * is ignored.  Reads each row once, writes no gradient.  This is the proximal log-prob
+ * recomputation the trainer runs at the start of every update ("proximal logprobs
+ * recomputed"; token_lp of this call is the prox_lp of the update's loss calls) and the source of
+ * the per-token entropy diagnostic (:232, :341). */
 AWR_API int awr_loss_fwd(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
                  void* workspace, size_t workspace_bytes, void* stream);
 
@@ -249,12 +268,6 @@ AWR_API int awr_version(void);
  * awr_loss_fwd_bwd call enqueues. */
 AWR_API int awr_select_kernel(int64_t V, int64_t ld, int32_t logits_dtype);
 AWR_API int awr_launches_per_call(void);
-
-/* Measurement hook (bench.py "roofline"): the NEXT awr_loss_fwd_bwd / awr_loss_fwd call made by
- * any thread records `ev_before` / `ev_after` (two cudaEvent_t created by the caller with timing
- * enabled) on its stream immediately around the row kernel (a2 + a3 + a4), then forgets them.
- * Pass NULL, NULL to cancel.  Not thread-safe by design: a profiling aid, not part of the path. */
-AWR_API int awr_profile_next_row_kernel(void* ev_before, void* ev_after);
 
 #ifdef __cplusplus
 }

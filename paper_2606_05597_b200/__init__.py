@@ -8,4 +8,4 @@ from ._abi import (AwrError, DTYPE_BF16, DTYPE_F32, ERRBIT_GROUP_OFF, ERRBIT_STE
 from .api import (HEAD_OPTIONAL_OUTPUTS, HeadLossCall, HostLossCall, LossCall, awr_gemm_bf16,
                   awr_loss_fwd_bwd_fused_head, head_launches_per_call, head_workspace_bytes, OPTIONAL_OUTPUTS, awr_group_advantage, awr_loss_fwd,
                   awr_loss_fwd_bwd, awr_loss_fwd_bwd_host, host_workspace_bytes,
-                  launches_per_call, make_params, profile_next_row_kernel, select_kernel, workspace_bytes)
+                  launches_per_call, make_params, select_kernel, workspace_bytes)

@@ -48,7 +48,7 @@ class awr_outputs(C.Structure):
     _fields_ = [("loss", _vp), ("dlogits", _vp), ("token_lp", _vp), ("clip_count", _vp),
                 ("adv", _vp), ("tok_traj", _vp), ("target_logit", _vp), ("tok_term", _vp),
                 ("tok_coef", _vp), ("err_word", _vp), ("dual_clip_count", _vp),
-                ("token_entropy", _vp)]
+                ("token_entropy", _vp), ("ev_row_begin", _vp), ("ev_row_end", _vp)]
 
 
 class awr_head_batch(C.Structure):
@@ -90,7 +90,6 @@ SYMBOLS = {
     "awr_version": (C.c_int, []),
     "awr_select_kernel": (C.c_int, [C.c_int64, C.c_int64, C.c_int32]),
     "awr_launches_per_call": (C.c_int, []),
-    "awr_profile_next_row_kernel": (C.c_int, [_vp, _vp]),
 }
 
 _lock = threading.Lock()

@@ -82,13 +82,14 @@ def _batch_struct(logits, target_ids, behave_lp, prox_lp, step_off, traj_off, gr
         raise TypeError("logits must live on the GPU (there is no CPU path)")
     _req(target_ids, torch.int32, "target_ids", cuda)
     _req(behave_lp, torch.float32, "behave_lp", cuda)
-    _req(prox_lp, torch.float32, "prox_lp", cuda)
+    if prox_lp is not None:              # may be None with FLAG_COUPLED (not read)
+        _req(prox_lp, torch.float32, "prox_lp", cuda)
     _req(step_off, torch.int32, "step_off", cuda)
     _req(traj_off, torch.int32, "traj_off", cuda)
     _req(group_off, torch.int32, "group_off", cuda)
     _req(rewards, torch.float32, "rewards", cuda)
     for t, name in ((target_ids, "target_ids"), (behave_lp, "behave_lp"), (prox_lp, "prox_lp")):
-        if t.numel() != n_tok:
+        if t is not None and t.numel() != n_tok:
             raise ValueError("%s must have n_tok = %d entries" % (name, n_tok))
     if traj_off.numel() != rewards.numel() + 1:
         raise ValueError("traj_off must have n_traj + 1 entries")
@@ -104,7 +105,8 @@ def _out_struct(o):
     return awr_outputs(_ptr(g("loss")), _ptr(g("dlogits")), _ptr(g("token_lp")),
                        _ptr(g("clip_count")), _ptr(g("adv")), _ptr(g("tok_traj")),
                        _ptr(g("target_logit")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
-                       _ptr(g("err_word")), _ptr(g("dual_clip_count")), _ptr(g("token_entropy")))
+                       _ptr(g("err_word")), _ptr(g("dual_clip_count")), _ptr(g("token_entropy")),
+                       None, None)
 
 
 class LossCall:
@@ -143,9 +145,20 @@ class LossCall:
         self._fn = self.lib.awr_loss_fwd_bwd if backward else self.lib.awr_loss_fwd
         self._name = "awr_loss_fwd_bwd" if backward else "awr_loss_fwd"
 
-    def run(self, stream=None):
-        rc = self._fn(C.byref(self.batch), C.byref(self.params), C.byref(self.outs),
-                      _ptr(self.workspace), self.ws_bytes, _stream_ptr(stream, self.device))
+    def run(self, stream=None, row_events=None):
+        """``row_events``: optional pair of ``torch.cuda.Event(enable_timing=True)`` that have been
+        recorded once (so that their handles exist); this call records them on its stream right
+        around the row kernel (``awr_outputs.ev_row_begin / ev_row_end``)."""
+        if row_events is not None:
+            self.outs.ev_row_begin = row_events[0].cuda_event
+            self.outs.ev_row_end = row_events[1].cuda_event
+        try:
+            rc = self._fn(C.byref(self.batch), C.byref(self.params), C.byref(self.outs),
+                          _ptr(self.workspace), self.ws_bytes, _stream_ptr(stream, self.device))
+        finally:
+            if row_events is not None:
+                self.outs.ev_row_begin = None
+                self.outs.ev_row_end = None
         check(rc, self._name)
         return self.out
 
@@ -184,14 +197,6 @@ def select_kernel(V, ld, dtype) -> int:
 
 def launches_per_call() -> int:
     return int(load().awr_launches_per_call())
-
-
-def profile_next_row_kernel(ev_before, ev_after) -> None:
-    """include/awr.h awr_profile_next_row_kernel; takes two torch.cuda.Event(enable_timing=True)
-    that have been recorded once (so that their handles exist), or (None, None)."""
-    a = None if ev_before is None else C.c_void_p(ev_before.cuda_event)
-    b = None if ev_after is None else C.c_void_p(ev_after.cuda_event)
-    check(load().awr_profile_next_row_kernel(a, b), "awr_profile_next_row_kernel")
 
 
 # ------------------------------------------------------------------ host-buffer entry point

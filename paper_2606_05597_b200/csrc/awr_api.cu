@@ -115,8 +115,6 @@ static cudaError_t launch_rows(int kernel, const RowArgs& a, int dtype, int num_
     return launch_rows_generic(a, dtype, num_sms, st);
 }
 
-static cudaEvent_t g_prof_before = nullptr, g_prof_after = nullptr;
-
 static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, void* ws_ptr,
                size_t ws_bytes, void* stream, bool backward) {
     if (!b || !p || !o) return AWR_ERR_NULL;
@@ -129,8 +127,11 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     if (!o->loss || !o->clip_count) return AWR_ERR_NULL;
     if (b->n_tok > 0 && (!o->token_lp || (backward && !o->dlogits))) return AWR_ERR_NULL;
     if (!b->step_off || !b->traj_off || !b->group_off) return AWR_ERR_NULL;
-    if (b->n_tok > 0 && (!b->logits || !b->target_ids || !b->behave_lp || !b->prox_lp)) return AWR_ERR_NULL;
+    const bool coupled = (p->flags & AWR_FLAG_COUPLED) != 0;      // prox_lp is not read (:114)
+    if (b->n_tok > 0 && (!b->logits || !b->target_ids || !b->behave_lp || (!coupled && !b->prox_lp)))
+        return AWR_ERR_NULL;
     if (b->n_traj > 0 && !b->rewards) return AWR_ERR_NULL;
+    if ((o->ev_row_begin == nullptr) != (o->ev_row_end == nullptr)) return AWR_ERR_NULL;
     const size_t esz = b->logits_dtype == AWR_DTYPE_BF16 ? 2 : 4;
     if ((reinterpret_cast<uintptr_t>(b->logits) & 15) || ((size_t)b->ld * esz) % 16) return AWR_ERR_ALIGN;
     if (backward && (reinterpret_cast<uintptr_t>(o->dlogits) & 15)) return AWR_ERR_ALIGN;
@@ -160,7 +161,7 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     // a0
     if (e == cudaSuccess)
         e = launch_segment_expand(b->step_off, b->traj_off, b->group_off, b->n_tok, b->n_steps,
-                                  b->n_traj, b->n_groups, tok_traj, err, st);
+                                  b->n_traj, b->n_groups, tok_traj, err, info.num_sms, st);
     // a1 (+ O6 scale)
     if (e == cudaSuccess)
         e = launch_group_advantage(b->rewards, b->group_off, b->traj_off, b->n_groups, b->n_traj,
@@ -178,8 +179,9 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     a.target_logit = o->target_logit; a.tok_flag = w.tok_flag; a.err_word = err;
     a.token_entropy = o->token_entropy;
     a.clip_eps = p->clip_eps; a.stale_cap = p->stale_cap; a.dual_c = p->dual_clip_c;
-    cudaEvent_t ev0 = g_prof_before, ev1 = g_prof_after;
-    g_prof_before = g_prof_after = nullptr;
+    // optional measurement events of THIS call (no library state): around the row kernel only
+    cudaEvent_t ev0 = reinterpret_cast<cudaEvent_t>(o->ev_row_begin);
+    cudaEvent_t ev1 = reinterpret_cast<cudaEvent_t>(o->ev_row_end);
     if (e == cudaSuccess && ev0) e = cudaEventRecord(ev0, st);
     if (e == cudaSuccess) {
         e = launch_rows(kernel, a, b->logits_dtype, info.num_sms, st);
@@ -227,13 +229,6 @@ int awr_select_kernel(int64_t V, int64_t ld, int32_t logits_dtype) {
 }
 
 int awr_launches_per_call(void) { return 4; }
-
-int awr_profile_next_row_kernel(void* ev_before, void* ev_after) {
-    if ((ev_before == nullptr) != (ev_after == nullptr)) return AWR_ERR_NULL;
-    g_prof_before = reinterpret_cast<cudaEvent_t>(ev_before);
-    g_prof_after = reinterpret_cast<cudaEvent_t>(ev_after);
-    return AWR_OK;
-}
 
 int awr_loss_fwd_bwd(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
                      void* workspace, size_t workspace_bytes, void* stream) {
@@ -292,7 +287,8 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     if (!o->loss || !o->clip_count || !o->dw_head) return AWR_ERR_NULL;
     if (b->n_tok > 0 && (!o->token_lp || !o->dhidden)) return AWR_ERR_NULL;
     if (!b->step_off || !b->traj_off || !b->group_off || !b->w_head) return AWR_ERR_NULL;
-    if (b->n_tok > 0 && (!b->hidden || !b->target_ids || !b->behave_lp || !b->prox_lp)) return AWR_ERR_NULL;
+    if (b->n_tok > 0 && (!b->hidden || !b->target_ids || !b->behave_lp ||
+                         (!(p->flags & AWR_FLAG_COUPLED) && !b->prox_lp))) return AWR_ERR_NULL;
     if (b->n_traj > 0 && !b->rewards) return AWR_ERR_NULL;
     if ((reinterpret_cast<uintptr_t>(b->hidden) & 15) || (reinterpret_cast<uintptr_t>(b->w_head) & 15) ||
         (reinterpret_cast<uintptr_t>(o->dhidden) & 15) || (reinterpret_cast<uintptr_t>(o->dw_head) & 15))
@@ -315,7 +311,7 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     if (e == cudaSuccess && o->adv && b->n_traj > 0) e = cudaMemsetAsync(o->adv, 0, (size_t)b->n_traj * 4, st);
     if (e == cudaSuccess)
         e = launch_segment_expand(b->step_off, b->traj_off, b->group_off, b->n_tok, b->n_steps,
-                                  b->n_traj, b->n_groups, tok_traj, err, st);
+                                  b->n_traj, b->n_groups, tok_traj, err, info.num_sms, st);
     if (e == cudaSuccess)
         e = launch_group_advantage(b->rewards, b->group_off, b->traj_off, b->n_groups, b->n_traj,
                                    p->flags, p->normalizer, p->k_norm, p->loss_scale, adv,
@@ -380,9 +376,8 @@ HostPlan host_plan(int64_t n_tok, int64_t V, int64_t ld, int32_t dtype, int32_t 
     HostPlan h;
     const size_t esz = dtype == AWR_DTYPE_BF16 ? 2 : 4;
     const size_t row_bytes = (size_t)ld * esz;
-    int64_t rows = (int64_t)((256u << 20) / (row_bytes ? row_bytes : 1));
-    rows = rows / 74 * 74;                         // whole waves of the 74-cluster schedule
-    if (rows < 74) rows = 74;
+    int64_t rows = (int64_t)((256u << 20) / (row_bytes ? row_bytes : 1));     // 256 MB panels
+    if (rows < 64) rows = 64;
     if (rows > n_tok) rows = n_tok > 0 ? n_tok : 1;
     h.panel_rows = rows;
     h.panel_bytes = align_up((size_t)rows * row_bytes, 256);
@@ -419,7 +414,9 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
     if (!ho->loss || !ho->clip_count) return AWR_ERR_NULL;
     if (hb->n_tok > 0 && (!ho->token_lp || !ho->dlogits)) return AWR_ERR_NULL;
     if (!hb->step_off || !hb->traj_off || !hb->group_off) return AWR_ERR_NULL;
-    if (hb->n_tok > 0 && (!hb->logits || !hb->target_ids || !hb->behave_lp || !hb->prox_lp)) return AWR_ERR_NULL;
+    const bool coupled = (p->flags & AWR_FLAG_COUPLED) != 0;      // prox_lp is neither read nor copied
+    if (hb->n_tok > 0 && (!hb->logits || !hb->target_ids || !hb->behave_lp || (!coupled && !hb->prox_lp)))
+        return AWR_ERR_NULL;
     if (hb->n_traj > 0 && !hb->rewards) return AWR_ERR_NULL;
     const size_t esz = hb->logits_dtype == AWR_DTYPE_BF16 ? 2 : 4;
     if (((size_t)hb->ld * esz) % 16) return AWR_ERR_ALIGN;
@@ -481,7 +478,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
     if (n > 0) {
         AWR_TRY(cudaMemcpyAsync(d_ids, hb->target_ids, (size_t)n * 4, H2D, s_k));
         AWR_TRY(cudaMemcpyAsync(d_b, hb->behave_lp, (size_t)n * 4, H2D, s_k));
-        AWR_TRY(cudaMemcpyAsync(d_q, hb->prox_lp, (size_t)n * 4, H2D, s_k));
+        if (!coupled) AWR_TRY(cudaMemcpyAsync(d_q, hb->prox_lp, (size_t)n * 4, H2D, s_k));
     }
     AWR_TRY(cudaMemcpyAsync(d_so, hb->step_off, (size_t)(hb->n_steps + 1) * 4, H2D, s_k));
     AWR_TRY(cudaMemcpyAsync(d_to, hb->traj_off, (size_t)(hb->n_traj + 1) * 4, H2D, s_k));
@@ -491,7 +488,8 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
     AWR_TRY(cudaMemsetAsync(d_ws, 0, w.zero_bytes, s_k));
     AWR_TRY(cudaMemsetAsync(d_scal, 0, 256, s_k));
     if (hb->n_traj > 0) AWR_TRY(cudaMemsetAsync(d_adv, 0, (size_t)hb->n_traj * 4, s_k));
-    AWR_TRY(launch_segment_expand(d_so, d_to, d_go, n, hb->n_steps, hb->n_traj, hb->n_groups, d_tt, d_err, s_k));
+    AWR_TRY(launch_segment_expand(d_so, d_to, d_go, n, hb->n_steps, hb->n_traj, hb->n_groups, d_tt, d_err,
+                                  info.num_sms, s_k));
     AWR_TRY(launch_group_advantage(d_rw, d_go, d_to, hb->n_groups, hb->n_traj, p->flags, p->normalizer,
                                    p->k_norm, p->loss_scale, d_adv, w.traj_scale, w.err + 1, s_k));
     // row panels: H2D -> kernel (in place) -> D2H, three buffers in flight
@@ -510,7 +508,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
         a.logits = buf; a.dlogits = buf;                 // in place on the panel
         a.n_tok = rows; a.V = hb->V; a.ld = hb->ld;
         a.target_ids = d_ids + r0; a.behave_lp = d_b + r0;
-        a.prox_lp = ((p->flags & AWR_FLAG_COUPLED) ? d_b : d_q) + r0;
+        a.prox_lp = (coupled ? d_b : d_q) + r0;
         a.tok_traj = d_tt + r0; a.adv = d_adv; a.traj_scale = w.traj_scale;
         a.token_lp = d_lp + r0; a.tok_term = d_term + r0; a.tok_coef = d_coef + r0;
         a.target_logit = d_tl + r0; a.tok_flag = w.tok_flag + r0; a.err_word = d_err;

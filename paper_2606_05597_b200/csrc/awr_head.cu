@@ -68,7 +68,7 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4 * CTAS); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_mbar_init();
     }
     if (warp == 2) {
         if constexpr (CTAS == 1) {
@@ -542,13 +542,14 @@ static bool make_operand(const OperandView& v, int tile_mn, CUtensorMap* map, Op
 template <int EPI, int CTAS, int NT>
 static cudaError_t launch_gemm_epi(const CUtensorMap& ta, const CUtensorMap& tb, const GemmArgs& g,
                                    int grid, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceInt attr_set;                    // the attribute is per device
+    const int dev = PerDeviceInt::device();
+    if (attr_set.get(dev) < 0) {
         cudaError_t e = cudaFuncSetAttribute(head_gemm_kernel<EPI, CTAS, NT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              EpiGeo<EPI, CTAS, NT>::kSmemBytes);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_set.set(dev, 1);
     }
     cudaLaunchConfig_t cfg = {};
     cudaLaunchAttribute attr[1];
@@ -610,28 +611,77 @@ using namespace head;
 
 static inline size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
+// Stored-logits mode: the dS pass of a row panel runs on a library-owned side stream beside the
+// forward GEMM of the next panel.  Side streams (each with its fork / join event pair) live in a
+// small per-device pool KEYED BY THE CALLER'S STREAM: calls on different user streams - from
+// different host threads, or one of them inside a CUDA-graph capture - never share a side stream
+// or an event, so one call's fork record cannot be overtaken by another's.  An entry is pinned
+// (refcount) while a call is enqueuing with it; an unpinned entry whose side stream is not part
+// of an ongoing capture may be handed to another user stream (least recently used first).  If
+// every entry is busy the call runs its dS pass on the caller's stream (no overlap, same result).
 struct SideStream {
+    cudaStream_t user;
     cudaStream_t stream;
     cudaEvent_t fork, join;
     bool ok;
+    int pinned;
+    uint64_t last_use;
 };
-// one per device, created on first use (thread-safe: guarded by a mutex)
-static const SideStream* side_stream() {
-    static SideStream cache[64] = {};
-    static std::mutex mu;
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
-    std::lock_guard<std::mutex> lock(mu);
-    SideStream& s = cache[dev];
-    if (!s.ok) {
+constexpr int kSidePerDevice = 8;
+struct SidePool {
+    std::mutex mu;
+    SideStream e[kMaxDevices][kSidePerDevice] = {};
+    uint64_t tick = 0;
+};
+static SidePool& side_pool() {
+    static SidePool pool;
+    return pool;
+}
+static SideStream* side_acquire(cudaStream_t user) {
+    const int dev = PerDeviceInt::device();
+    if (dev < 0) return nullptr;
+    SidePool& pool = side_pool();
+    std::lock_guard<std::mutex> lock(pool.mu);
+    SideStream* row = pool.e[dev];
+    SideStream* pick = nullptr;
+    for (int i = 0; i < kSidePerDevice && !pick; ++i)
+        if (row[i].ok && row[i].user == user) pick = &row[i];
+    for (int i = 0; i < kSidePerDevice && !pick; ++i) {
+        if (row[i].ok) continue;
+        SideStream& s = row[i];
         if (cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess)
+            cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
             return nullptr;
-        s.ok = true;
+        }
+        s.ok = true; s.pinned = 0;
+        pick = &s;
     }
-    return &s;
+    if (!pick) {                         // re-key the least recently used idle entry
+        for (int i = 0; i < kSidePerDevice; ++i) {
+            SideStream& s = row[i];
+            if (s.pinned > 0 || (pick && s.last_use >= pick->last_use)) continue;
+            cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+            if (cudaStreamIsCapturing(s.stream, &cs) != cudaSuccess) { cudaGetLastError(); continue; }
+            if (cs == cudaStreamCaptureStatusNone) pick = &s;
+        }
+    }
+    if (!pick) return nullptr;
+    pick->user = user;
+    pick->pinned += 1;
+    pick->last_use = ++pool.tick;
+    return pick;
 }
+static void side_release(SideStream* s) {
+    if (!s) return;
+    std::lock_guard<std::mutex> lock(side_pool().mu);
+    s->pinned -= 1;
+}
+struct SideGuard {
+    SideStream* s;
+    ~SideGuard() { side_release(s); }
+};
 
 struct HeadWs {
     float *zy, *row_lse, *row_coef, *row_gy;
@@ -730,16 +780,14 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
 
     // Stored mode: the HBM-bound dS pass of panel p runs on a side stream beside the tensor-bound
     // forward GEMM of panel p + 1 (two logits buffers); both join before the panel's dhidden GEMM.
-    // The side stream and the two fork / join events are created once per device and kept (the
-    // only state the library keeps besides function attributes); the fork / join pattern is legal
-    // inside a CUDA-graph capture of the caller's stream.
+    // The side stream and its fork / join events come from the per-device pool keyed by the
+    // caller's stream (side_acquire above: the only state the library keeps besides per-device
+    // function attributes); the fork / join pattern is legal inside a CUDA-graph capture of the
+    // caller's stream.
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-    if (store_z) {
-        const SideStream* ss = side_stream();
-        if (!ss) return cudaErrorUnknown;
-        side = ss->stream; ev_fork = ss->fork; ev_join = ss->join;
-    }
+    SideGuard guard{store_z ? side_acquire(st) : nullptr};
+    if (guard.s) { side = guard.s->stream; ev_fork = guard.s->fork; ev_join = guard.s->join; }
     float* zbuf[2] = {w.zpanel, w.zpanel2};
     if (store_z && w.n_panels > 0) {
         const int64_t rows0 = c.n_tok < w.panel_rows ? c.n_tok : w.panel_rows;
@@ -754,15 +802,18 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         const __nv_bfloat16* Hp = H + r0 * c.K;
         if (store_z) {
             // dS of this panel from its stored fp32 logits: one streaming pass, on the side stream
-            e = cudaEventRecord(ev_fork, st);
-            if (e == cudaSuccess) e = cudaStreamWaitEvent(side, ev_fork, 0);
-            if (e != cudaSuccess) return e;
+            cudaStream_t ds_stream = side ? side : st;      // no idle side stream: in line
+            if (side) {
+                e = cudaEventRecord(ev_fork, st);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(side, ev_fork, 0);
+                if (e != cudaSuccess) return e;
+            }
             const unsigned blocks = (unsigned)(rows < 4 * (int64_t)num_sms ? rows : 4 * (int64_t)num_sms);
-            head_ds_kernel<<<blocks, 512, 0, side>>>(zbuf[p & 1], w.z_ld, rows, c.V,
-                                                     c.rows->target_ids + r0, w.row_lse + r0,
-                                                     w.row_coef + r0, w.row_gy + r0, w.ds, w.ds_ld);
+            head_ds_kernel<<<blocks, 512, 0, ds_stream>>>(zbuf[p & 1], w.z_ld, rows, c.V,
+                                                          c.rows->target_ids + r0, w.row_lse + r0,
+                                                          w.row_coef + r0, w.row_gy + r0, w.ds, w.ds_ld);
             e = cudaGetLastError();
-            if (e == cudaSuccess) e = cudaEventRecord(ev_join, side);
+            if (e == cudaSuccess && side) e = cudaEventRecord(ev_join, side);
             if (e != cudaSuccess) return e;
             if (p + 1 < w.n_panels) {       // meanwhile: forward of the next panel into the other buffer
                 const int64_t r1 = r0 + w.panel_rows;
@@ -770,7 +821,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
                 e = forward(r1, rows1, zbuf[(p + 1) & 1]);
                 if (e != cudaSuccess) return e;
             }
-            e = cudaStreamWaitEvent(st, ev_join, 0);
+            if (side) e = cudaStreamWaitEvent(st, ev_join, 0);
         } else {
             EpiArgs e1 = {};
             e1.target_ids = c.rows->target_ids + r0; e1.row_lse = w.row_lse + r0;

@@ -3,14 +3,32 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 namespace awr {
 
 struct RowArgs;
 
+// One cached int per device ordinal (-1 = not set yet).  Function attributes
+// (cudaFuncAttributeMaxDynamicSharedMemorySize) and occupancy answers belong to a DEVICE, not to
+// the process: a process that drives several GPUs must set / query them on each.  Devices with an
+// ordinal >= kMaxDevices are not cached (the setup simply runs on every call).
+constexpr int kMaxDevices = 64;
+struct PerDeviceInt {
+    std::atomic<int> v[kMaxDevices];
+    PerDeviceInt() { for (auto& x : v) x.store(-1, std::memory_order_relaxed); }
+    static int device() {
+        int d = 0;
+        return (cudaGetDevice(&d) == cudaSuccess && d >= 0 && d < kMaxDevices) ? d : -1;
+    }
+    int get(int dev) const { return dev < 0 ? -1 : v[dev].load(std::memory_order_acquire); }
+    void set(int dev, int x) { if (dev >= 0) v[dev].store(x, std::memory_order_release); }
+};
+
 cudaError_t launch_segment_expand(const int32_t* step_off, const int32_t* traj_off,
                                   const int32_t* group_off, int64_t n_tok, int n_steps,
                                   int n_traj, int n_groups, int32_t* tok_traj, uint32_t* err,
-                                  cudaStream_t st);
+                                  int num_sms, cudaStream_t st);
 cudaError_t launch_group_advantage(const float* rewards, const int32_t* group_off,
                                    const int32_t* traj_off, int n_groups, int n_traj,
                                    uint32_t flags, int normalizer, float k_norm,

@@ -18,6 +18,7 @@
 //     and are written from a shared zero page.
 #include "awr_common.cuh"
 #include "awr_kernels.h"
+#include "awr_ptx.cuh"
 
 namespace awr {
 
@@ -44,88 +45,7 @@ struct Ctrl {
 };
 static_assert(sizeof(Ctrl) <= kCtrlBytes, "control block");
 
-// ---------------------------------------------------------------- PTX wrappers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes,
-                                          uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_store(void* dst, uint32_t src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst),
-                 "r"(src), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_commit() {
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-}
-template <int N> __device__ __forceinline__ void bulk_wait_read() {
-    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
-}
-__device__ __forceinline__ void bulk_wait_all() {
-    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
-__device__ __forceinline__ void cluster_arrive() {
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void cluster_wait() {
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-    uint32_t r;
-    asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ uint32_t cluster_id_x() {
-    uint32_t r;
-    asm("mov.u32 %0, %%clusterid.x;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void st_cluster_f32x2(uint32_t local_addr, uint32_t rank, float a,
-                                                 float b) {
-    uint32_t remote;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(rank));
-    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(remote), "f"(a), "f"(b)
-                 : "memory");
-}
-__device__ __forceinline__ uint4 lds128(uint32_t addr) {
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                 : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
-    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y),
-                 "r"(v.z), "r"(v.w)
-                 : "memory");
-}
+using namespace ptx;
 
 // ---------------------------------------------------------------- the kernel
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kCThreads, 1)
@@ -163,7 +83,7 @@ rows_cluster_kernel(RowArgs a, ClusterPlan p) {
         reinterpret_cast<uint32_t*>(smem + kCtrlBytes)[i] = 0u;
     if (lane == 0)
         for (int s = 0; s < S; ++s) mbar_init(bar0 + 8u * s, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_mbar_init();
     fence_proxy_async();      // zero page (generic writes) -> later TMA store reads
     __syncthreads();
     cluster_arrive();
@@ -431,7 +351,7 @@ bool rows_cluster_supported(int64_t V, int64_t ld, int dtype) {
     if (V % 8 != 0 || ld % 8 != 0) return false;
     if (V / 8 > (1 << 24)) return false;
     ClusterPlan p;
-    return make_plan(V, 148, 1 << 20, p);
+    return make_plan(V, 2, 1, p);      // feasibility only: the SM count sets the grid, not the plan
 }
 
 cudaError_t launch_rows_cluster(const RowArgs& a, int num_sms, cudaStream_t st) {
@@ -439,13 +359,14 @@ cudaError_t launch_rows_cluster(const RowArgs& a, int num_sms, cudaStream_t st) 
     ClusterPlan p;
     if (!make_plan(a.V, num_sms, a.n_tok, p)) return cudaErrorInvalidValue;
     const int smem = kCtrlBytes + p.chunk_units * 16 + kCWarps * p.slots * p.chunk_units * 16;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceInt attr_set;                    // the attribute is per device
+    const int dev = PerDeviceInt::device();
+    if (attr_set.get(dev) < 0) {
         cudaError_t e = cudaFuncSetAttribute(rows_cluster_kernel,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              kSmemLimit);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_set.set(dev, 1);
     }
     rows_cluster_kernel<<<2 * p.num_clusters, kCThreads, smem, st>>>(a, p);
     return cudaGetLastError();

@@ -22,6 +22,7 @@
 //     pass 2 and are written as zeros.
 #include "awr_common.cuh"
 #include "awr_kernels.h"
+#include "awr_ptx.cuh"
 
 namespace awr {
 
@@ -66,87 +67,6 @@ struct RfCtrl {
 };
 static_assert(sizeof(RfCtrl) <= kRfCtrlBytes, "control block");
 
-namespace rf {
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes,
-                                          uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
-        : "memory");
-}
-__device__ __forceinline__ void cluster_arrive() {
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void cluster_wait() {
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-    uint32_t r;
-    asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ uint32_t cluster_id_x() {
-    uint32_t r;
-    asm("mov.u32 %0, %%clusterid.x;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void st_cluster_f32x2(uint32_t local_addr, uint32_t rank, float a,
-                                                 float b) {
-    uint32_t remote;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(rank));
-    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(remote), "f"(a), "f"(b)
-                 : "memory");
-}
-__device__ __forceinline__ void st_cluster_f32(uint32_t local_addr, uint32_t rank, float a) {
-    uint32_t remote;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(rank));
-    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(remote), "f"(a) : "memory");
-}
-__device__ __forceinline__ void lds128(uint32_t (&v)[4], uint32_t addr) {
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
-                 : "r"(addr));
-}
-// Streaming (evict-first) stores: the gradient is written once and not read back by this kernel;
-// measured 4.61 ms against 4.74 ms with default stores on config 1 (.wt: 4.77 ms).
-__device__ __forceinline__ void stg128(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-    asm volatile("st.global.cs.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(a), "r"(b), "r"(c),
-                 "r"(d)
-                 : "memory");
-}
-__device__ __forceinline__ uint32_t mul_bf16x2(uint32_t a, uint32_t b) {
-    uint32_t r;
-    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
-    return r;
-}
-__device__ __forceinline__ uint32_t fma_bf16x2(uint32_t a, uint32_t b, uint32_t c) {
-    uint32_t r;
-    asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
-    return r;
-}
-}  // namespace rf
 
 // ---------------------------------------------------------------- the kernel
 // NU = rounds per warp part = ceil(max part units / 32); every round but the last is full for
@@ -154,7 +74,7 @@ __device__ __forceinline__ uint32_t fma_bf16x2(uint32_t a, uint32_t b, uint32_t 
 template <int NU, int CL, bool ENT>
 __global__ void __launch_bounds__(RfShape<CL>::kThreads, RfShape<CL>::kCtasPerSm)
 rows_rf_kernel(RowArgs a, RfPlan p) {
-    using namespace rf;
+    using namespace ptx;
     constexpr int kRfWarps = RfShape<CL>::kWarps;
     constexpr int kRfSlots = RfShape<CL>::kSlots;
     constexpr int NCH = (NU + kRfChunkRounds - 1) / kRfChunkRounds;
@@ -186,7 +106,7 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
 
     if (lane == 0)
         for (int s = 0; s < kRfSlots; ++s) mbar_init(bar0 + 8u * s, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_mbar_init();
     __syncwarp();
     cluster_arrive();     // both CTAs are resident before any distributed-shared-memory store
     cluster_wait();
@@ -346,7 +266,7 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
 #pragma unroll
                 for (int k = 0; k < NU; ++k)
                     if (k < NU - 1 || k * 32 + lane < part_units)
-                        stg128(g + k * (32 * 16), 0u, 0u, 0u, 0u);
+                        stg128_cs(g + k * (32 * 16), 0u, 0u, 0u, 0u);
             } else {
                 // e was taken relative to m (0 if the part held nothing finite)
                 const float F = ts.coef * ex2_approx(fmaf(-ts.lse, kLog2e, -nref));
@@ -367,7 +287,7 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
                             o[j] = (j == y_word) ? ((o[j] & y_keep) | gy2) : o[j];
                     }
                     if (k < NU - 1 || k * 32 + lane < part_units)
-                        stg128(g + k * (32 * 16), o[0], o[1], o[2], o[3]);
+                        stg128_cs(g + k * (32 * 16), o[0], o[1], o[2], o[3]);
                 }
             }
         }
@@ -399,7 +319,9 @@ bool rows_rf_supported(int64_t V, int64_t ld, int dtype) {
 template <int NU, int CL, bool ENT>
 static cudaError_t launch_nu(const RowArgs& a, RfPlan p, int num_sms, cudaStream_t st) {
     using S = RfShape<CL>;
-    static int max_clusters = -1;            // co-resident clusters (device query, cached)
+    static PerDeviceInt cached;              // co-resident clusters (device query, cached per device)
+    const int dev = PerDeviceInt::device();
+    int max_clusters = cached.get(dev);
     cudaLaunchConfig_t cfg = {};
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -422,6 +344,7 @@ static cudaError_t launch_nu(const RowArgs& a, RfPlan p, int num_sms, cudaStream
         if (e != cudaSuccess) return e;
         const int want = num_sms * S::kCtasPerSm / CL;
         max_clusters = n < 1 ? 1 : (n > want ? want : n);
+        cached.set(dev, max_clusters);
     }
     int nc = max_clusters;
     if ((int64_t)nc > a.n_tok) nc = (int)a.n_tok;

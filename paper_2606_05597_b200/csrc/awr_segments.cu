@@ -147,11 +147,11 @@ final_reduce_kernel(const float* __restrict__ tok_term, const uint8_t* __restric
 cudaError_t launch_segment_expand(const int32_t* step_off, const int32_t* traj_off,
                                   const int32_t* group_off, int64_t n_tok, int n_steps,
                                   int n_traj, int n_groups, int32_t* tok_traj, uint32_t* err,
-                                  cudaStream_t st) {
+                                  int num_sms, cudaStream_t st) {
     int64_t work = n_tok > n_steps + 1 ? n_tok : n_steps + 1;
     int blocks = (int)((work + 255) / 256);
     if (blocks < 1) blocks = 1;
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > num_sms * 8) blocks = num_sms * 8;   // 8 CTAs of 256 threads per SM: one wave
     segment_expand_kernel<<<blocks, 256, 0, st>>>(step_off, traj_off, group_off, n_tok, n_steps,
                                                   n_traj, n_groups, tok_traj, err);
     return cudaGetLastError();

@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol():
     out = subprocess.check_output(["nm", "-D", "--defined-only", _abi.lib_path()]).decode()
     exported = set(re.findall(r"\bT (awr_\w+)", out))
     assert exported == set(declared_symbols()), exported ^ set(declared_symbols())
-    assert lib.awr_version() == 100
+    assert lib.awr_version() == 200
 
 
 def test_struct_layout_matches_c(tmp_path):
