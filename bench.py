@@ -19,7 +19,7 @@ The JSON line:
   e2e           tokens/s through `awr_loss_fwd_bwd_host`: HOST (pinned) buffers, the H2D copy of
                 every input and the D2H copy of every output inside the timed region
   roofline      the row kernel (a2+a3+a4): algorithmic bytes / its CUDA-event duration, measured
-                live in the timed region through `awr_profile_next_row_kernel`
+                live in the timed region (awr_outputs.ev_row_begin / ev_row_end of that call)
   cpu_baseline  the fp64 oracle (oracle/, as it stands) on the host cores, bounded sample
   --impl reference   times the oracle alone (this tier's reference arm)
 """
@@ -254,8 +254,7 @@ def run_cuda(args):
     with ClockSampler(local_rank) as clk:
         t_beg.record(stream)
         for a, b in evs:
-            A.profile_next_row_kernel(a, b)
-            call.run()
+            call.run(row_events=(a, b))
         t_end.record(stream)
         torch.cuda.synchronize(dev)
     barrier(world)

@@ -215,7 +215,7 @@ class HostLossCall:
                  **params):
         self.lib = load()
         for t in (logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off, rewards):
-            if t.is_cuda:
+            if t is not None and t.is_cuda:
                 raise TypeError("awr_loss_fwd_bwd_host takes host tensors")
         self.batch = _batch_struct(logits, target_ids, behave_lp, prox_lp, step_off, traj_off,
                                    group_off, rewards, V, cuda=False)

@@ -8,6 +8,14 @@ Bars (BASELINE.json north_star):
               advantages sum to zero per group so the loss is a difference of large sums)
   dlogits     bf16: |d| <= max(2 ulp_bf16(oracle), 1e-3 max_v |oracle row|); rows with c_t = 0
               must be all-bits-zero.  fp32: |d| <= 2e-5 |oracle| + 1e-5 rowmax.
+              Supplementary for bf16 (the 1e-3 rowmax floor hides most non-target entries at
+              V = 151,936): the sum of the NON-TARGET entries of every row against the oracle's
+              c_t (1 - p_y) within 8 sigma of independent bf16 roundings (catches a zeroed or
+              mis-scaled part of a row); tests also compare the cluster kernels with the generic
+              kernel element by element and run a peaked-logits workload.
+
+Every loss comparison is logged (LOSS_LOG: conditioning sum|term| / |sum term|, and whether the
+1e-5 |loss| term alone would have passed) and printed in pytest's terminal summary (conftest.py).
 """
 from __future__ import annotations
 
@@ -21,6 +29,20 @@ from oracle import awr_oracle as O
 LP_ATOL = 1e-4
 LOSS_RTOL = 1e-5
 LOSS_COND_FLOOR = 1e-6
+LOSS_LOG = []          # (label, |loss|, cond, |diff|, rel-only tolerance, passed on the rel term alone)
+
+
+def check_loss(got, ora_loss, ora_term, label=""):
+    """north_star: 1e-5 relative.  DESIGN.md section 3 adds the conditioning floor
+    1e-6 sum|term_t| for batches whose advantages cancel (P3: config 0 at ratio 1 sums to 0)."""
+    abs_sum = float(np.abs(ora_term).sum())
+    diff = abs(float(got) - float(ora_loss))
+    rel_tol = LOSS_RTOL * abs(float(ora_loss))
+    cond = abs_sum / abs(float(ora_loss)) if ora_loss != 0 else float("inf")
+    LOSS_LOG.append((label, abs(float(ora_loss)), cond, diff, rel_tol, diff <= rel_tol))
+    tol = rel_tol + LOSS_COND_FLOOR * abs_sum
+    assert diff <= tol + 1e-30, "loss %r vs oracle %r (tol %g, conditioning %g)" % (
+        float(got), float(ora_loss), tol, cond)
 
 
 def bf16_ulp(x):
@@ -49,7 +71,7 @@ def run_oracle(batch, grad_rows=None, want_dlogits=True, **over):
     return O.awr_loss_fwd_bwd(*args, want_dlogits=want_dlogits, grad_rows=grad_rows, **kw)
 
 
-def check_scalars(gpu, ora, rows=None):
+def check_scalars(gpu, ora, rows=None, label=""):
     """Everything except dlogits.  rows: compare per-token arrays on these rows only."""
     sel = slice(None) if rows is None else np.asarray(rows)
     g = {k: v.cpu().numpy() for k, v in gpu.items() if k != "dlogits"}
@@ -81,13 +103,12 @@ def check_scalars(gpu, ora, rows=None):
             assert int(g["dual_clip_count"][0]) == ora["dual_clip_count"], \
                 "dual_clip_count %d != oracle %d" % (int(g["dual_clip_count"][0]),
                                                      ora["dual_clip_count"])
-        tol = LOSS_RTOL * abs(ora["loss"]) + LOSS_COND_FLOOR * np.abs(ora["term"]).sum()
-        assert abs(float(g["loss"][0]) - ora["loss"]) <= tol + 1e-30, \
-            "loss %r vs oracle %r (tol %g)" % (float(g["loss"][0]), ora["loss"], tol)
+        check_loss(g["loss"][0], ora["loss"], ora["term"], label)
 
 
-def check_dlogits(dl_gpu, ora, V, rows=None):
-    """dl_gpu: torch tensor [n_tok, ld]; ora['dlogits'] holds ora['grad_rows'] rows."""
+def check_dlogits(dl_gpu, ora, V, rows=None, y=None):
+    """dl_gpu: torch tensor [n_tok, ld]; ora['dlogits'] holds ora['grad_rows'] rows.
+    y: target ids of ALL rows (numpy); enables the non-target row-sum check for bf16."""
     grows = ora["grad_rows"]
     G = ora["dlogits"]
     is_bf16 = dl_gpu.dtype == torch.bfloat16
@@ -115,12 +136,79 @@ def check_dlogits(dl_gpu, ora, V, rows=None):
         # P8 holds for the GPU result too: rows sum to ~0 relative to their size
         if not is_bf16:
             assert np.all(np.abs(got.sum(axis=1)) <= 1e-4 * rowmax[:, 0] + 1e-30)
+        elif y is not None:
+            # bf16: every entry is the oracle's value rounded at most twice (e, then e * F), i.e.
+            # an independent error of std <= sqrt(2) ulp / sqrt(12) with ulp <= 2^-7 |entry|.
+            # The non-target entries therefore sum to the oracle's c_t (1 - p_y) within
+            # 8 sigma = 8 sqrt(2) 2^-7 / sqrt(12) ||non-target row||_2 (+ 1e-6 for the lse).
+            yy = np.asarray(y)[idx].astype(np.int64)
+            ok = (yy >= 0) & (yy < V)
+            r = np.arange(idx.size)
+            g_nt, r_nt = got.copy(), ref.copy()
+            g_nt[r[ok], yy[ok]] = 0.0
+            r_nt[r[ok], yy[ok]] = 0.0
+            bound = 8.0 * np.sqrt(2.0 / 12.0) * 2.0 ** -7 * np.sqrt((r_nt ** 2).sum(axis=1)) \
+                + 1e-6 * np.abs(r_nt).sum(axis=1) + 1e-30
+            d = np.abs(g_nt.sum(axis=1) - r_nt.sum(axis=1))
+            assert np.all(d <= bound), "non-target row sum off: row %d, |d| %g > %g" % (
+                idx[int(np.argmax(d / bound))], d.max(), bound[int(np.argmax(d / bound))])
 
 
 def full_check(batch, backward=True, **over):
     gpu = run_gpu(batch, backward=backward, **over)
     ora = run_oracle(batch, want_dlogits=backward, **over)
-    check_scalars(gpu, ora)
+    check_scalars(gpu, ora, label=batch.get("name", ""))
     if backward:
-        check_dlogits(gpu["dlogits"], ora, batch["V"])
+        check_dlogits(gpu["dlogits"], ora, batch["V"], y=batch["target_ids"].cpu().numpy())
     return gpu, ora
+
+
+def oracle_forward_all_rows(batch, params, rows_fn, n_threads=None, chunk=256):
+    """The oracle's forward steps over ALL rows of a full-size batch: O.token_logprob on row
+    chunks (rows_fn(lo, hi) -> exact float32 / float64 logits of rows [lo, hi)), then one
+    O.token_terms call over all tokens and the sequential fp64 sum in token order (O7).  Row
+    chunks only bound memory and let the host's cores work side by side (numpy releases the GIL
+    inside exp / sum); every row goes through the unchanged oracle functions."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    so, to, go = (batch[k].cpu().numpy() for k in ("step_off", "traj_off", "group_off"))
+    rewards = batch["rewards"].cpu().numpy()
+    n_tok, V = batch["n_tok"], batch["V"]
+    flags = params.get("flags", 0)
+    seg = O.segment_expand(so, to, go)
+    adv = O.group_advantage(rewards, go, flags)
+    scale = O.traj_scale(so, to, go, params["k_norm"], params["normalizer"],
+                         params.get("loss_scale", 1.0), rewards, flags)
+    y = batch["target_ids"].cpu().numpy().astype(np.int64)
+    lse = np.empty(n_tok)
+    lp = np.empty(n_tok)
+    zy = np.empty(n_tok)
+
+    def work(lo):
+        hi = min(n_tok, lo + chunk)
+        lse[lo:hi], lp[lo:hi], zy[lo:hi] = O.token_logprob(rows_fn(lo, hi), y[lo:hi])
+
+    n_threads = n_threads or max(1, min(32, len(os.sched_getaffinity(0))))
+    with ThreadPoolExecutor(n_threads) as ex:
+        list(ex.map(work, range(0, n_tok, chunk)))
+    return dict(seg=seg, adv=adv, scale=scale, lse=lse, token_lp=lp, target_logit=zy, y=y,
+                tok_traj=seg["tok_traj"], err_word=O.check_offsets(so, to, go, n_tok))
+
+
+def oracle_terms_all_rows(fw, batch, params):
+    """O4..O7, O9 on the result of oracle_forward_all_rows for one parameter set."""
+    y, V = fw["y"], batch["V"]
+    q = batch["prox_lp"].cpu().numpy()
+    b = batch["behave_lp"].cpu().numpy()
+    if params.get("flags", 0) & O.FLAG_COUPLED:
+        q = b
+    tt = fw["tok_traj"]
+    valid = (y >= 0) & (y < V)
+    term, coef, trig, r, w, dual = O.token_terms(fw["token_lp"], q, b, fw["adv"][tt], fw["scale"][tt],
+                                                 params["clip_eps"], params["stale_cap"], valid,
+                                                 params.get("dual_clip_c", 0.0), want_dual=True)
+    loss = 0.0
+    for t in range(term.size):                                   # O7: token order, fp64
+        loss -= term[t]
+    return dict(fw, term=term, coef=coef, trig=trig, ratio=r, stale_w=w, dual=dual, loss=loss,
+                clip_count=int(trig.sum()), dual_clip_count=int(dual.sum()))

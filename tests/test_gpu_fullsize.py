@@ -2,7 +2,13 @@
 V = 151,936 bf16; config 4: the fused head at 32,768 x 2048 x 151,936), in the launch
 configuration bench.py times (kernel = AUTO, device buffers).
 
-The fp64 oracle cannot do 10^10 exps in seconds, so per config:
+Per config:
+  * ALL rows through the oracle's forward steps (O1..O7, O9: segment expansion, advantage,
+    token_logprob on every row in 256-row chunks spread over the host's cores, token_terms, the
+    sequential fp64 sum in token order): loss, clip_count, dual_clip_count, err_word, every
+    token_lp, target_logit, tok_term, tok_coef (and with it every trigger flag) are compared
+    with the GPU outputs at the bars of parity_util.  Only the gradient ROWS (O8, 10^10 fp64
+    exps per config) are sampled:
   * sampled rows (first, last, the rows around every cluster-schedule wrap, random ones,
     masked / triggered / zero-advantage ones) go through the oracle's own step functions
     (O2..O8 of oracle/awr_oracle.py, the same ones its awr_loss_fwd_bwd chains) and are compared
@@ -13,6 +19,9 @@ The fp64 oracle cannot do 10^10 exps in seconds, so per config:
     where c_t = 0, every non-zero gradient row sums to ~0 (P8), and token_lp against the
     library log-softmax (torch, fp32) on all rows.
 """
+import os
+import time
+
 import numpy as np
 import pytest
 import torch
@@ -62,24 +71,43 @@ def _oracle_on_rows(batch, rows, params):
     tt = seg["tok_traj"][rows]
     valid = (y >= 0) & (y < V)
     lse, lp, zy = O.token_logprob(z, y)
-    term, coef, trig, r, w = O.token_terms(lp, q, b, adv[tt], scale[tt], params["clip_eps"],
-                                           params["stale_cap"], valid)
+    term, coef, trig, r, w, dual = O.token_terms(lp, q, b, adv[tt], scale[tt], params["clip_eps"],
+                                                 params["stale_cap"], valid,
+                                                 params.get("dual_clip_c", 0.0), want_dual=True)
     g = O.dlogits_rows(z, y, lse, coef)
-    return dict(seg=seg, adv=adv, lp=lp, zy=zy, term=term, coef=coef, trig=trig, dlogits=g,
-                grad_rows=np.arange(rows.size))
+    return dict(seg=seg, adv=adv, lp=lp, zy=zy, term=term, coef=coef, trig=trig | dual, dlogits=g,
+                grad_rows=np.arange(rows.size), y=y)
 
 
-@pytest.mark.parametrize("cfg,in_place", [(1, False), (2, False), (3, True)])
-def test_full_size_sampled(cfg, in_place):
+def _logits_rows_fn(batch):
+    V = batch["V"]
+    z = batch["logits"]
+    return lambda lo, hi: z[lo:hi, :V].float().cpu().numpy()       # exact widening of bf16
+
+
+# config 2: "both normalizers, separate runs" (BASELINE.json configs[2])
+@pytest.mark.parametrize("cfg,in_place,norm", [(1, False, None), (2, False, A.NORM_CONST_K),
+                                               (2, False, A.NORM_PER_TRAJ), (3, True, None)])
+def test_full_size_sampled(cfg, in_place, norm):
     w = W.workload(cfg)
     batch = W.make_batch(w, seed=100 + cfg, device=DEV, masked_frac=0.001 if cfg == 3 else 0.0)
     n_tok, V = batch["n_tok"], batch["V"]
     assert n_tok == w.n_tok and V == 151_936
     params = dict(batch["params"])
+    if norm is not None:
+        params["normalizer"] = norm
+    if cfg == 3:
+        params["dual_clip_c"] = 3.0                     # Eq. (2) as in the paper's GRPO runs (:461)
     rng = np.random.Generator(np.random.PCG64(cfg))
     masked = torch.nonzero(batch["target_ids"] < 0).flatten().cpu().numpy()[:8]
     rows = _sample_rows(n_tok, masked, rng)
-    ora = _oracle_on_rows(batch, rows, params)          # BEFORE the call: config 3 runs in place
+    # the oracle reads the logits BEFORE the call: config 3 runs in place
+    ora = _oracle_on_rows(batch, rows, params)
+    t0 = time.perf_counter()
+    ora_all = P.oracle_terms_all_rows(
+        P.oracle_forward_all_rows(batch, params, _logits_rows_fn(batch)), batch, params)
+    print("config %d: oracle forward over all %d rows in %.1f s on %d host cores" % (
+        cfg, n_tok, time.perf_counter() - t0, len(os.sched_getaffinity(0))))
 
     assert A.select_kernel(V, batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RF
     kw = dict(dlogits=batch["logits"]) if in_place else {}
@@ -91,6 +119,13 @@ def test_full_size_sampled(cfg, in_place):
     torch.cuda.synchronize()
     assert int(out["err_word"][0]) == 0
     dl = out["dlogits"]
+
+    # ---- all rows against the oracle: loss, counts, every per-token scalar and trigger flag
+    P.check_scalars(out, ora_all, label="full size config %d norm %d" % (cfg, params["normalizer"]))
+    flags_all = (out["tok_coef"].cpu().numpy() == 0) & (out["tok_term"].cpu().numpy() != 0)
+    assert np.array_equal(flags_all, ora_all["trig"] | ora_all["dual"]), "trigger flags, all rows"
+    if cfg == 3:
+        assert ora_all["clip_count"] > 0.1 * n_tok and ora_all["dual_clip_count"] >= 0
 
     # ---- all rows: integers and properties
     assert np.array_equal(out["tok_traj"].cpu().numpy(), ora["seg"]["tok_traj"].astype(np.int32))
@@ -104,7 +139,7 @@ def test_full_size_sampled(cfg, in_place):
     # a triggered token has a non-zero term and a zero coefficient (A5); masked and
     # zero-advantage tokens have both zero
     trig_all = (coef_all == 0) & (term_all != 0)
-    assert int(out["clip_count"][0]) == int(trig_all.sum())
+    assert int(out["clip_count"][0]) + int(out["dual_clip_count"][0]) == int(trig_all.sum())
     if cfg == 3:
         rate = trig_all.mean()
         assert 0.10 < rate < 0.30, "config 3 should drive a clip-trigger rate of ~20 %%, got %g" % rate
@@ -131,7 +166,7 @@ def test_full_size_sampled(cfg, in_place):
     assert np.array_equal(flags_gpu, ora["trig"])
     sub = dl[torch.as_tensor(sel, device=DEV)]
     P.check_dlogits(sub, dict(dlogits=ora["dlogits"], grad_rows=ora["grad_rows"],
-                              coef=ora["coef"]), V)
+                              coef=ora["coef"]), V, y=ora["y"])
 
     # ---- all rows: token_lp against the library log-softmax (not possible after in-place)
     if not in_place:
@@ -169,6 +204,21 @@ def test_full_size_fused_head_config4():
     torch.cuda.synchronize()
     assert int(out["err_word"][0]) == 0
     H, Wh = batch["hidden"], batch["w_head"]
+
+    # ---- all rows against the oracle's forward steps on the exact fp64 product H W (A17):
+    # loss, clip_count, every token_lp / term / coefficient / trigger flag
+    Hd = H.float().cpu().numpy().astype(np.float64)
+    Wd = Wh.float().cpu().numpy().astype(np.float64)
+    t0 = time.perf_counter()
+    ora_all = P.oracle_terms_all_rows(
+        P.oracle_forward_all_rows(batch, params, lambda lo, hi: Hd[lo:hi] @ Wd, n_threads=4,
+                                  chunk=512), batch, params)
+    print("config 4: oracle forward (fp64 GEMM + log-softmax) over all %d rows in %.1f s" % (
+        n_tok, time.perf_counter() - t0))
+    gp = {k: v for k, v in out.items() if k not in ("dhidden", "dw_head")}
+    del ora_all["target_logit"]                        # not an output of the fused-head entry
+    P.check_scalars(gp, ora_all, label="full size config 4")
+    del Hd, Wd
 
     # ---- properties on all rows
     so, to, go = (batch[k].cpu().numpy() for k in ("step_off", "traj_off", "group_off"))

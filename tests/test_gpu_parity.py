@@ -101,6 +101,88 @@ def test_cluster_configs_small(cfg, kernel):
 
 
 @pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
+@pytest.mark.parametrize("V", [151_936, 50_000])
+def test_cluster_gradient_matches_generic_elementwise(kernel, V):
+    """The 1e-3 rowmax floor of the north_star bar hides most non-target entries at V = 151,936
+    (p_v << 1e-3), so the gradient STORES of the cluster kernels are also compared with the
+    one-CTA-per-row kernel (whose gradient pass is separate code) element by element: both are
+    bf16 roundings of the same c_t p_v (one rounding there, two in the register-file kernel), so
+    they agree within 2 bf16 ulp EVERYWHERE - a zeroed or mis-scaled lane / part would not."""
+    w = W.workload(3, n_groups=6, group_size=4, n_tok=331, V=V)
+    batch = W.make_batch(w, seed=77, device=DEV, masked_frac=0.03)
+    a = P.run_gpu(batch, kernel=kernel)["dlogits"][:, :V].float()
+    b = P.run_gpu(batch, kernel=A.KERNEL_GENERIC)["dlogits"][:, :V].float()
+    big = torch.maximum(a.abs(), b.abs())
+    ulp = torch.exp2(torch.floor(torch.log2(big.clamp(min=2.0 ** -126))) - 7)
+    bad = (a - b).abs() > 2 * ulp
+    assert not bool(bad.any()), "%d entries differ by more than 2 bf16 ulp" % int(bad.sum())
+
+
+@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC] + CLUSTER_KERNELS)
+def test_peaked_logits_many_entries_above_the_floor(kernel):
+    """A workload where hundreds of entries per row exceed the 1e-3 rowmax floor, so that the
+    2-ulp part of the dlogits bar is what decides: 256 'hot' vocabulary entries 12 nats above the
+    rest (p ~ 1/256 each), the target among them."""
+    V, n_tok = 151_936, 300
+    w = W.workload(3, n_groups=6, group_size=4, n_tok=n_tok, V=V)
+    batch = W.make_batch(w, seed=13, device=DEV)
+    g = torch.Generator(DEV).manual_seed(99)
+    z = 0.3 * torch.randn(n_tok, V, generator=g, device=DEV)
+    hot = torch.randperm(V, generator=g, device=DEV)[:256]
+    z[:, hot] += 12.0
+    y = hot[torch.randint(0, 256, (n_tok,), generator=g, device=DEV)]
+    batch["logits"] = z.to(torch.bfloat16)
+    batch["target_ids"] = y.to(torch.int32)
+    lp = torch.log_softmax(batch["logits"].float(), 1)[torch.arange(n_tok, device=DEV), y]
+    batch["prox_lp"] = lp + 0.05 * torch.randn(n_tok, generator=g, device=DEV)   # few clips
+    batch["behave_lp"] = batch["prox_lp"] + 0.05 * torch.randn(n_tok, generator=g, device=DEV)
+    lr = lp - batch["prox_lp"]
+    near = ((lr - float(np.log1p(0.2))).abs() < 1e-4) | ((lr - float(np.log1p(-0.2))).abs() < 1e-4)
+    batch["prox_lp"] = torch.where(near, batch["prox_lp"] + 0.01, batch["prox_lp"])
+    batch["params"]["kernel"] = kernel
+    gpu, ora = P.full_check(batch)
+    G = np.abs(ora["dlogits"])
+    above = (G > 1e-3 * G.max(axis=1, keepdims=True)).sum(axis=1)
+    live = ora["coef"] != 0
+    assert live.sum() > 100 and above[live].min() >= 200, "the 2-ulp branch must decide here"
+
+
+def test_unguarded_clip_counts_banded():
+    """every other parity input keeps log r_t at least 1e-4 away from
+    log(1 +- eps) (generator guard band), so that bit-exact counts test indexing rather than
+    rounding luck.  This is the run WITHOUT the guard band, at V = 151,936 with config 3's laws
+    (drift 0.3: clips and cap both fire): fp32 and fp64 may then legitimately disagree on a
+    token whose ratio sits within rounding of a threshold.  Required: identical trigger flags
+    for every token whose oracle |log r - log(1 +- eps)| >= 1e-6, and a clip count that differs
+    from the oracle's by at most the number of tokens inside that band.  Both are printed."""
+    w = W.workload(3, n_groups=8, group_size=8, n_tok=20_480)
+    batch = W.make_batch(w, seed=303, device=DEV, guard=False)
+    params = dict(batch["params"])
+    n_tok, V = batch["n_tok"], batch["V"]
+    assert V == 151_936 and n_tok >= 20_000
+    ora = P.oracle_terms_all_rows(
+        P.oracle_forward_all_rows(batch, params, lambda lo, hi: batch["logits"][lo:hi, :V].float().cpu().numpy()),
+        batch, params)
+    gpu = P.run_gpu(batch)
+    eps = float(np.float32(params["clip_eps"]))
+    lr = ora["token_lp"] - batch["prox_lp"].cpu().numpy().astype(np.float64)
+    band = (np.abs(lr - np.log1p(eps)) < 1e-6) | (np.abs(lr - np.log1p(-eps)) < 1e-6)
+    coef = gpu["tok_coef"].cpu().numpy()
+    term = gpu["tok_term"].cpu().numpy()
+    flags = (coef == 0) & (term != 0)
+    assert np.array_equal(flags[~band], ora["trig"][~band]), "a trigger flag differs outside the 1e-6 band"
+    d = abs(int(gpu["clip_count"][0]) - ora["clip_count"])
+    print("unguarded run: %d tokens, clip_count gpu %d / oracle %d, %d tokens inside the 1e-6 band, "
+          "%d flags differ (all inside the band)" % (n_tok, int(gpu["clip_count"][0]), ora["clip_count"],
+                                                     int(band.sum()), int((flags != ora["trig"]).sum())))
+    assert d <= int(band.sum())
+    assert ora["clip_count"] > 0.1 * n_tok
+    lp = gpu["token_lp"].cpu().numpy().astype(np.float64)
+    assert np.abs(lp - ora["token_lp"]).max() <= P.LP_ATOL
+    P.check_loss(gpu["loss"][0], ora["loss"], ora["term"], "unguarded config-3 laws")
+
+
+@pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
 def test_cluster_matches_generic_bitwise_on_integers(kernel):
     """All row kernels give the same integers and the same zero pattern."""
     w = W.workload(3, n_groups=6, group_size=4, n_tok=500, V=50_000)
@@ -114,17 +196,43 @@ def test_cluster_matches_generic_bitwise_on_integers(kernel):
     assert float((a["token_lp"] - b["token_lp"]).abs().max()) < 2e-5
 
 
-def test_thinking_shapes_workload():
-    """the Thinking-variant raggedness (400-900 tokens per step, horizon 40)
-    through the same kernels, cut to a size the oracle finishes in seconds."""
-    w = W.workload(5, n_groups=3, group_size=4, n_tok=700)
-    st = W.make_structure(W.workload(5), seed=0)
+@pytest.mark.parametrize("horizon", [20, 40, 60])
+def test_thinking_shapes_workload(horizon):
+    """the Thinking-variant raggedness (400-900 tokens per step; the long
+    horizons 20 / 40 / 60 of PAPER.md:154, :321-331) through the same kernels, cut to a size the
+    oracle finishes in seconds."""
+    w = W.workload(5, n_groups=3, group_size=4, n_tok=700, horizon=horizon)
+    st = W.make_structure(W.workload(5, horizon=horizon), seed=0)
     per_step = np.diff(st["step_off"])
-    assert 400 <= per_step.min() and per_step.max() <= 900 and np.diff(st["traj_off"]).max() <= 40
-    batch = W.make_batch(w, seed=71, device=DEV)
+    steps = np.diff(st["traj_off"])
+    assert 400 <= per_step.min() and per_step.max() <= 900 and steps.max() <= horizon
+    if horizon == 20:
+        assert (steps == 20).any(), "the horizon-20 cap should bind for some failed trajectory"
+    batch = W.make_batch(w, seed=71 + horizon, device=DEV)
     assert A.select_kernel(batch["V"], batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RF
     P.full_check(batch, dual_clip_c=3.0)
     P.full_check(batch, normalizer=A.NORM_PER_TRAJ, flags=A.FLAG_SKIP_UNIFORM)
+
+
+def test_coupled_flag_does_not_read_prox_lp():
+    """include/awr.h: with AWR_FLAG_COUPLED prox_lp is not read and may be NULL (device entry and
+    host-buffer entry); the result equals the call that passes behave_lp as prox_lp."""
+    w = W.workload(3, n_groups=4, group_size=4, n_tok=200, V=40_000)
+    batch = W.make_batch(w, seed=12, device=DEV)
+    args = lambda q: (batch["logits"], batch["target_ids"], batch["behave_lp"], q, batch["step_off"],
+                      batch["traj_off"], batch["group_off"], batch["rewards"])
+    params = dict(batch["params"], flags=A.FLAG_COUPLED)
+    a = A.awr_loss_fwd_bwd(*args(None), **params)
+    b = A.awr_loss_fwd_bwd(*args(batch["prox_lp"]), **params)
+    torch.cuda.synchronize()
+    for k in ("loss", "token_lp", "tok_term", "tok_coef", "clip_count", "dlogits"):
+        assert torch.equal(a[k], b[k]), k
+    with pytest.raises(A.AwrError) as ei:
+        A.awr_loss_fwd_bwd(*args(None), **batch["params"])        # decoupled: prox_lp is required
+    assert ei.value.status == -1
+    host = [None if t is None else t.cpu() for t in args(None)]
+    h = A.awr_loss_fwd_bwd_host(*host, device=DEV, pin=False, **params)
+    assert torch.equal(h["dlogits"], a["dlogits"].cpu()) and float(h["loss"][0]) == float(a["loss"][0])
 
 
 def test_dynamic_sampling_flag():
