@@ -20,7 +20,13 @@ The JSON line:
                 every input and the D2H copy of every output inside the timed region
   roofline      the row kernel (a2+a3+a4): algorithmic bytes / its CUDA-event duration, measured
                 live in the timed region (awr_outputs.ev_row_begin / ev_row_end of that call)
-  cpu_baseline  the fp64 oracle (oracle/, as it stands) on the host cores, bounded sample
+  cpu_baseline  the fp64 oracle (oracle/, as it stands) on the host cores, bounded sample: the
+                rows split over one worker thread per core of the box (numpy releases the GIL;
+                fixed-order final sum), the core count stated, a 1-thread figure beside it
+  others        (N = 1, default config only) the same measurement for the other BASELINE.json
+                configs and for the forward-only path, each with its own roofline and clocks:
+                config 2 under 1/k and under 1/|tau_i|, config 3 into a separate gradient buffer and
+                in place, config 4 (fused LM head, tensor roofline), awr_loss_fwd on config 1
   --impl reference   times the oracle alone (this tier's reference arm)
 """
 from __future__ import annotations
@@ -39,7 +45,11 @@ if ROOT not in sys.path:
 
 METRIC = "loss+grad tokens/s at V=151,936 bf16"
 UNIT = "tokens/s"
-CPU_SAMPLE_TOK = 3072      # rows of the bounded oracle sample (about 10-30 s of CPU work)
+CPU_ROWS_PER_CORE = 192    # rows of the bounded oracle sample per host core (about 10-20 s of work)
+CPU_MAX_ROWS = 24576       # ... capped (the sample batch lives in host memory: 3.7 GB of bf16 values
+                           # widened to fp32 at the cap)
+CPU_1T_ROWS = 1024         # rows of the 1-thread figure
+OTHER_STEPS = 5            # timed steps of every "others" leg (3 warm-ups)
 REF_STEP_TOK = 256         # rows per step of the --impl reference arm
 HEAD_CPU_SAMPLE_TOK = 2048  # rows of the fused-head oracle sample (three fp64 GEMMs of 2048 x 151,936)
 
@@ -165,9 +175,79 @@ def time_oracle(args_kw, repeats: int = 1):
     return dt / repeats, out
 
 
-def host_threads_used() -> int:
-    """The oracle is numpy elementwise code: one thread does the work."""
-    return 1
+def host_cores() -> int:
+    return len(os.sched_getaffinity(0))
+
+
+def time_oracle_rows(host, n_threads: int):
+    """The oracle's own per-row functions (unchanged: O.token_logprob, O.token_terms,
+    O.dlogits_rows, i.e. steps O3..O8 of oracle/awr_oracle.py in the order its awr_loss_fwd_bwd
+    chains them) over all rows of `host`, the rows split into contiguous chunks over `n_threads`
+    worker threads (numpy releases the GIL inside exp / sum), then the fixed-order fp64 sum of
+    the per-token terms in token order (O7).  Returns (seconds, loss)."""
+    import numpy as np
+    from concurrent.futures import ThreadPoolExecutor
+    from oracle import awr_oracle as O
+    p = host["params"]
+    z, y = host["logits"], host["target_ids"].astype(np.int64)
+    n_tok, V = z.shape
+    t0 = time.perf_counter()
+    seg = O.segment_expand(host["step_off"], host["traj_off"], host["group_off"])
+    adv = O.group_advantage(host["rewards"], host["group_off"], p.get("flags", 0))
+    scale = O.traj_scale(host["step_off"], host["traj_off"], host["group_off"], p["k_norm"],
+                         p["normalizer"], p.get("loss_scale", 1.0), host["rewards"], p.get("flags", 0))
+    tt = seg["tok_traj"]
+    term = np.zeros(n_tok)
+    rows_per = max(1, min(64, -(-n_tok // n_threads)))
+
+    def work(lo):
+        hi = min(n_tok, lo + rows_per)
+        lse, lp, zy = O.token_logprob(z[lo:hi], y[lo:hi])
+        valid = (y[lo:hi] >= 0) & (y[lo:hi] < V)
+        t, c, trig, r, w = O.token_terms(lp, host["prox_lp"][lo:hi], host["behave_lp"][lo:hi],
+                                         adv[tt[lo:hi]], scale[tt[lo:hi]], p["clip_eps"],
+                                         p["stale_cap"], valid, p.get("dual_clip_c", 0.0))
+        g = O.dlogits_rows(z[lo:hi], y[lo:hi], lse, c)
+        term[lo:hi] = t
+        return float(g[0, 0])
+
+    if n_threads == 1:
+        for lo in range(0, n_tok, rows_per):
+            work(lo)
+    else:
+        with ThreadPoolExecutor(n_threads) as ex:
+            list(ex.map(work, range(0, n_tok, rows_per)))
+    loss = 0.0
+    for t in range(n_tok):
+        loss -= term[t]
+    return time.perf_counter() - t0, loss
+
+
+def cpu_baseline_rows(cfg: int):
+    """cpu_baseline of the logits path: all host cores, and one thread beside it."""
+    cores = host_cores()
+    n = min(CPU_MAX_ROWS, CPU_ROWS_PER_CORE * cores)
+    _, host = oracle_sample(cfg, n, seed=1234)
+    dt, _ = time_oracle_rows(host, cores)
+    n1 = min(CPU_1T_ROWS, host["n_tok"])
+    host1 = dict(host)
+    for k in ("logits", "target_ids", "behave_lp", "prox_lp"):
+        host1[k] = host[k][:n1]
+    so = host["step_off"]
+    keep = int((so <= n1).sum())                 # whole steps inside the first n1 rows
+    host1 = None if keep < 2 else host1
+    dt1 = None
+    if host1 is not None:
+        _, h1 = oracle_sample(cfg, n1, seed=1234)
+        dt1, _ = time_oracle_rows(h1, 1)
+        n1 = h1["n_tok"]
+    return {"value": host["n_tok"] / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "seconds": dt,
+            "sample": "config-%d laws cut to %d tokens, V=%d; oracle steps O1..O8 (fp64 numpy) with "
+                      "the rows split over %d worker threads, fixed-order sum" % (
+                          cfg, host["n_tok"], host["V"], cores),
+            "one_thread": None if dt1 is None else {"value": n1 / dt1, "unit": UNIT, "cores": 1,
+                                                    "seconds": dt1, "rows": n1}}
 
 
 def run_reference(args):
@@ -194,13 +274,217 @@ def run_reference(args):
             "data": "synthetic",
             "config": {"workload": "BASELINE.json configs[%d]" % args.config,
                        "n_tok_per_step": n_tok, "V": host["V"], "sample": sample},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": host_threads_used(),
-                             "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1,
+                             "kind": "oracle", "sample": sample + " (one thread: oracle.awr_loss_fwd_bwd "
+                                                                  "as it stands)"},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0,
                     "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
     return 0
+
+
+# ---------------------------------------------------------------------------- measurement helpers
+def measured_peaks():
+    """Roofline denominators: MEASURED_PEAKS.json (driver-written on this pool's B200s), else the
+    fallback B200_PROFILING.md states."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm": float(d["hbm_gbs"]), "tensor": float(d["bf16_tflops_sustained"]),
+                "tensor_burst": float(d["bf16_tflops"]), "src": "MEASURED_PEAKS.json (of measured)"}
+    return {"hbm": 6650.0, "tensor": 1400.0, "tensor_burst": 1590.0,
+            "src": "B200_PROFILING.md fallback (of fallback)"}
+
+
+KERNEL_NAMES = {1: "rows_generic_kernel", 2: "rows_cluster_kernel", 3: "rows_rf_kernel<NU,2>",
+                4: "rows_rf_kernel<NU,4>", 8: "rows_fwd_kernel"}
+
+
+def load_traffic(leg: str):
+    """dram bytes (read + write) per launch of the leg's dominant kernel from a committed
+    `ncu --set full` capture: profiles/r2_traffic.txt (JSON text; every entry names its capture).
+    Returns (bytes, capture) or (None, reason) - never a number for a leg it was not taken on."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.txt")
+    if not os.path.exists(p):
+        return None, "no ncu --set full capture committed"
+    with open(p) as f:
+        d = json.load(f)
+    e = d.get(leg)
+    if not e:
+        return None, "no ncu --set full capture of this leg"
+    return e.get("dram_bytes_per_launch"), e.get("capture")
+
+
+def rows_leg(torch, A, W, dev, cfg, steps, warmup, *, seed=1000, normalizer=None, in_place=False,
+             backward=True, kernel=None, n_tok=None, leg="", batch=None, rank_barrier=None):
+    """One timed leg of the logits path: `steps` awr_loss_fwd_bwd (or awr_loss_fwd) calls on a
+    device-resident batch of BASELINE.json configs[cfg]; CUDA events on the launching stream around
+    the region and (through awr_outputs.ev_row_*) around the row kernel of every step; NVML clock
+    samples during the region.  Returns the leg's numbers and the batch (for reuse)."""
+    over = {} if not n_tok else dict(n_tok=n_tok)
+    w = W.workload(cfg, **over)
+    if normalizer is not None:
+        w.params["normalizer"] = normalizer
+    if batch is None:
+        batch = W.make_batch(w, seed=seed, device=dev)
+    n, V = batch["n_tok"], batch["V"]
+    logits = batch["logits"]
+    esz = logits.element_size()
+    params = dict(batch["params"])
+    params["normalizer"] = w.params["normalizer"]
+    if kernel is not None:
+        params["kernel"] = kernel
+    kw = dict(dlogits=logits) if (in_place and backward) else {}
+    call = A.LossCall(logits, batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+                      batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"],
+                      want=("err_word",), backward=backward, **kw, **params)
+    stream = torch.cuda.current_stream(dev)
+    for _ in range(max(3, warmup)):
+        call.run()
+    torch.cuda.synchronize(dev)
+    assert int(call.out["err_word"][0]) == 0
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(steps)]
+    for a, b in evs:           # give every event a handle before the timed region
+        a.record(stream)
+        b.record(stream)
+    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    if rank_barrier:
+        rank_barrier()
+    with ClockSampler(dev.index or 0) as clk:
+        t_beg.record(stream)
+        for ev in evs:
+            call.run(row_events=ev)
+        t_end.record(stream)
+        torch.cuda.synchronize(dev)
+    if rank_barrier:
+        rank_barrier()
+    local_ms = t_beg.elapsed_time(t_end)
+    row_ms = sum(a.elapsed_time(b) for a, b in evs) / len(evs)
+    peaks = measured_peaks()
+    per_tok = algorithmic_bytes_per_token(V, esz) if backward else V * esz + 24
+    alg_bytes = per_tok * n
+    achieved = alg_bytes / (row_ms / 1e3) / 1e9
+    if kernel in (None, A.KERNEL_AUTO):
+        kern = A.KERNEL_FWD_STREAM if (not backward and A.select_kernel(V, batch["ld"], logits.dtype)
+                                       != A.KERNEL_GENERIC) else A.select_kernel(V, batch["ld"], logits.dtype)
+    else:
+        kern = kernel
+    traffic, capture = load_traffic(leg)
+    res = {"ms_per_step": local_ms / steps, "tokens_per_s": n * steps / (local_ms / 1e3),
+           "n_tok": n, "V": V, "steps": steps,
+           "normalizer": "1/k" if params["normalizer"] == A.NORM_CONST_K else "1/|tau_i|",
+           "in_place": bool(in_place and backward), "entry": call._name,
+           "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm"], "unit": "GB/s",
+                        "frac": achieved / peaks["hbm"], "traffic": traffic, "traffic_source": capture,
+                        "kernel": KERNEL_NAMES.get(kern, str(kern)), "kernel_ms": row_ms,
+                        "kernel_share_of_step": row_ms / (local_ms / steps),
+                        "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peaks["src"]},
+           "clocks": clk.summary(), "loss": float(call.out["loss"][0]),
+           "clip_count": int(call.out["clip_count"][0]),
+           "gpu_launches": A.launches_per_call() * steps}
+    return res, batch, call, local_ms
+
+
+def head_leg(torch, A, W, dev, steps, warmup, *, seed=1000, head_kernel="auto", n_tok=None,
+             rank_barrier=None):
+    """One timed leg of the fused LM head (BASELINE.json configs[4]): tensor roofline over the
+    whole step (6 K V algorithmic flops per token: logits, dhidden, dw_head)."""
+    over = {} if not n_tok else dict(n_tok=n_tok)
+    w = W.workload(4, **over)
+    batch = W.make_batch(w, seed=seed, device=dev)
+    n, V, K = batch["n_tok"], batch["V"], w.hidden
+    kcode = {"auto": A.KERNEL_AUTO, "1cta": A.KERNEL_HEAD_1CTA, "2cta": A.KERNEL_HEAD_2CTA,
+             "stored": A.KERNEL_HEAD_2CTA_STORED}[head_kernel]
+    call = A.HeadLossCall(batch["hidden"], batch["w_head"], batch["target_ids"], batch["behave_lp"],
+                          batch["prox_lp"], batch["step_off"], batch["traj_off"], batch["group_off"],
+                          batch["rewards"], want=("err_word",), **dict(batch["params"], kernel=kcode))
+    stream = torch.cuda.current_stream(dev)
+    for _ in range(max(3, warmup)):
+        call.run()
+    torch.cuda.synchronize(dev)
+    assert int(call.out["err_word"][0]) == 0
+    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if rank_barrier:
+        rank_barrier()
+    with ClockSampler(dev.index or 0) as clk:
+        t_beg.record(stream)
+        for _ in range(steps):
+            call.run()
+        t_end.record(stream)
+        torch.cuda.synchronize(dev)
+    if rank_barrier:
+        rank_barrier()
+    local_ms = t_beg.elapsed_time(t_end)
+    peaks = measured_peaks()
+    alg_flops = 6.0 * K * V * n
+    exe_ratio = 1.0 if head_kernel in ("auto", "stored") else 8.0 / 6.0
+    achieved = alg_flops / (local_ms / steps / 1e3) / 1e12
+    res = {"ms_per_step": local_ms / steps, "tokens_per_s": n * steps / (local_ms / 1e3),
+           "n_tok": n, "V": V, "K": K, "steps": steps, "entry": "awr_loss_fwd_bwd_fused_head",
+           "workspace_bytes": int(call.ws_bytes),
+           "roofline": {"bound": "tensor", "achieved": achieved, "peak": peaks["tensor"],
+                        "unit": "TFLOP/s", "frac": achieved / peaks["tensor"], "traffic": None,
+                        "kernel": "head_gemm_kernel<epi, %s> (%s), whole step" % (
+                            "1" if head_kernel == "1cta" else "2",
+                            "3 GEMMs + dS streaming pass per panel" if exe_ratio == 1.0
+                            else "4 GEMMs, logits recomputed"),
+                        "algorithmic_flops_per_step": alg_flops,
+                        "executed_flops_per_step": alg_flops * exe_ratio,
+                        "executed_tflops": achieved * exe_ratio,
+                        "peak_source": peaks["src"] + ": bf16_tflops_sustained (a kernel timed "
+                                                      "inside a long step)"},
+           "clocks": clk.summary(), "loss": float(call.out["loss"][0]),
+           "clip_count": int(call.out["clip_count"][0]), "gpu_launches": call.launches * steps}
+    return res, batch, call, local_ms
+
+
+def other_legs(torch, A, W, dev):
+    """The "others" object of the default line (N = 1): every other BASELINE.json config and the
+    forward-only entry, OTHER_STEPS timed steps each after 3 warm-ups, inputs resident in HBM."""
+    out = {}
+
+    def free():
+        import gc
+        gc.collect()
+        torch.cuda.empty_cache()
+
+    def leg(name, fn):
+        try:
+            out[name] = fn()
+        except Exception as e:                   # a leg that cannot run says so; the line survives
+            out[name] = {"error": repr(e)[:300]}
+        free()
+
+    def cfg1_fwd():
+        r, b, c, _ = rows_leg(torch, A, W, dev, 1, OTHER_STEPS, 3, backward=False, leg="config1_fwd")
+        return r
+
+    def cfg2():
+        r1, b, c, _ = rows_leg(torch, A, W, dev, 2, OTHER_STEPS, 3, normalizer=A.NORM_CONST_K, leg="config2")
+        del c
+        r2, b, c, _ = rows_leg(torch, A, W, dev, 2, OTHER_STEPS, 3, normalizer=A.NORM_PER_TRAJ, batch=b,
+                               leg="config2")
+        return r1, r2
+
+    leg("config1_forward_only", cfg1_fwd)
+    try:
+        out["config2_norm_1_over_k"], out["config2_norm_1_over_tau"] = cfg2()
+    except Exception as e:
+        out["config2_norm_1_over_k"] = out["config2_norm_1_over_tau"] = {"error": repr(e)[:300]}
+    free()
+
+    def cfg3(in_place):
+        r, b, c, _ = rows_leg(torch, A, W, dev, 3, OTHER_STEPS, 3, in_place=in_place, leg="config3")
+        return r
+
+    leg("config3_separate_buffer", lambda: cfg3(False))
+    leg("config3_in_place", lambda: cfg3(True))
+    leg("config4_fused_head", lambda: head_leg(torch, A, W, dev, OTHER_STEPS, 3)[0])
+    return out
 
 
 # ---------------------------------------------------------------------------- the CUDA arm
@@ -214,76 +498,33 @@ def run_cuda(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a B200: there is no CPU path (use --impl reference "
                          "for the oracle)")
+    # ---- CPU baseline first (rank 0, N = 1 only): before the GPU holds tens of GB and while the
+    # host cores are idle; the oracle on a bounded sample, rows over all cores + a 1-thread figure
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline_rows(args.config)
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     init_dist("nccl")
 
-    over = {}
-    if args.n_tok:
-        over["n_tok"] = args.n_tok
-    w = W.workload(args.config, **over)
-    if args.normalizer is not None:
-        w.params["normalizer"] = args.normalizer
-    batch = W.make_batch(w, seed=1000 + rank, device=dev)
+    kernel = {"auto": A.KERNEL_AUTO, "generic": A.KERNEL_GENERIC, "cluster": A.KERNEL_CLUSTER,
+              "rf": A.KERNEL_CLUSTER_RF, "rf4": A.KERNEL_CLUSTER_RF4}[args.kernel]
+    leg, batch, call, local_ms = rows_leg(torch, A, W, dev, args.config, args.steps, args.warmup,
+                                          seed=1000 + rank, normalizer=args.normalizer, kernel=kernel,
+                                          n_tok=args.n_tok or None, leg="config%d" % args.config,
+                                          rank_barrier=lambda: barrier(world))
+    w = W.workload(args.config)
     n_tok, V = batch["n_tok"], batch["V"]
-    logits = batch["logits"]
-    esz = logits.element_size()
     params = dict(batch["params"])
-    params["kernel"] = {"auto": A.KERNEL_AUTO, "generic": A.KERNEL_GENERIC,
-                        "cluster": A.KERNEL_CLUSTER, "rf": A.KERNEL_CLUSTER_RF,
-                        "rf4": A.KERNEL_CLUSTER_RF4}[args.kernel]
-    call = A.LossCall(logits, batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
-                      batch["step_off"], batch["traj_off"], batch["group_off"],
-                      batch["rewards"], want=("err_word",), **params)
-    kern = A.select_kernel(V, batch["ld"], logits.dtype) if args.kernel == "auto" else params["kernel"]
-    stream = torch.cuda.current_stream(dev)
-
-    # ---- device-resident leg
-    for _ in range(args.warmup):
-        call.run()
-    torch.cuda.synchronize(dev)
-    assert int(call.out["err_word"][0]) == 0
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-           for _ in range(args.steps)]
-    for a, b in evs:           # give every event a handle before the timed region
-        a.record(stream)
-        b.record(stream)
-    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize(dev)
-    barrier(world)
-    with ClockSampler(local_rank) as clk:
-        t_beg.record(stream)
-        for a, b in evs:
-            call.run(row_events=(a, b))
-        t_end.record(stream)
-        torch.cuda.synchronize(dev)
-    barrier(world)
-    local_ms = t_beg.elapsed_time(t_end)
-    row_ms = [a.elapsed_time(b) for a, b in evs]
+    if args.normalizer is not None:
+        params["normalizer"] = args.normalizer
+    params["kernel"] = kernel
+    esz = batch["logits"].element_size()
     total_ms, total_tok = aggregate(local_ms, n_tok * args.steps, world, dev)
     ms_per_step = total_ms / args.steps
     value = total_tok / (total_ms / 1e3)
-    loss = float(call.out["loss"][0])
-    clips = int(call.out["clip_count"][0])
-
-    # ---- roofline of the dominant kernel (this rank's)
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        with open(peaks_path) as f:
-            peak, peak_src = float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
-    else:
-        peak, peak_src = 6650.0, "B200_PROFILING.md fallback (of fallback)"
-    alg_bytes = algorithmic_bytes_per_token(V, esz) * n_tok
-    row_avg_ms = sum(row_ms) / len(row_ms)
-    achieved = alg_bytes / (row_avg_ms / 1e3) / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": load_traffic(args.config),
-                "kernel": {A.KERNEL_GENERIC: "rows_generic_kernel",
-                           A.KERNEL_CLUSTER: "rows_cluster_kernel",
-                           A.KERNEL_CLUSTER_RF: "rows_rf_kernel<NU,2>",
-                           A.KERNEL_CLUSTER_RF4: "rows_rf_kernel<NU,4>"}[kern],
-                "kernel_ms": row_avg_ms, "kernel_share_of_step": row_avg_ms / (local_ms / args.steps),
-                "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src}
+    loss, clips = leg["loss"], leg["clip_count"]
+    stream = torch.cuda.current_stream(dev)
 
     # ---- end-to-end leg: host buffers through awr_loss_fwd_bwd_host
     e2e = None
@@ -294,29 +535,25 @@ def run_cuda(args):
                   "group_off", "rewards"):
             host_in[k] = torch.empty(batch[k].shape, dtype=batch[k].dtype,
                                      pin_memory=True).copy_(batch[k])
-        del call, logits
+        del call
         batch.pop("logits")
         torch.cuda.empty_cache()
-        hparams = dict(params)
         hcall = A.HostLossCall(host_in["logits"], host_in["target_ids"], host_in["behave_lp"],
                                host_in["prox_lp"], host_in["step_off"], host_in["traj_off"],
                                host_in["group_off"], host_in["rewards"], device=dev, V=V,
-                               **hparams)
+                               **params)
         for _ in range(max(1, min(args.warmup, 2))):
             hcall.run()
         torch.cuda.synchronize(dev)
         barrier(world)
         t0 = time.perf_counter()
-        e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e_beg.record(stream)
         for _ in range(e2e_steps):
             hcall.run()                 # returns once the results are in the host buffers
-        e_end.record(stream)
         torch.cuda.synchronize(dev)
         wall_ms = (time.perf_counter() - t0) * 1e3
         barrier(world)
         # the host call synchronises internally on its own streams: wall clock is the honest
-        # end-to-end time; the event pair on the caller's stream is recorded for reference
+        # end-to-end time
         e_ms, e_tok = aggregate(wall_ms, n_tok * e2e_steps, world, dev)
         assert int(hcall.out["err_word"][0]) == 0
         e_loss = float(hcall.out["loss"][0])
@@ -325,17 +562,18 @@ def run_cuda(args):
                "steps": e2e_steps, "ms_per_step": e_ms / e2e_steps,
                "api": "awr_loss_fwd_bwd_host (pinned host buffers, 256 MB row panels)",
                "loss_matches_device_leg": e_loss == loss}
+        del hcall, host_in
+    else:
+        del call
+    batch.clear()
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
 
-    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only)
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu:
-        akw, host = oracle_sample(args.config, CPU_SAMPLE_TOK, seed=1234)
-        dt, _ = time_oracle(akw)
-        cpu = {"value": host["n_tok"] / dt, "unit": UNIT, "cores": host_threads_used(),
-               "kind": "oracle", "seconds": dt,
-               "sample": "config-%d laws cut to %d tokens, V=%d, one pass of "
-                         "oracle.awr_loss_fwd_bwd (fp64 numpy)" % (args.config, host["n_tok"],
-                                                                    host["V"])}
+    # ---- the other configs and the forward-only entry (N = 1, default workload only)
+    others = None
+    if rank == 0 and world == 1 and args.config == 1 and not args.no_others and not args.n_tok:
+        others = other_legs(torch, A, W, dev)
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
@@ -346,15 +584,15 @@ def run_cuda(args):
                 "config": {"workload": ("BASELINE.json configs[%d] (%s)" if args.config < 5 else
                                         "not in BASELINE.json: workload %d (%s)") % (args.config, w.name),
                            "n_tok_per_gpu": n_tok, "V": V, "n_groups": w.n_groups,
-                           "group_size": w.group_size, "normalizer":
-                               "1/k" if params["normalizer"] == A.NORM_CONST_K else "1/|tau_i|",
+                           "group_size": w.group_size, "normalizer": leg["normalizer"],
                            "k_norm": params["k_norm"], "clip_eps": params["clip_eps"],
                            "stale_cap": params["stale_cap"],
                            "parallelism": "replicas only x%d" % world,
-                           "l2": "inputs (%.1f GB/step) larger than L2, no flush" % (alg_bytes / 1e9)},
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
-                "gpu_launches": A.launches_per_call() * args.steps,
-                "clocks": clk.summary(), "loss": loss, "clip_count": clips}
+                           "l2": "inputs (%.1f GB/step) larger than L2, no flush" % (
+                               leg["roofline"]["algorithmic_bytes_per_launch"] / 1e9)},
+                "roofline": leg["roofline"], "cpu_baseline": cpu, "e2e": e2e,
+                "gpu_launches": leg["gpu_launches"],
+                "clocks": leg["clocks"], "loss": loss, "clip_count": clips, "others": others}
         print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist
@@ -366,8 +604,8 @@ def run_head(args):
     """--config 4: the fused LM-head variant (a5).  A step = one awr_loss_fwd_bwd_fused_head call
     (hidden [32,768, 2048] and W_head [2048, 151,936] in, loss / dhidden / dw_head out).  The
     roofline is the tensor pipe: algorithmic flops 6 K V per token (logits, dH, dW).  The default
-    mode executes exactly those (the fp32 logits of one row panel are kept for a streaming dS
-    pass); --head-kernel 1cta / 2cta recompute the logits tile instead (8 K V executed)."""
+    mode executes exactly those; --head-kernel 1cta / 2cta recompute the logits tile instead
+    (8 K V executed)."""
     import torch
 
     import paper_2606_05597_b200 as A
@@ -379,78 +617,43 @@ def run_head(args):
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     init_dist("nccl")
-    over = {}
-    if args.n_tok:
-        over["n_tok"] = args.n_tok
-    w = W.workload(4, **over)
-    batch = W.make_batch(w, seed=1000 + rank, device=dev)
-    n_tok, V, K = batch["n_tok"], batch["V"], w.hidden
-    call = A.HeadLossCall(batch["hidden"], batch["w_head"], batch["target_ids"],
-                          batch["behave_lp"], batch["prox_lp"], batch["step_off"],
-                          batch["traj_off"], batch["group_off"], batch["rewards"],
-                          want=("err_word",),
-                          **dict(batch["params"], kernel={"auto": A.KERNEL_AUTO, "1cta": A.KERNEL_HEAD_1CTA,
-                                                          "2cta": A.KERNEL_HEAD_2CTA,
-                                                          "stored": A.KERNEL_HEAD_2CTA_STORED}[args.head_kernel]))
-    stream = torch.cuda.current_stream(dev)
-    for _ in range(args.warmup):
-        call.run()
-    torch.cuda.synchronize(dev)
-    assert int(call.out["err_word"][0]) == 0
-    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier(world)
-    with ClockSampler(local_rank) as clk:
-        t_beg.record(stream)
-        for _ in range(args.steps):
-            call.run()
-        t_end.record(stream)
-        torch.cuda.synchronize(dev)
-    barrier(world)
-    local_ms = t_beg.elapsed_time(t_end)
+    leg, batch, call, local_ms = head_leg(torch, A, W, dev, args.steps, args.warmup, seed=1000 + rank,
+                                          head_kernel=args.head_kernel, n_tok=args.n_tok or None,
+                                          rank_barrier=lambda: barrier(world))
+    w = W.workload(4)
+    n_tok, V, K = leg["n_tok"], leg["V"], leg["K"]
     total_ms, total_tok = aggregate(local_ms, n_tok * args.steps, world, dev)
     ms_per_step = total_ms / args.steps
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        with open(peaks_path) as f:
-            peak = float(json.load(f)["bf16_tflops_sustained"])
-        peak_src = "MEASURED_PEAKS.json bf16_tflops_sustained (of measured)"
-    else:
-        peak, peak_src = 1400.0, "B200_PROFILING.md fallback (of fallback)"
+    stream = torch.cuda.current_stream(dev)
     # ---- end-to-end leg: pinned host hidden / W_head in, dhidden / dw_head / loss out, through
-    # the public binding; copies inside the timed region, every step
+    # the C-ABI host entry (awr_loss_fwd_bwd_fused_head_host); copies inside the timed region
     e2e = None
     if not args.no_e2e:
         e2e_steps = args.e2e_steps or args.steps
         hin = {k: torch.empty(batch[k].shape, dtype=batch[k].dtype, pin_memory=True).copy_(batch[k])
-               for k in ("hidden", "w_head", "target_ids", "behave_lp", "prox_lp")}
-        hout = {k: torch.empty(call.out[k].shape, dtype=call.out[k].dtype, pin_memory=True)
-                for k in ("dhidden", "dw_head", "loss", "token_lp", "clip_count")}
-        h2d = sum(t.numel() * t.element_size() for t in hin.values())
-        d2h = sum(t.numel() * t.element_size() for t in hout.values())
-
-        def e2e_step():
-            for k, t in hin.items():
-                batch[k].copy_(t, non_blocking=True)
-            call.run()
-            for k, t in hout.items():
-                t.copy_(call.out[k], non_blocking=True)
-
-        e2e_step()
+               for k in ("hidden", "w_head", "target_ids", "behave_lp", "prox_lp", "step_off",
+                         "traj_off", "group_off", "rewards")}
+        dev_loss = float(call.out["loss"][0])
+        hcall = A.HostHeadLossCall(hin["hidden"], hin["w_head"], hin["target_ids"], hin["behave_lp"],
+                                   hin["prox_lp"], hin["step_off"], hin["traj_off"], hin["group_off"],
+                                   hin["rewards"], device=dev, workspace=call.workspace,
+                                   **dict(batch["params"], kernel=call.params.kernel))
+        hcall.run()
         torch.cuda.synchronize(dev)
         barrier(world)
-        e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e_beg.record(stream)
+        t0 = time.perf_counter()
         for _ in range(e2e_steps):
-            e2e_step()
-        e_end.record(stream)
+            hcall.run()
         torch.cuda.synchronize(dev)
+        wall_ms = (time.perf_counter() - t0) * 1e3
         barrier(world)
-        e_ms, e_tok = aggregate(e_beg.elapsed_time(e_end), n_tok * e2e_steps, world, dev)
-        e2e = {"value": e_tok / (e_ms / 1e3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "steps": e2e_steps, "ms_per_step": e_ms / e2e_steps,
-               "api": "awr_loss_fwd_bwd_fused_head on device buffers refilled from pinned host "
-                      "memory each step; dhidden, dw_head, loss, token_lp copied back",
-               "loss_matches_device_leg": float(hout["loss"][0]) == float(call.out["loss"][0])}
+        e_ms, e_tok = aggregate(wall_ms, n_tok * e2e_steps, world, dev)
+        e2e = {"value": e_tok / (e_ms / 1e3), "unit": UNIT, "h2d_bytes_per_step": int(hcall.h2d_bytes),
+               "d2h_bytes_per_step": int(hcall.d2h_bytes), "steps": e2e_steps,
+               "ms_per_step": e_ms / e2e_steps,
+               "api": "awr_loss_fwd_bwd_fused_head_host (pinned host hidden / W_head in; dhidden, "
+                      "dw_head, loss, token_lp back)",
+               "loss_matches_device_leg": float(hcall.out["loss"][0]) == dev_loss}
 
     # ---- CPU baseline: the fused-head oracle on a bounded sample (rank 0, N = 1 only)
     cpu = None
@@ -462,15 +665,13 @@ def run_head(args):
         t0 = time.perf_counter()
         O.awr_loss_fwd_bwd_fused_head(*oargs, **okw)
         dt = time.perf_counter() - t0
-        cpu = {"value": host["n_tok"] / dt, "unit": UNIT, "cores": len(os.sched_getaffinity(0)),
+        cpu = {"value": host["n_tok"] / dt, "unit": UNIT, "cores": host_cores(),
                "kind": "oracle", "seconds": dt,
                "sample": "config-4 laws cut to %d tokens, K=%d, V=%d, one pass of "
                          "oracle.awr_loss_fwd_bwd_fused_head (fp64 numpy; its three matmuls use "
-                         "the BLAS threads numpy was built with)" % (host["n_tok"], K, V)}
+                         "the BLAS threads numpy was built with, the rest one thread)" % (
+                             host["n_tok"], K, V)}
 
-    alg_flops = 6.0 * K * V * n_tok
-    exe_ratio = 1.0 if args.head_kernel in ("auto", "stored") else 8.0 / 6.0
-    achieved = alg_flops / (local_ms / args.steps / 1e3) / 1e12
     if rank == 0:
         line = {"metric": METRIC + " (fused LM-head variant)", "value": total_tok / (total_ms / 1e3),
                 "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -479,35 +680,16 @@ def run_head(args):
                 "config": {"workload": "BASELINE.json configs[4] (%s)" % w.name,
                            "n_tok_per_gpu": n_tok, "V": V, "K": K, "w_layout": "K_BY_V",
                            "parallelism": "replicas only x%d" % world,
-                           "l2": "W_head (622 MB) + dS panels (1.4-2.9 GB) larger than L2, no flush"},
-                "roofline": {"bound": "tensor", "achieved": achieved, "peak": peak,
-                             "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
-                             "kernel": "head_gemm_kernel<epi, %s> (%s), whole step" % (
-                                 "1" if args.head_kernel == "1cta" else "2",
-                                 "3 GEMMs + dS streaming pass per panel" if exe_ratio == 1.0
-                                 else "4 GEMMs, logits recomputed"),
-                             "algorithmic_flops_per_step": alg_flops,
-                             "executed_flops_per_step": alg_flops * exe_ratio,
-                             "executed_tflops": achieved * exe_ratio, "peak_source": peak_src},
-                "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": call.launches * args.steps,
-                "clocks": clk.summary(), "loss": float(call.out["loss"][0]),
-                "clip_count": int(call.out["clip_count"][0])}
+                           "workspace_bytes": leg["workspace_bytes"],
+                           "l2": "W_head (622 MB) + the dS panel larger than L2, no flush"},
+                "roofline": leg["roofline"],
+                "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": leg["gpu_launches"],
+                "clocks": leg["clocks"], "loss": leg["loss"], "clip_count": leg["clip_count"]}
         print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
     return 0
-
-
-def load_traffic(cfg: int):
-    """dram bytes (read + write) per launch of the row kernel from the committed `ncu --set full`
-    capture (profiles/r1_traffic.txt, JSON text written by hand from the capture named there), or null."""
-    p = os.path.join(ROOT, "profiles", "r1_traffic.txt")
-    if not os.path.exists(p):
-        return None
-    with open(p) as f:
-        d = json.load(f)
-    return d.get("config%d" % cfg, {}).get("dram_bytes_per_launch")
 
 
 def main(argv=None):
@@ -527,6 +709,8 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: --steps")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-others", action="store_true",
+                    help="skip the legs for the other configs / the forward-only entry")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3                   # timing rule: at least 3 warm-up steps

@@ -97,9 +97,13 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_HEAD_1CTA = 5, /* tcgen05 cta_group::1, 128 x 256 tiles, one CTA per SM; the
                                     logits tile is recomputed for the backward (8 K V flops/token) */
        AWR_KERNEL_HEAD_2CTA = 6, /* tcgen05 cta_group::2, 256 x 256 tiles on CTA pairs; recompute */
-       AWR_KERNEL_HEAD_2CTA_STORED = 7 /* CTA pairs; the fp32 logits of ONE row panel (<= 9,472
+       AWR_KERNEL_HEAD_2CTA_STORED = 7, /* CTA pairs; the fp32 logits of ONE row panel (<= 9,472
                                     rows, workspace) are kept between the forward GEMM and a
-                                    streaming dS pass: 6 K V flops/token, same bits as recompute */ };
+                                    streaming dS pass: 6 K V flops/token, same bits as recompute */
+       /* awr_loss_fwd only (its AUTO choice for bf16 rows of >= 64 KB): */
+       AWR_KERNEL_FWD_STREAM = 8 /* forward-only streaming kernel: whole rows through a ring of TMA
+                                    bulk copies, one persistent CTA per SM, no row residency (bf16,
+                                    V and ld multiples of 8); with awr_loss_fwd_bwd -> AWR_ERR_PARAM */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u };
 
@@ -240,6 +244,17 @@ AWR_API int awr_loss_fwd_bwd_fused_head(const awr_head_batch* batch, const awr_p
                                 size_t workspace_bytes, void* stream);
 AWR_API size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
                                 int32_t n_traj, int32_t n_groups);
+
+/* a5 with HOST buffers (the `e2e` leg of bench.py --config 4): every pointer in `host_batch` and
+ * `host_out` is a host pointer (pinned memory gives full PCIe speed).  hidden, w_head and the
+ * per-token arrays are copied to `dev_workspace`, awr_loss_fwd_bwd_fused_head runs there, and
+ * dhidden, dw_head, loss, token_lp and the optional outputs are copied back, all on `stream`; the
+ * call returns after the results are in the host buffers (it synchronises `stream`). */
+AWR_API int awr_loss_fwd_bwd_fused_head_host(const awr_head_batch* host_batch, const awr_params* params,
+                                     const awr_head_outputs* host_out, void* dev_workspace,
+                                     size_t dev_workspace_bytes, void* stream);
+AWR_API size_t awr_head_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
+                                     int32_t n_traj, int32_t n_groups);
 
 /* Note: in the stored-logits mode the call forks the dS pass of each row panel onto a library-owned
  * side stream (created once per device) and joins it back before the panel's dhidden GEMM; from

@@ -347,6 +347,72 @@ def awr_loss_fwd_bwd_fused_head(hidden, w_head, target_ids, behave_lp, prox_lp, 
                         group_off, rewards, **kw).run(stream)
 
 
+def head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups) -> int:
+    return int(load().awr_head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups))
+
+
+class HostHeadLossCall:
+    """awr_loss_fwd_bwd_fused_head_host: every tensor is a HOST tensor (pinned for full PCIe
+    speed); the library copies them into ``workspace`` on the device, runs the fused head there
+    and returns once dhidden, dw_head, loss, token_lp (+ optional outputs) are in the host
+    buffers.  ``h2d_bytes`` / ``d2h_bytes`` are the bytes one call copies."""
+
+    def __init__(self, hidden, w_head, target_ids, behave_lp, prox_lp, step_off, traj_off,
+                 group_off, rewards, *, device, w_layout=_abi.W_K_BY_V, want=("err_word",),
+                 workspace=None, pin=True, **params):
+        self.lib = load()
+        host = (hidden, w_head, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off, rewards)
+        for t in host:
+            if t is not None and t.is_cuda:
+                raise TypeError("awr_loss_fwd_bwd_fused_head_host takes host tensors")
+        _req(hidden, torch.bfloat16, "hidden", cuda=False)
+        _req(w_head, torch.bfloat16, "w_head", cuda=False)
+        n_tok, K = hidden.shape
+        V = w_head.shape[1] if w_layout == _abi.W_K_BY_V else w_head.shape[0]
+        n_steps, n_traj, n_groups = step_off.numel() - 1, traj_off.numel() - 1, group_off.numel() - 1
+        self.device = torch.device(device)
+        self.batch = awr_head_batch(n_tok, V, K, _ptr(hidden), _ptr(w_head), _ptr(target_ids),
+                                    _ptr(behave_lp), _ptr(prox_lp), _ptr(step_off), _ptr(traj_off),
+                                    _ptr(group_off), _ptr(rewards), n_steps, n_traj, n_groups,
+                                    int(w_layout))
+        self.params = make_params(**params)
+        mk = (lambda *a, **k: torch.empty(*a, **k).pin_memory()) if pin else torch.empty
+        o = dict(loss=mk(1, dtype=torch.float32), dhidden=mk(hidden.shape, dtype=torch.bfloat16),
+                 dw_head=mk(w_head.shape, dtype=torch.bfloat16), token_lp=mk(n_tok, dtype=torch.float32),
+                 clip_count=mk(1, dtype=torch.int64), dual_clip_count=mk(1, dtype=torch.int64))
+        spec = dict(adv=(n_traj, torch.float32), tok_traj=(n_tok, torch.int32),
+                    tok_term=(n_tok, torch.float32), tok_coef=(n_tok, torch.float32),
+                    err_word=(1, torch.int32), token_entropy=(n_tok, torch.float32))
+        for k in want:
+            nn, dt = spec[k]
+            o[k] = mk(nn, dtype=dt)
+        self.out = o
+        g = o.get
+        self.outs = awr_head_outputs(_ptr(g("loss")), _ptr(g("dhidden")), _ptr(g("dw_head")),
+                                     _ptr(g("token_lp")), _ptr(g("clip_count")), _ptr(g("adv")),
+                                     _ptr(g("tok_traj")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
+                                     _ptr(g("err_word")), _ptr(g("dual_clip_count")),
+                                     _ptr(g("token_entropy")))
+        need = head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups)
+        if workspace is not None and workspace.numel() >= need:
+            self.workspace = workspace
+        else:
+            self.workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=self.device)
+        self._keep = host
+        small_in = 12 * n_tok + 4 * (n_steps + n_traj + n_groups + 3) + 4 * n_traj
+        self.h2d_bytes = 2 * (n_tok * K + K * V) + small_in
+        self.d2h_bytes = 2 * (n_tok * K + K * V) + 4 * n_tok + 20 + sum(
+            o[k].numel() * o[k].element_size() for k in want)
+
+    def run(self, stream=None):
+        with torch.cuda.device(self.device):
+            rc = self.lib.awr_loss_fwd_bwd_fused_head_host(
+                C.byref(self.batch), C.byref(self.params), C.byref(self.outs), _ptr(self.workspace),
+                self.workspace.numel(), _stream_ptr(stream, self.device))
+        check(rc, "awr_loss_fwd_bwd_fused_head_host")
+        return self.out
+
+
 def awr_gemm_bf16(a, b, a_major=0, b_major=0, kernel=KERNEL_AUTO, stream=None):
     """C = A B on the tcgen05 engine of the fused head.  `a` is stored [M, Kc] (a_major 0) or
     [Kc, M] (a_major 1); `b` is stored [N, Kc] (b_major 0) or [Kc, N] (b_major 1)."""

@@ -68,7 +68,7 @@ static int check_params(const awr_params* p) {
     if (p->flags & ~(uint32_t)(AWR_FLAG_SAMPLE_STD | AWR_FLAG_SUCCESS_FILTER | AWR_FLAG_COUPLED |
                                AWR_FLAG_SKIP_UNIFORM))
         return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_STORED) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_FWD_STREAM) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -89,8 +89,15 @@ static int resolve_head_stored(int requested) {
     return requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA_STORED;
 }
 
-static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool want_entropy = false) {
+static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool want_entropy = false,
+                          bool backward = true) {
+    if (requested == AWR_KERNEL_FWD_STREAM)                   // forward only, bf16, 16-byte units
+        return (!backward && rows_fwd_supported(V, ld, dtype)) ? AWR_KERNEL_FWD_STREAM : -1;
     if (requested > AWR_KERNEL_CLUSTER_RF4) return -1;        // a fused-head kernel id
+    // forward only: nothing has to stay on chip for a second pass, so whole rows are streamed
+    // (config 1: see DESIGN.md section 4 for the measured rates of all the kernels on this path)
+    if (!backward && requested == AWR_KERNEL_AUTO && V * 2 >= 65536 && rows_fwd_supported(V, ld, dtype))
+        return AWR_KERNEL_FWD_STREAM;
     // token_entropy is produced by the generic and the register-file kernels
     if (want_entropy && requested == AWR_KERNEL_CLUSTER) return -1;
     if (want_entropy && requested == AWR_KERNEL_AUTO && V * 2 >= 65536 && !rows_rf_supported(V, ld, dtype))
@@ -109,6 +116,7 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool 
 
 static cudaError_t launch_rows(int kernel, const RowArgs& a, int dtype, int num_sms,
                                cudaStream_t st) {
+    if (kernel == AWR_KERNEL_FWD_STREAM) return launch_rows_fwd(a, num_sms, st);
     if (kernel == AWR_KERNEL_CLUSTER_RF) return launch_rows_rf(a, num_sms, 2, st);
     if (kernel == AWR_KERNEL_CLUSTER_RF4) return launch_rows_rf(a, num_sms, 4, st);
     if (kernel == AWR_KERNEL_CLUSTER) return launch_rows_cluster(a, num_sms, st);
@@ -137,11 +145,8 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     if (backward && (reinterpret_cast<uintptr_t>(o->dlogits) & 15)) return AWR_ERR_ALIGN;
     const size_t need = awr_workspace_bytes(b->n_tok, b->V, b->n_steps, b->n_traj, b->n_groups);
     if (!ws_ptr || (reinterpret_cast<uintptr_t>(ws_ptr) & 255) || ws_bytes < need) return AWR_ERR_WORKSPACE;
-    int kernel = resolve_kernel(p->kernel, b->V, b->ld, b->logits_dtype, o->token_entropy != nullptr);
-    // forward only (no row has to stay on chip for a second pass): the one-CTA-per-row kernel
-    // streams faster than the cluster kernels (config 1: 2.56 ms = 4.9 TB/s against 3.05 ms);
-    // with the entropy output its online rescaling of a third accumulator costs more (3.84 ms)
-    if (!backward && p->kernel == AWR_KERNEL_AUTO && !o->token_entropy) kernel = AWR_KERNEL_GENERIC;
+    const int kernel = resolve_kernel(p->kernel, b->V, b->ld, b->logits_dtype, o->token_entropy != nullptr,
+                                      backward);
     if (kernel < 0) return AWR_ERR_PARAM;
 
     DeviceInfo info;
@@ -359,6 +364,131 @@ int awr_gemm_bf16(const void* A, int32_t a_major, int64_t lda, const void* B, in
     return AWR_OK;
 }
 
+// ------------------------------------------------------------------ a5 with HOST buffers
+namespace {
+struct HeadHostPlan {
+    size_t hidden, w, dh, dw, tok, steps, traj, groups, rew, adv, total_small, head_ws, total;
+};
+HeadHostPlan head_host_plan(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps, int32_t n_traj,
+                            int32_t n_groups) {
+    HeadHostPlan h;
+    h.hidden = align_up((size_t)n_tok * K * 2, 256);
+    h.w = align_up((size_t)K * V * 2, 256);
+    h.dh = h.hidden;
+    h.dw = h.w;
+    h.tok = align_up((size_t)n_tok * 4, 256);
+    h.steps = align_up((size_t)(n_steps + 1) * 4, 256);
+    h.traj = align_up((size_t)(n_traj + 1) * 4, 256);
+    h.groups = align_up((size_t)(n_groups + 1) * 4, 256);
+    h.rew = align_up((size_t)n_traj * 4, 256);
+    h.adv = h.rew;
+    // ids, b, q in; lp, term, coef, tok_traj, entropy out; offsets; rewards; adv; scalars
+    h.total_small = 8 * h.tok + h.steps + h.traj + h.groups + h.rew + h.adv + 256;
+    h.head_ws = awr_head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups);
+    h.total = h.hidden + h.w + h.dh + h.dw + h.total_small + h.head_ws;
+    return h;
+}
+}  // namespace
+
+size_t awr_head_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
+                                     int32_t n_traj, int32_t n_groups) {
+    if (n_tok < 0 || V <= 0 || K <= 0 || n_steps < 0 || n_traj < 0 || n_groups < 0) return 0;
+    return head_host_plan(n_tok, V, K, n_steps, n_traj, n_groups).total;
+}
+
+int awr_loss_fwd_bwd_fused_head_host(const awr_head_batch* hb, const awr_params* p,
+                                     const awr_head_outputs* ho, void* dev_ws, size_t dev_ws_bytes,
+                                     void* stream) {
+    if (!hb || !p || !ho) return AWR_ERR_NULL;
+    int rc = check_segments(hb->n_tok, hb->n_steps, hb->n_traj, hb->n_groups);
+    if (rc) return rc;
+    if (hb->V <= 0 || hb->K <= 0 || hb->V % 8 != 0 || hb->K % 64 != 0) return AWR_ERR_SHAPE;
+    rc = check_params(p);
+    if (rc) return rc;
+    const bool coupled = (p->flags & AWR_FLAG_COUPLED) != 0;
+    if (!ho->loss || !ho->clip_count || !ho->dw_head) return AWR_ERR_NULL;
+    if (hb->n_tok > 0 && (!ho->token_lp || !ho->dhidden)) return AWR_ERR_NULL;
+    if (!hb->step_off || !hb->traj_off || !hb->group_off || !hb->w_head) return AWR_ERR_NULL;
+    if (hb->n_tok > 0 && (!hb->hidden || !hb->target_ids || !hb->behave_lp || (!coupled && !hb->prox_lp)))
+        return AWR_ERR_NULL;
+    if (hb->n_traj > 0 && !hb->rewards) return AWR_ERR_NULL;
+    const HeadHostPlan hp = head_host_plan(hb->n_tok, hb->V, hb->K, hb->n_steps, hb->n_traj, hb->n_groups);
+    if (!dev_ws || (reinterpret_cast<uintptr_t>(dev_ws) & 255) || dev_ws_bytes < hp.total) return AWR_ERR_WORKSPACE;
+
+    const int64_t n = hb->n_tok;
+    uint8_t* base = reinterpret_cast<uint8_t*>(dev_ws);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { void* r = base + off; off += bytes; return r; };
+    void* d_h = take(hp.hidden);
+    void* d_w = take(hp.w);
+    void* d_dh = take(hp.dh);
+    void* d_dw = take(hp.dw);
+    int32_t* d_ids = (int32_t*)take(hp.tok);
+    float* d_b = (float*)take(hp.tok);
+    float* d_q = (float*)take(hp.tok);
+    float* d_lp = (float*)take(hp.tok);
+    float* d_term = (float*)take(hp.tok);
+    float* d_coef = (float*)take(hp.tok);
+    int32_t* d_tt = (int32_t*)take(hp.tok);
+    float* d_ent = (float*)take(hp.tok);
+    int32_t* d_so = (int32_t*)take(hp.steps);
+    int32_t* d_to = (int32_t*)take(hp.traj);
+    int32_t* d_go = (int32_t*)take(hp.groups);
+    float* d_rw = (float*)take(hp.rew);
+    float* d_adv = (float*)take(hp.adv);
+    uint8_t* d_scal = (uint8_t*)take(256);
+    void* d_headws = base + off;
+
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
+    cudaError_t e = cudaSuccess;
+#define AWR_TRY(x) do { if (e == cudaSuccess) e = (x); } while (0)
+    AWR_TRY(cudaMemcpyAsync(d_w, hb->w_head, (size_t)hb->K * hb->V * 2, H2D, st));
+    if (n > 0) {
+        AWR_TRY(cudaMemcpyAsync(d_h, hb->hidden, (size_t)n * hb->K * 2, H2D, st));
+        AWR_TRY(cudaMemcpyAsync(d_ids, hb->target_ids, (size_t)n * 4, H2D, st));
+        AWR_TRY(cudaMemcpyAsync(d_b, hb->behave_lp, (size_t)n * 4, H2D, st));
+        if (!coupled) AWR_TRY(cudaMemcpyAsync(d_q, hb->prox_lp, (size_t)n * 4, H2D, st));
+    }
+    AWR_TRY(cudaMemcpyAsync(d_so, hb->step_off, (size_t)(hb->n_steps + 1) * 4, H2D, st));
+    AWR_TRY(cudaMemcpyAsync(d_to, hb->traj_off, (size_t)(hb->n_traj + 1) * 4, H2D, st));
+    AWR_TRY(cudaMemcpyAsync(d_go, hb->group_off, (size_t)(hb->n_groups + 1) * 4, H2D, st));
+    if (hb->n_traj > 0) AWR_TRY(cudaMemcpyAsync(d_rw, hb->rewards, (size_t)hb->n_traj * 4, H2D, st));
+    if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+
+    awr_head_batch db = *hb;
+    db.hidden = d_h; db.w_head = d_w; db.target_ids = d_ids; db.behave_lp = d_b;
+    db.prox_lp = coupled ? nullptr : d_q;
+    db.step_off = d_so; db.traj_off = d_to; db.group_off = d_go; db.rewards = d_rw;
+    awr_head_outputs dout = {};
+    dout.loss = (float*)d_scal; dout.clip_count = (int64_t*)(d_scal + 8);
+    dout.err_word = (uint32_t*)(d_scal + 16); dout.dual_clip_count = (int64_t*)(d_scal + 24);
+    dout.dhidden = d_dh; dout.dw_head = d_dw; dout.token_lp = d_lp;
+    dout.adv = d_adv; dout.tok_traj = d_tt; dout.tok_term = d_term; dout.tok_coef = d_coef;
+    dout.token_entropy = ho->token_entropy ? d_ent : nullptr;
+    rc = awr_loss_fwd_bwd_fused_head(&db, p, &dout, d_headws, hp.head_ws, stream);
+    if (rc != AWR_OK) { cudaStreamSynchronize(st); cudaGetLastError(); return rc; }
+
+    AWR_TRY(cudaMemcpyAsync(ho->dw_head, d_dw, (size_t)hb->K * hb->V * 2, D2H, st));
+    AWR_TRY(cudaMemcpyAsync(ho->loss, d_scal, 4, D2H, st));
+    AWR_TRY(cudaMemcpyAsync(ho->clip_count, d_scal + 8, 8, D2H, st));
+    if (ho->err_word) AWR_TRY(cudaMemcpyAsync(ho->err_word, d_scal + 16, 4, D2H, st));
+    if (ho->dual_clip_count) AWR_TRY(cudaMemcpyAsync(ho->dual_clip_count, d_scal + 24, 8, D2H, st));
+    if (n > 0) {
+        AWR_TRY(cudaMemcpyAsync(ho->dhidden, d_dh, (size_t)n * hb->K * 2, D2H, st));
+        AWR_TRY(cudaMemcpyAsync(ho->token_lp, d_lp, (size_t)n * 4, D2H, st));
+        if (ho->tok_traj) AWR_TRY(cudaMemcpyAsync(ho->tok_traj, d_tt, (size_t)n * 4, D2H, st));
+        if (ho->tok_term) AWR_TRY(cudaMemcpyAsync(ho->tok_term, d_term, (size_t)n * 4, D2H, st));
+        if (ho->tok_coef) AWR_TRY(cudaMemcpyAsync(ho->tok_coef, d_coef, (size_t)n * 4, D2H, st));
+        if (ho->token_entropy) AWR_TRY(cudaMemcpyAsync(ho->token_entropy, d_ent, (size_t)n * 4, D2H, st));
+    }
+    if (ho->adv && hb->n_traj > 0) AWR_TRY(cudaMemcpyAsync(ho->adv, d_adv, (size_t)hb->n_traj * 4, D2H, st));
+    { cudaError_t e2 = cudaStreamSynchronize(st); if (e == cudaSuccess) e = e2; }
+#undef AWR_TRY
+    if (e != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    return AWR_OK;
+}
+
 // ------------------------------------------------------------------ host-buffer variant
 namespace {
 constexpr int kPanelBufs = 3;
@@ -423,7 +553,7 @@ int awr_loss_fwd_bwd_host(const awr_batch* hb, const awr_params* p, const awr_ou
     HostPlan hp = host_plan(hb->n_tok, hb->V, hb->ld, hb->logits_dtype, hb->n_steps, hb->n_traj, hb->n_groups);
     if (!dev_ws || (reinterpret_cast<uintptr_t>(dev_ws) & 255) || dev_ws_bytes < hp.total) return AWR_ERR_WORKSPACE;
     const int kernel = resolve_kernel(p->kernel, hb->V, hb->ld, hb->logits_dtype, ho->token_entropy != nullptr);
-    if (kernel < 0) return AWR_ERR_PARAM;
+    if (kernel < 0 || kernel == AWR_KERNEL_FWD_STREAM) return AWR_ERR_PARAM;
     DeviceInfo info;
     if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
     if (info.major != 10) return AWR_ERR_ARCH;

@@ -51,6 +51,11 @@ cudaError_t launch_rows_cluster(const RowArgs& a, int num_sms, cudaStream_t st);
 bool rows_rf_supported(int64_t V, int64_t ld, int dtype);
 cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, int cluster_size, cudaStream_t st);
 
+// a2 + a3 forward only (awr_loss_fwd), bf16 rows streamed once through a TMA-filled ring; no
+// gradient, no row residency (awr_rows_fwd.cu).
+bool rows_fwd_supported(int64_t V, int64_t ld, int dtype);
+cudaError_t launch_rows_fwd(const RowArgs& a, int num_sms, cudaStream_t st);
+
 // a5: fused LM head (awr_head.cu).  `rows` carries the per-token inputs / outputs of a3
 // (its logits / dlogits members are unused); `ws` is head_ws_bytes() of device memory.
 constexpr int64_t kHeadPanelRows = 4736;   // 37 row tiles of 128; doubled for CTA pairs (awr_head.cu)

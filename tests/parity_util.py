@@ -29,18 +29,22 @@ from oracle import awr_oracle as O
 LP_ATOL = 1e-4
 LOSS_RTOL = 1e-5
 LOSS_COND_FLOOR = 1e-6
+LOSS_COND_MIN = 100.0  # the floor applies only to sums at least this ill-conditioned
 LOSS_LOG = []          # (label, |loss|, cond, |diff|, rel-only tolerance, passed on the rel term alone)
 
 
 def check_loss(got, ora_loss, ora_term, label=""):
     """north_star: 1e-5 relative.  DESIGN.md section 3 adds the conditioning floor
-    1e-6 sum|term_t| for batches whose advantages cancel (P3: config 0 at ratio 1 sums to 0)."""
+    1e-6 sum|term_t| ONLY for batches whose advantages cancel almost exactly - conditioning
+    sum|term| / |sum term| >= 100 (P3: config 0 at ratio 1 sums to 0 exactly; config 0 as drawn
+    has conditioning 1,238).  Measured over the 156 loss comparisons of the GPU suite (round 2):
+    151 pass on the 1e-5 term alone; the 5 that need the floor have conditioning 570 ... 3.8e9."""
     abs_sum = float(np.abs(ora_term).sum())
     diff = abs(float(got) - float(ora_loss))
     rel_tol = LOSS_RTOL * abs(float(ora_loss))
     cond = abs_sum / abs(float(ora_loss)) if ora_loss != 0 else float("inf")
     LOSS_LOG.append((label, abs(float(ora_loss)), cond, diff, rel_tol, diff <= rel_tol))
-    tol = rel_tol + LOSS_COND_FLOOR * abs_sum
+    tol = rel_tol + (LOSS_COND_FLOOR * abs_sum if cond >= LOSS_COND_MIN else 0.0)
     assert diff <= tol + 1e-30, "loss %r vs oracle %r (tol %g, conditioning %g)" % (
         float(got), float(ora_loss), tol, cond)
 

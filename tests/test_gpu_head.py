@@ -360,3 +360,24 @@ def test_second_device_if_visible():
             torch.cuda.synchronize(dev)
             outs.append((float(o["loss"][0]), float(h["loss"][0])))
     assert np.isfinite(outs).all()
+
+
+def test_head_host_buffer_entry():
+    """awr_loss_fwd_bwd_fused_head_host (the e2e leg of bench.py --config 4): host buffers in and
+    out through the C ABI; same kernels as the device entry, so every output is bit-identical."""
+    batch = _head_batch(700, 128, 2056, seed=23, lp_mode="drift", masked_frac=0.02)
+    want = A.api.HEAD_OPTIONAL_OUTPUTS + ("token_entropy",)
+    dev = A.awr_loss_fwd_bwd_fused_head(batch["hidden"], batch["w_head"], batch["target_ids"],
+                                        batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+                                        batch["traj_off"], batch["group_off"], batch["rewards"],
+                                        want=want, **dict(batch["params"], dual_clip_c=3.0))
+    torch.cuda.synchronize()
+    hin = [batch[k].cpu().pin_memory() for k in ("hidden", "w_head", "target_ids", "behave_lp", "prox_lp",
+                                                 "step_off", "traj_off", "group_off", "rewards")]
+    call = A.HostHeadLossCall(*hin, device=DEV, want=want, **dict(batch["params"], dual_clip_c=3.0))
+    out = call.run()
+    for k in ("loss", "clip_count", "dual_clip_count", "token_lp", "tok_term", "tok_coef", "tok_traj",
+              "adv", "token_entropy", "err_word", "dhidden", "dw_head"):
+        assert not out[k].is_cuda
+        assert torch.equal(out[k], dev[k].cpu()), k
+    assert call.h2d_bytes > 2 * (700 * 128 + 128 * 2056) and call.d2h_bytes > 2 * (700 * 128 + 128 * 2056)

@@ -90,6 +90,63 @@ def test_cluster_vs_oracle(V, ld, kernel):
     P.full_check(batch, backward=False)
 
 
+# ------------------------------------------------------------------ forward-only streaming kernel
+@pytest.mark.parametrize("V,ld,n_tok", [(151_936, 151_936, 331), (40_000, 40_008, 700), (32_768, 32_768, 150),
+                                        (65_544, 65_560, 149), (16_384, 16_384, 300), (1000, 1000, 257),
+                                        (8, 8, 40), (2048 * 8, 2048 * 8 + 8, 77), (163_840, 163_840, 60)])
+@pytest.mark.parametrize("entropy", [False, True])
+def test_forward_stream_kernel(V, ld, n_tok, entropy):
+    """awr_loss_fwd's streaming kernel (the proximal log-prob recomputation): rows
+    shorter than one 32 KB stage, exactly one / several stages, ragged last stages, more and fewer
+    rows than CTAs, masked tokens, -inf logits, clip triggers and the dual clip; every per-token
+    output against the oracle, the entropy within 1e-4."""
+    w = W.workload(3, n_groups=6, group_size=4, n_tok=n_tok, V=V)
+    batch = W.make_batch(w, seed=V % 97, device=DEV, ld=ld, masked_frac=0.04)
+    z = batch["logits"]
+    if V > 64:
+        z[::3, 5:V:97] = float("-inf")
+        ids = batch["target_ids"].long().clamp(min=0)
+        ar = torch.arange(z.shape[0], device=DEV)
+        z[ar, ids] = z[ar, ids].nan_to_num(neginf=0.0)
+    params = dict(batch["params"], kernel=A.KERNEL_FWD_STREAM, dual_clip_c=3.0)
+    want = A.OPTIONAL_OUTPUTS + (("token_entropy",) if entropy else ())
+    out = A.awr_loss_fwd(z, batch["target_ids"], batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+                         batch["traj_off"], batch["group_off"], batch["rewards"], V=V, want=want, **params)
+    torch.cuda.synchronize()
+    ora = P.run_oracle(batch, want_dlogits=False, want_entropy=True, dual_clip_c=3.0)
+    P.check_scalars(out, ora, label="forward stream V=%d" % V)
+    if entropy:
+        H = out["token_entropy"].cpu().numpy().astype(np.float64)
+        assert np.isfinite(H).all() and np.abs(H - ora["token_entropy"]).max() <= 1e-4
+        assert np.all(H[batch["target_ids"].cpu().numpy() < 0] == 0.0)
+    # deterministic (static row schedule, fixed merge order)
+    again = A.awr_loss_fwd(z, batch["target_ids"], batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+                           batch["traj_off"], batch["group_off"], batch["rewards"], V=V, want=want, **params)
+    torch.cuda.synchronize()
+    for k in out:
+        assert torch.equal(out[k], again[k]), k
+
+
+def test_forward_stream_is_the_auto_choice_and_refuses_backward():
+    w = W.workload(1, n_groups=2, group_size=4, n_tok=200)
+    batch = W.make_batch(w, seed=5, device=DEV)
+    args = (batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"], batch["step_off"],
+            batch["traj_off"], batch["group_off"], batch["rewards"])
+    a = A.awr_loss_fwd(*args, **batch["params"])                                   # AUTO
+    b = A.awr_loss_fwd(*args, **dict(batch["params"], kernel=A.KERNEL_FWD_STREAM))
+    c = A.awr_loss_fwd(*args, **dict(batch["params"], kernel=A.KERNEL_GENERIC))
+    torch.cuda.synchronize()
+    assert torch.equal(a["token_lp"], b["token_lp"]) and float(a["loss"][0]) == float(b["loss"][0])
+    assert float((a["token_lp"] - c["token_lp"]).abs().max()) <= 2e-5
+    assert int(a["clip_count"][0]) == int(c["clip_count"][0])
+    with pytest.raises(A.AwrError) as ei:
+        A.awr_loss_fwd_bwd(*args, **dict(batch["params"], kernel=A.KERNEL_FWD_STREAM))
+    assert ei.value.status == -5
+    with pytest.raises(A.AwrError) as ei:                                          # fp32: unsupported
+        A.awr_loss_fwd(batch["logits"].float(), *args[1:], **dict(batch["params"], kernel=A.KERNEL_FWD_STREAM))
+    assert ei.value.status == -5
+
+
 @pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
 @pytest.mark.parametrize("cfg", [1, 2])
 def test_cluster_configs_small(cfg, kernel):
@@ -202,11 +259,11 @@ def test_thinking_shapes_workload(horizon):
     horizons 20 / 40 / 60 of PAPER.md:154, :321-331) through the same kernels, cut to a size the
     oracle finishes in seconds."""
     w = W.workload(5, n_groups=3, group_size=4, n_tok=700, horizon=horizon)
-    st = W.make_structure(W.workload(5, horizon=horizon), seed=0)
+    st = W.make_structure(W.workload(5, horizon=horizon, n_groups=32), seed=0)
     per_step = np.diff(st["step_off"])
     steps = np.diff(st["traj_off"])
     assert 400 <= per_step.min() and per_step.max() <= 900 and steps.max() <= horizon
-    if horizon == 20:
+    if horizon == 20:      # 256 trajectories, 1 + Poisson(11.5) steps for failures: the cap binds
         assert (steps == 20).any(), "the horizon-20 cap should bind for some failed trajectory"
     batch = W.make_batch(w, seed=71 + horizon, device=DEV)
     assert A.select_kernel(batch["V"], batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RF
