@@ -45,7 +45,7 @@ if ROOT not in sys.path:
 
 METRIC = "loss+grad tokens/s at V=151,936 bf16"
 UNIT = "tokens/s"
-CPU_ROWS_PER_CORE = 192    # rows of the bounded oracle sample per host core (about 10-20 s of work)
+CPU_ROWS_PER_CORE = 512    # rows of the bounded oracle sample per host core (a few seconds of work on
 CPU_MAX_ROWS = 24576       # ... capped (the sample batch lives in host memory: 3.7 GB of bf16 values
                            # widened to fp32 at the cap)
 CPU_1T_ROWS = 1024         # rows of the 1-thread figure

@@ -93,7 +93,7 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     16K <= V <= 163,840); shared memory is a TMA load FIFO */
        AWR_KERNEL_CLUSTER_RF4 = 4, /* the same with a row quarter per CTA of a 4-CTA cluster and
                                     two CTAs (of different rows) resident per SM */
-       /* fused-head entry points only (AUTO = AWR_KERNEL_HEAD_2CTA_STORED): */
+       /* fused-head entry points only (AUTO = AWR_KERNEL_HEAD_2CTA_E16): */
        AWR_KERNEL_HEAD_1CTA = 5, /* tcgen05 cta_group::1, 128 x 256 tiles, one CTA per SM; the
                                     logits tile is recomputed for the backward (8 K V flops/token) */
        AWR_KERNEL_HEAD_2CTA = 6, /* tcgen05 cta_group::2, 256 x 256 tiles on CTA pairs; recompute */
@@ -101,9 +101,13 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     rows, workspace) are kept between the forward GEMM and a
                                     streaming dS pass: 6 K V flops/token, same bits as recompute */
        /* awr_loss_fwd only (its AUTO choice for bf16 rows of >= 64 KB): */
-       AWR_KERNEL_FWD_STREAM = 8 /* forward-only streaming kernel: whole rows through a ring of TMA
+       AWR_KERNEL_FWD_STREAM = 8, /* forward-only streaming kernel: whole rows through a ring of TMA
                                     bulk copies, one persistent CTA per SM, no row residency (bf16,
-                                    V and ld multiples of 8); with awr_loss_fwd_bwd -> AWR_ERR_PARAM */ };
+                                    V and ld multiples of 8); with awr_loss_fwd_bwd -> AWR_ERR_PARAM */
+       AWR_KERNEL_HEAD_2CTA_E16 = 9 /* fused head, CTA pairs: the forward epilogue leaves E = bf16(exp(z -
+                                    tile row max)) of ONE row panel (<= 9,472 rows) in the dS buffer and one
+                                    in-place pass rescales it to dS: 6 K V flops/token, 2 bytes of
+                                    transient per logit of the panel, no side stream */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u };
 
@@ -242,8 +246,10 @@ typedef struct awr_head_outputs {
 AWR_API int awr_loss_fwd_bwd_fused_head(const awr_head_batch* batch, const awr_params* params,
                                 const awr_head_outputs* out, void* workspace,
                                 size_t workspace_bytes, void* stream);
+/* Workspace of the fused head for `kernel` (an AWR_KERNEL_HEAD_* id or AUTO); the modes differ:
+ * config 4 (32,768 x 2048 x 151,936) needs 4.4 GB with E16 (AUTO), 15.9 GB with HEAD_2CTA_STORED. */
 AWR_API size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
-                                int32_t n_traj, int32_t n_groups);
+                                int32_t n_traj, int32_t n_groups, int32_t kernel);
 
 /* a5 with HOST buffers (the `e2e` leg of bench.py --config 4): every pointer in `host_batch` and
  * `host_out` is a host pointer (pinned memory gives full PCIe speed).  hidden, w_head and the
@@ -254,7 +260,7 @@ AWR_API int awr_loss_fwd_bwd_fused_head_host(const awr_head_batch* host_batch, c
                                      const awr_head_outputs* host_out, void* dev_workspace,
                                      size_t dev_workspace_bytes, void* stream);
 AWR_API size_t awr_head_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
-                                     int32_t n_traj, int32_t n_groups);
+                                     int32_t n_traj, int32_t n_groups, int32_t kernel);
 
 /* Note: in the stored-logits mode the call forks the dS pass of each row panel onto a library-owned
  * side stream (created once per device) and joins it back before the panel's dhidden GEMM; from

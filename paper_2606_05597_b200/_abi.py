@@ -26,6 +26,7 @@ W_K_BY_V, W_V_BY_K = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_CLUSTER, KERNEL_CLUSTER_RF, KERNEL_CLUSTER_RF4 = 0, 1, 2, 3, 4
 KERNEL_HEAD_1CTA, KERNEL_HEAD_2CTA, KERNEL_HEAD_2CTA_STORED = 5, 6, 7
 KERNEL_FWD_STREAM = 8
+KERNEL_HEAD_2CTA_E16 = 9
 ERRBIT_STEP_OFF, ERRBIT_TRAJ_OFF, ERRBIT_GROUP_OFF, ERRBIT_TARGET_RANGE = 1, 2, 4, 8
 
 _vp = C.c_void_p
@@ -83,11 +84,11 @@ SYMBOLS = {
     "awr_loss_fwd_bwd_fused_head": (C.c_int, [C.POINTER(awr_head_batch), C.POINTER(awr_params),
                                               C.POINTER(awr_head_outputs), _vp, C.c_size_t, _vp]),
     "awr_head_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int64, C.c_int64, C.c_int32,
-                                              C.c_int32, C.c_int32]),
+                                              C.c_int32, C.c_int32, C.c_int32]),
     "awr_loss_fwd_bwd_fused_head_host": (C.c_int, [C.POINTER(awr_head_batch), C.POINTER(awr_params),
                                                    C.POINTER(awr_head_outputs), _vp, C.c_size_t, _vp]),
     "awr_head_host_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int64, C.c_int64, C.c_int32,
-                                                   C.c_int32, C.c_int32]),
+                                                   C.c_int32, C.c_int32, C.c_int32]),
     "awr_head_launches_per_call": (C.c_int, [C.c_int64, C.c_int64, C.c_int64, C.c_int32]),
     "awr_gemm_bf16": (C.c_int, [_vp, C.c_int32, C.c_int64, _vp, C.c_int32, C.c_int64, C.c_int64,
                                 C.c_int64, C.c_int64, _vp, C.c_int64, C.c_int32, _vp]),

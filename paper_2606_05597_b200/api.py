@@ -261,8 +261,8 @@ def awr_loss_fwd_bwd_host(logits, target_ids, behave_lp, prox_lp, step_off, traj
 HEAD_OPTIONAL_OUTPUTS = ("adv", "tok_traj", "tok_term", "tok_coef", "err_word")
 
 
-def head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups) -> int:
-    return int(load().awr_head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups))
+def head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups, kernel=KERNEL_AUTO) -> int:
+    return int(load().awr_head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups, int(kernel)))
 
 
 def head_launches_per_call(n_tok, V, K, kernel=KERNEL_AUTO) -> int:
@@ -324,7 +324,7 @@ class HeadLossCall:
                                      _ptr(g("tok_traj")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
                                      _ptr(g("err_word")), _ptr(g("dual_clip_count")),
                                      _ptr(g("token_entropy")))
-        need = head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups)
+        need = head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups, self.params.kernel)
         self.workspace = workspace if workspace is not None else torch.empty(
             max(need, 256), dtype=torch.uint8, device=dev)
         self.ws_bytes = self.workspace.numel()
@@ -347,8 +347,8 @@ def awr_loss_fwd_bwd_fused_head(hidden, w_head, target_ids, behave_lp, prox_lp, 
                         group_off, rewards, **kw).run(stream)
 
 
-def head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups) -> int:
-    return int(load().awr_head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups))
+def head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups, kernel=KERNEL_AUTO) -> int:
+    return int(load().awr_head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups, int(kernel)))
 
 
 class HostHeadLossCall:
@@ -393,7 +393,7 @@ class HostHeadLossCall:
                                      _ptr(g("tok_traj")), _ptr(g("tok_term")), _ptr(g("tok_coef")),
                                      _ptr(g("err_word")), _ptr(g("dual_clip_count")),
                                      _ptr(g("token_entropy")))
-        need = head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups)
+        need = head_host_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups, self.params.kernel)
         if workspace is not None and workspace.numel() >= need:
             self.workspace = workspace
         else:

@@ -68,7 +68,7 @@ static int check_params(const awr_params* p) {
     if (p->flags & ~(uint32_t)(AWR_FLAG_SAMPLE_STD | AWR_FLAG_SUCCESS_FILTER | AWR_FLAG_COUPLED |
                                AWR_FLAG_SKIP_UNIFORM))
         return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_FWD_STREAM) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_E16) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -81,12 +81,13 @@ static int check_segments(int64_t n_tok, int32_t n_steps, int32_t n_traj, int32_
 // fused-head entry points: which tcgen05 shape (CTAs per tile) a kernel request means, or -1
 static int resolve_head_ctas(int requested) {
     if (requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA ||
-        requested == AWR_KERNEL_HEAD_2CTA_STORED) return 2;
+        requested == AWR_KERNEL_HEAD_2CTA_STORED || requested == AWR_KERNEL_HEAD_2CTA_E16) return 2;
     if (requested == AWR_KERNEL_HEAD_1CTA) return 1;
     return -1;
 }
-static int resolve_head_stored(int requested) {
-    return requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA_STORED;
+static int resolve_head_mode(int requested) {
+    if (requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA_E16) return kHeadE16;
+    return requested == AWR_KERNEL_HEAD_2CTA_STORED ? kHeadStored32 : kHeadRecompute;
 }
 
 static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool want_entropy = false,
@@ -265,16 +266,17 @@ int awr_group_advantage(const float* rewards, const int32_t* group_off, int32_t 
 
 // ------------------------------------------------------------------ a5: fused LM head
 size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
-                                int32_t n_traj, int32_t n_groups) {
+                                int32_t n_traj, int32_t n_groups, int32_t kernel) {
     (void)n_steps; (void)n_groups;
-    if (n_tok < 0 || n_traj < 0 || V <= 0 || K <= 0) return 0;
-    return carve(nullptr, n_tok, n_traj).total + head_ws_bytes(n_tok, V, K);
+    if (n_tok < 0 || n_traj < 0 || V <= 0 || K <= 0 || resolve_head_ctas(kernel) < 0) return 0;
+    return carve(nullptr, n_tok, n_traj).total +
+           head_ws_bytes(n_tok, V, K, resolve_head_ctas(kernel), resolve_head_mode(kernel));
 }
 
 int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K, int32_t kernel) {
     const int ctas = resolve_head_ctas(kernel);
     if (ctas < 0) return AWR_ERR_PARAM;
-    return 3 + head_launches(n_tok, V, K, ctas, resolve_head_stored(kernel));     // a0, a1, [F, scalars, 3 per panel], final sum
+    return 3 + head_launches(n_tok, V, K, ctas, resolve_head_mode(kernel));     // a0, a1, [F, scalars, 3 per panel], final sum
 }
 
 int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
@@ -298,7 +300,8 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     if ((reinterpret_cast<uintptr_t>(b->hidden) & 15) || (reinterpret_cast<uintptr_t>(b->w_head) & 15) ||
         (reinterpret_cast<uintptr_t>(o->dhidden) & 15) || (reinterpret_cast<uintptr_t>(o->dw_head) & 15))
         return AWR_ERR_ALIGN;
-    const size_t need = awr_head_workspace_bytes(b->n_tok, b->V, b->K, b->n_steps, b->n_traj, b->n_groups);
+    const size_t need = awr_head_workspace_bytes(b->n_tok, b->V, b->K, b->n_steps, b->n_traj, b->n_groups,
+                                                 p->kernel);
     if (!ws_ptr || (reinterpret_cast<uintptr_t>(ws_ptr) & 255) || ws_bytes < need) return AWR_ERR_WORKSPACE;
     DeviceInfo info;
     if (device_info(info) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
@@ -336,7 +339,7 @@ int awr_loss_fwd_bwd_fused_head(const awr_head_batch* b, const awr_params* p,
     c.dhidden = o->dhidden; c.dw_head = o->dw_head;
     c.ws = reinterpret_cast<uint8_t*>(ws_ptr) + w.total;
     c.ctas = resolve_head_ctas(p->kernel);
-    c.store_logits = resolve_head_stored(p->kernel);
+    c.mode = resolve_head_mode(p->kernel);
     if (e == cudaSuccess) e = launch_head(c, info.num_sms, st);
     if (e == cudaSuccess) e = launch_final_reduce(tok_term, w.tok_flag, b->n_tok, o->loss, o->clip_count,
                                                     o->dual_clip_count, st);
@@ -370,7 +373,7 @@ struct HeadHostPlan {
     size_t hidden, w, dh, dw, tok, steps, traj, groups, rew, adv, total_small, head_ws, total;
 };
 HeadHostPlan head_host_plan(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps, int32_t n_traj,
-                            int32_t n_groups) {
+                            int32_t n_groups, int32_t kernel) {
     HeadHostPlan h;
     h.hidden = align_up((size_t)n_tok * K * 2, 256);
     h.w = align_up((size_t)K * V * 2, 256);
@@ -384,16 +387,17 @@ HeadHostPlan head_host_plan(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps
     h.adv = h.rew;
     // ids, b, q in; lp, term, coef, tok_traj, entropy out; offsets; rewards; adv; scalars
     h.total_small = 8 * h.tok + h.steps + h.traj + h.groups + h.rew + h.adv + 256;
-    h.head_ws = awr_head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups);
+    h.head_ws = awr_head_workspace_bytes(n_tok, V, K, n_steps, n_traj, n_groups, kernel);
     h.total = h.hidden + h.w + h.dh + h.dw + h.total_small + h.head_ws;
     return h;
 }
 }  // namespace
 
 size_t awr_head_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
-                                     int32_t n_traj, int32_t n_groups) {
+                                     int32_t n_traj, int32_t n_groups, int32_t kernel) {
     if (n_tok < 0 || V <= 0 || K <= 0 || n_steps < 0 || n_traj < 0 || n_groups < 0) return 0;
-    return head_host_plan(n_tok, V, K, n_steps, n_traj, n_groups).total;
+    if (resolve_head_ctas(kernel) < 0) return 0;
+    return head_host_plan(n_tok, V, K, n_steps, n_traj, n_groups, kernel).total;
 }
 
 int awr_loss_fwd_bwd_fused_head_host(const awr_head_batch* hb, const awr_params* p,
@@ -412,7 +416,9 @@ int awr_loss_fwd_bwd_fused_head_host(const awr_head_batch* hb, const awr_params*
     if (hb->n_tok > 0 && (!hb->hidden || !hb->target_ids || !hb->behave_lp || (!coupled && !hb->prox_lp)))
         return AWR_ERR_NULL;
     if (hb->n_traj > 0 && !hb->rewards) return AWR_ERR_NULL;
-    const HeadHostPlan hp = head_host_plan(hb->n_tok, hb->V, hb->K, hb->n_steps, hb->n_traj, hb->n_groups);
+    if (resolve_head_ctas(p->kernel) < 0) return AWR_ERR_PARAM;
+    const HeadHostPlan hp = head_host_plan(hb->n_tok, hb->V, hb->K, hb->n_steps, hb->n_traj, hb->n_groups,
+                                           p->kernel);
     if (!dev_ws || (reinterpret_cast<uintptr_t>(dev_ws) & 255) || dev_ws_bytes < hp.total) return AWR_ERR_WORKSPACE;
 
     const int64_t n = hb->n_tok;

@@ -281,6 +281,90 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                     if (want_ent) g.e.partz[(int64_t)n_blk * g.e.part_ld + row] = sz;
                     if (y_here) g.e.zy[row] = zy;
                 }
+            } else if constexpr (EPI == kEpiLse16) {
+                // The tile is kept as E = bf16(exp(z - m)), m = this row's max over the tile (target
+                // left out): 2 bytes per logit instead of 4, and the same exponentials feed the
+                // log-sum-exp partial (unrounded).  Pass A takes the max, pass B the rest.
+                const int y = row_ok ? g.e.target_ids[row] : -1;
+                const bool want_ent = g.e.partz != nullptr;
+                const bool y_here = (y >= n0) && (y < n0 + kTN) && (y < g.N);
+                float m = -INFINITY, zy = 0.f;
+                auto mask = [&](int c, float (&v)[32]) {      // columns >= N and the target -> -inf
+                    const int c0 = n0 + c * 32;
+                    if (c0 + 32 > g.N) {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) if (c0 + j >= g.N) v[j] = -INFINITY;
+                    }
+                    if (y_here && y >= c0 && y < c0 + 32) {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) if (c0 + j == y) { zy = v[j]; v[j] = -INFINITY; }
+                    }
+                };
+                float vb[32];
+                tmem_ld32_issue(t_addr, v);
+#pragma unroll 1
+                for (int c = 0; c < kTN / 32; c += 2) {
+                    tmem_ld_wait(v);
+                    tmem_ld32_issue(t_addr + (c + 1) * 32, vb);
+                    mask(c, v);
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) m = fmaxf(m, v[j]);
+                    tmem_ld_wait(vb);
+                    if (c + 2 < kTN / 32) tmem_ld32_issue(t_addr + (c + 2) * 32, v);
+                    mask(c + 1, vb);
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) m = fmaxf(m, vb[j]);
+                }
+                const float nref = (m == -INFINITY) ? 0.f : -m * kLog2e;
+                float s = 0.f, sz = 0.f;
+                uint32_t* stg = reinterpret_cast<uint32_t*>(zstage) + q * (32 * kZStageLd);
+                const int row_w = row - lane;                 // tile row of this warp's TMEM lane 0
+                auto expchunk = [&](int c, float (&v)[32], int half) {
+                    mask(c, v);
+                    float acc = 0.f, accz = 0.f;
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const float z = v[j];
+                        v[j] = ex2_approx(fmaf(z, kLog2e, nref));
+                        acc += v[j];
+                        if (want_ent) accz = fmaf(v[j], fmaxf(z, kZFloor), accz);
+                    }
+                    s += acc;
+                    sz += accz;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        *reinterpret_cast<uint4*>(stg + lane * kZStageLd + half * 16 + 4 * j) = make_uint4(
+                            pack_bf16x2(v[8 * j], v[8 * j + 1]), pack_bf16x2(v[8 * j + 2], v[8 * j + 3]),
+                            pack_bf16x2(v[8 * j + 4], v[8 * j + 5]), pack_bf16x2(v[8 * j + 6], v[8 * j + 7]));
+                };
+                tmem_ld32_issue(t_addr, v);
+#pragma unroll 1
+                for (int c = 0; c < kTN / 32; c += 2) {
+                    tmem_ld_wait(v);
+                    tmem_ld32_issue(t_addr + (c + 1) * 32, vb);
+                    expchunk(c, v, 0);
+                    tmem_ld_wait(vb);
+                    if (c + 2 < kTN / 32) tmem_ld32_issue(t_addr + (c + 2) * 32, v);
+                    expchunk(c + 1, vb, 1);
+                    __syncwarp();
+                    // 64 columns of 32 rows are staged: every store instruction writes 4 whole
+                    // 128-byte row segments
+                    const int c0 = n0 + c * 32;
+                    const int cc = (lane & 7) * 8;            // bf16 column inside the 64
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int r = i * 4 + (lane >> 3);
+                        const uint4 t = *reinterpret_cast<const uint4*>(stg + r * kZStageLd + (lane & 7) * 4);
+                        if (row_w + r < g.M && c0 + cc < g.N)
+                            *reinterpret_cast<uint4*>(g.e.eout + (int64_t)(row_w + r) * g.e.eout_ld + c0 + cc) = t;
+                    }
+                    __syncwarp();
+                }
+                if (row_ok) {
+                    g.e.part[(int64_t)n_blk * g.e.part_ld + row] = make_float2(m, s);
+                    if (want_ent) g.e.partz[(int64_t)n_blk * g.e.part_ld + row] = sz;
+                    if (y_here) g.e.zy[row] = zy;
+                }
             } else if constexpr (EPI == kEpiDs) {
                 int y = -1;
                 float lse = 0.f, coef = 0.f, gy = 0.f;
@@ -473,6 +557,46 @@ head_ds_kernel(const float* __restrict__ z, int64_t z_ld, int64_t rows, int64_t 
     }
 }
 
+// a4 for the E16 mode: the panel holds E = bf16(exp(z - m_j)), m_j the row's max over column tile
+// j (the .x of the forward partials).  In place: dS = bf16(E c_t exp(m_j - lse)); the target entry
+// becomes c_t (p_y - 1); rows with c_t = 0 are written as zeros without a read.  HBM-bound:
+// 2 B read + 2 B written per element.
+__global__ void __launch_bounds__(512)
+head_ds16_kernel(__nv_bfloat16* __restrict__ e, int64_t ld, int64_t rows, int64_t V,
+                 const int32_t* __restrict__ target_ids, const float2* __restrict__ part,
+                 int64_t part_ld, const float* __restrict__ row_lse, const float* __restrict__ row_coef,
+                 const float* __restrict__ row_gy) {
+    const int units = (int)(V >> 3);                    // V is a multiple of 8
+    constexpr int kUnitsPerTile = kBN / 8;
+    for (int64_t row = blockIdx.x; row < rows; row += gridDim.x) {
+        const float coef = row_coef[row];
+        uint4* p = reinterpret_cast<uint4*>(e + row * ld);
+        if (coef == 0.f) {
+            for (int i = threadIdx.x; i < units; i += blockDim.x) p[i] = make_uint4(0u, 0u, 0u, 0u);
+            continue;
+        }
+        const int y = target_ids[row];
+        const float gy = row_gy[row];
+        const float nlse = -row_lse[row] * kLog2e;
+#pragma unroll 4
+        for (int i = threadIdx.x; i < units; i += blockDim.x) {
+            const float mj = part[(int64_t)(i / kUnitsPerTile) * part_ld + row].x;
+            const float gj = (mj == -INFINITY) ? 0.f : coef * ex2_approx(fmaf(mj, kLog2e, nlse));
+            const uint4 a = p[i];
+            float v[8] = {bf16_lo(a.x), bf16_hi(a.x), bf16_lo(a.y), bf16_hi(a.y),
+                          bf16_lo(a.z), bf16_hi(a.z), bf16_lo(a.w), bf16_hi(a.w)};
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] *= gj;
+            if ((y >> 3) == i && y >= 0) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) v[k] = (k == (y & 7)) ? gy : v[k];
+            }
+            p[i] = make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]),
+                              pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
+        }
+    }
+}
+
 // ================================================================== host side
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
@@ -596,6 +720,7 @@ static cudaError_t launch_gemm(int epi, const OperandView& A, const OperandView&
     if (nt == 2) return launch_gemm_epi<kEpiStoreBf16, 2, 2>(ta, tb, g, grid, st);
     switch (epi) {
         AWR_HEAD_CASE(kEpiLse) AWR_HEAD_CASE(kEpiDs) AWR_HEAD_CASE(kEpiStoreBf16) AWR_HEAD_CASE(kEpiAccum)
+        AWR_HEAD_CASE(kEpiLse16)
         default: return cudaErrorInvalidValue;
     }
 #undef AWR_HEAD_CASE
@@ -701,8 +826,9 @@ struct HeadWs {
 // 37 x 8 = 296 tiles = 2 x 148 CTAs (ctas = 1) or 4 x 74 CTA pairs (ctas = 2).
 static int64_t head_panel_rows(int ctas) { return ctas == 2 ? 2 * kHeadPanelRows : kHeadPanelRows; }
 
-static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ctas, bool store_z,
+static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ctas, int mode,
                          bool entropy = true) {
+    const bool store_z = mode == kHeadStored32;
     HeadWs w;
     uint8_t* p = reinterpret_cast<uint8_t*>(base);
     size_t off = 0;
@@ -728,10 +854,8 @@ static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ct
     return w;
 }
 
-size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K) {
-    const size_t a = head_carve(nullptr, n_tok, V, K, 1, false).total;
-    const size_t b = head_carve(nullptr, n_tok, V, K, 2, true).total;
-    return a > b ? a : b;
+size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode) {
+    return head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2, mode).total;
 }
 
 cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
@@ -741,8 +865,9 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     }
     const int ctas = c.ctas == 1 ? 1 : 2;
     const int gm = 4096 / (kBM * ctas);               // raster groups of 4096 rows
-    const bool store_z = c.store_logits != 0;
-    const HeadWs w = head_carve(c.ws, c.n_tok, c.V, c.K, ctas, store_z);
+    const bool store_z = c.mode == kHeadStored32;
+    const bool e16 = c.mode == kHeadE16;
+    const HeadWs w = head_carve(c.ws, c.n_tok, c.V, c.K, ctas, c.mode);
     const bool kv = c.w_layout == AWR_W_K_BY_V;
     const __nv_bfloat16* H = reinterpret_cast<const __nv_bfloat16*>(c.hidden);
     // W as the B operand of Z = H W (n = v, contraction = k) and of dH = dS W^T (n = k, contraction = v)
@@ -755,6 +880,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     // Partials / gathered logits are indexed by global row (pointers pre-offset by r0).
     auto forward = [&](int64_t r0, int64_t rows, float* zout) -> cudaError_t {
         EpiArgs ea = {};
+        ea.eout = e16 ? w.ds : nullptr; ea.eout_ld = w.ds_ld;
         ea.part = w.part + r0; ea.part_ld = w.part_ld; ea.zy = w.zy + r0;
         ea.partz = c.rows->token_entropy ? w.partz + r0 : nullptr;
         ea.target_ids = c.rows->target_ids + r0;
@@ -762,8 +888,8 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         // raster: when the H rows of this call fit in L2 (a panel: 39 MB at K = 2048) walk all of
         // its row tiles before the next W column tile, so W_head streams from HBM exactly once
         const int fgm = rows * c.K * 2 <= (48ll << 20) ? (int)((rows + kBM * ctas - 1) / (kBM * ctas)) : gm;
-        cudaError_t err = launch_gemm(kEpiLse, OperandView{H + r0 * c.K, rows, c.K, c.K, kMajorK}, w_fwd,
-                                      0, fgm, ea, num_sms, ctas, st);
+        cudaError_t err = launch_gemm(e16 ? kEpiLse16 : kEpiLse, OperandView{H + r0 * c.K, rows, c.K, c.K, kMajorK},
+                                      w_fwd, 0, fgm, ea, num_sms, ctas, st);
         if (err != cudaSuccess) return err;
         const int warps = 8;
         const unsigned blocks = (unsigned)((rows + warps - 1) / warps);
@@ -773,7 +899,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
                                                            r0, r0 + rows);
         return cudaGetLastError();
     };
-    if (!store_z) {
+    if (c.mode == kHeadRecompute) {
         e = forward(0, c.n_tok, nullptr);
         if (e != cudaSuccess) return e;
     }
@@ -786,7 +912,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     // caller's stream.
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-    SideGuard guard{store_z ? side_acquire(st) : nullptr};
+    SideGuard guard{store_z ? side_acquire(st) : nullptr};       // E16 / recompute: no side stream
     if (guard.s) { side = guard.s->stream; ev_fork = guard.s->fork; ev_join = guard.s->join; }
     float* zbuf[2] = {w.zpanel, w.zpanel2};
     if (store_z && w.n_panels > 0) {
@@ -822,6 +948,16 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
                 if (e != cudaSuccess) return e;
             }
             if (side) e = cudaStreamWaitEvent(st, ev_join, 0);
+        } else if (e16) {
+            // E16 mode: forward GEMM of this panel writes E = bf16(exp(z - tile max)) into the dS
+            // panel; one in-place streaming pass turns it into dS.  One buffer, one stream.
+            e = forward(r0, rows, nullptr);
+            if (e != cudaSuccess) return e;
+            const unsigned blocks = (unsigned)(rows < 4 * (int64_t)num_sms ? rows : 4 * (int64_t)num_sms);
+            head_ds16_kernel<<<blocks, 512, 0, st>>>(w.ds, w.ds_ld, rows, c.V, c.rows->target_ids + r0,
+                                                     w.part + r0, w.part_ld, w.row_lse + r0,
+                                                     w.row_coef + r0, w.row_gy + r0);
+            e = cudaGetLastError();
         } else {
             EpiArgs e1 = {};
             e1.target_ids = c.rows->target_ids + r0; e1.row_lse = w.row_lse + r0;
@@ -854,10 +990,10 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     return cudaSuccess;
 }
 
-int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int store_logits) {
-    const HeadWs w = head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2, store_logits != 0);
-    // recompute: F, scalars, then (dS GEMM, dH, dW) per panel; stored: (F, scalars, dS pass, dH, dW) per panel
-    return store_logits ? 5 * w.n_panels : 2 + 3 * w.n_panels;
+int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode) {
+    const HeadWs w = head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2, mode);
+    // recompute: F, scalars, then (dS GEMM, dH, dW) per panel; stored / E16: (F, scalars, dS pass, dH, dW) per panel
+    return mode != kHeadRecompute ? 5 * w.n_panels : 2 + 3 * w.n_panels;
 }
 
 cudaError_t launch_gemm_bf16(const void* A, int a_major, int64_t lda, const void* B, int b_major,

@@ -75,11 +75,12 @@ constexpr int kZStageBytes = 4 * 32 * kZStageLd * 4;            // 4 epilogue wa
 template <int EPI, int CTAS, int NT>
 struct EpiGeo {
     using G = Geo<CTAS, NT>;
-    static constexpr bool kStaged = EPI == 0;                   // kEpiLse
+    static constexpr bool kStaged = EPI == 0 || EPI == 4;       // kEpiLse, kEpiLse16
     static constexpr int kStages = (kStaged && CTAS == 2 && NT == 1) ? G::kStages - 1 : G::kStages;
     static constexpr int kSmemBytes = kStages * G::kStageBytes + 1024 + 256 + (kStaged ? kZStageBytes : 0);
 };
 static_assert(EpiGeo<0, 2, 1>::kSmemBytes <= 232448 && EpiGeo<0, 1, 1>::kSmemBytes <= 232448, "shared memory");
+static_assert(EpiGeo<4, 2, 1>::kSmemBytes <= 232448 && EpiGeo<4, 1, 1>::kSmemBytes <= 232448, "shared memory");
 static_assert(Geo<2>::kStages <= kMaxStages && Geo<2>::kSmemBytes <= 232448, "shared memory");
 static_assert(Geo<2, 2>::kSmemBytes <= 232448, "shared memory");
 
@@ -87,7 +88,9 @@ enum { kMajorK = 0, kMajorMN = 1 };
 enum { kEpiLse = 0,      // a2 on the tile: per-row (max, sum exp) partials + target gather
        kEpiDs = 1,       // a4 on the tile: dS = c_t (exp(z - lse) - onehot) -> bf16 panel
        kEpiStoreBf16 = 2,// C -> bf16 (dhidden)
-       kEpiAccum = 3 };  // C accumulated over row panels in fp32, bf16 on the last panel (dw_head)
+       kEpiAccum = 3,    // C accumulated over row panels in fp32, bf16 on the last panel (dw_head)
+       kEpiLse16 = 4 };  // kEpiLse that also keeps the tile as E = bf16(exp(z - tile row max)): two
+                         // passes over the accumulator (max, then exp + sum + store)
 
 // How one operand is staged and described to the tensor core (all runtime values).
 struct Operand {
@@ -112,6 +115,8 @@ struct EpiArgs {
     const int32_t* target_ids; // [M] (kEpiLse, kEpiDs), already offset to row 0 of this GEMM
     float* zout;               // optional [M, zout_ld]: the fp32 logits tile, kept for the dS pass
     int64_t zout_ld;
+    __nv_bfloat16* eout;       // kEpiLse16 [M, eout_ld]: E = exp(z - m) with m the (max) of part[]
+    int64_t eout_ld;
     // kEpiDs
     const float* row_lse;      // [M] log-sum-exp of the whole row
     const float* row_coef;     // [M] c_t

@@ -69,11 +69,15 @@ struct HeadCall {
     void* dw_head;
     void* ws;
     int ctas;        // 1: cta_group::1 tiles of 128 rows; anything else: CTA pairs, 256-row tiles
-    int store_logits;  // 0: recompute the logits tile for dS (8 K V flops / token); 1: keep the fp32
-                       // logits of one row panel and form dS in a streaming pass (6 K V)
+    int mode;        // kHead*
 };
-size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K);
-int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int store_logits);
+enum { kHeadRecompute = 0,  // the logits tile is recomputed for dS (8 K V flops / token)
+       kHeadStored32 = 1,   // the fp32 logits of a row panel are kept (two buffers, side stream); dS in
+                            // a streaming pass (6 K V); same bits as recompute
+       kHeadE16 = 2 };      // the forward epilogue keeps E = bf16(exp(z - tile max)) IN the dS panel; one
+                            // in-place pass rescales it to dS (6 K V; 2 bytes per logit of transient)
+size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode);
+int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode);
 cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st);
 // C[M, N] (bf16, row-major, ldc) = A B on the tcgen05 engine; majors: 0 = contraction index
 // contiguous, 1 = row (A) / column (B) index contiguous.

@@ -13,8 +13,9 @@
 // them to registers, takes their max with packed bf16x2 max, rescales its running (max, sum)
 // state ONCE per stage and then issues 32 independent ex2 - one MUFU per logit, the secondary
 // bound of the pass (16 / clk / SM: 1,024 clocks per stage against ~1,400 at the HBM rate).
-// At the end of a row the 16 warps meet at one named barrier; one warp (rotating) merges the 16
-// partial states and evaluates a3 while the others are already consuming the next row.
+// At the end of a row every warp publishes its partial state in a shared-memory slot and goes
+// straight on to the next row; a 17th warp merges the 16 states and evaluates a3 a row behind
+// (mbarrier hand-shakes, no block-wide barrier anywhere in the row loop).
 // Rows are dealt round-robin to CTAs: a static schedule, so results are bit-reproducible.
 #include "awr_common.cuh"
 #include "awr_kernels.h"
@@ -24,12 +25,13 @@ namespace awr {
 
 constexpr int kFwdWarps = 16;                       // consumer warps
 constexpr int kFwdConsumers = kFwdWarps * 32;
-constexpr int kFwdThreads = kFwdConsumers + 32;     // + the producer warp
+constexpr int kFwdThreads = kFwdConsumers + 64;     // + the producer warp + the a3 warp
 constexpr int kFwdRounds = 4;                       // 16-byte units per thread per stage
 constexpr int kFwdStageUnits = kFwdConsumers * kFwdRounds;
 constexpr int kFwdStageBytes = kFwdStageUnits * 16; // 32 KB
 constexpr int kFwdStages = 6;
-constexpr int kFwdCtrlBytes = 1024;
+constexpr int kFwdSlots = 8;                        // per-row state slots in flight (> kFwdStages)
+constexpr int kFwdCtrlBytes = 2048;
 constexpr int kFwdSmemBytes = kFwdCtrlBytes + kFwdStages * kFwdStageBytes;
 constexpr uint32_t kFwdNegInf2 = 0xff80ff80u;       // bf16x2 (-inf, -inf)
 static_assert(kFwdSmemBytes <= 232448, "227 KB of dynamic shared memory per CTA");
@@ -37,11 +39,19 @@ static_assert(kFwdSmemBytes <= 232448, "227 KB of dynamic shared memory per CTA"
 struct FwdCtrl {
     uint64_t full[kFwdStages];
     uint64_t empty[kFwdStages];
-    float2 stats[2][kFwdWarps];      // [row parity][warp] (max, sum) of the warp's share of the row
-    float statz[2][kFwdWarps];       // [row parity][warp] sum e z (entropy output only)
+    uint64_t done[kFwdSlots];                // all 16 consumer warps have published the row's state
+    uint64_t freed[kFwdSlots];               // the a3 warp has read the slot
+    float2 stats[kFwdSlots][kFwdWarps];      // [slot][warp] (max, sum) of the warp's share of the row
+    float statz[kFwdSlots][kFwdWarps];       // [slot][warp] sum e z (entropy output only)
 };
 static_assert(sizeof(FwdCtrl) <= kFwdCtrlBytes, "control block");
 
+// Three roles, no block-wide barrier after the prologue:
+//   warps 0..15  consumers: ring stage -> registers -> (max, sum) state; publish it per row
+//   warp 16      producer: lane 0 issues one 32 KB bulk copy per stage
+//   warp 17      a3: merges the 16 published states of a row and evaluates the token scalars,
+//                with the row's header loads issued a row ahead; consumers never wait for it
+//                (only for a free state slot, 8 rows later)
 template <bool ENT>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 rows_fwd_kernel(RowArgs a, int units_per_row) {
@@ -54,11 +64,14 @@ rows_fwd_kernel(RowArgs a, int units_per_row) {
     const uint32_t ring = smem_u32(smem + kFwdCtrlBytes);
     const uint32_t full0 = smem_u32(&ctrl->full[0]);
     const uint32_t empty0 = smem_u32(&ctrl->empty[0]);
+    const uint32_t done0 = smem_u32(&ctrl->done[0]);
+    const uint32_t freed0 = smem_u32(&ctrl->freed[0]);
     const int nch = (units_per_row + kFwdStageUnits - 1) / kFwdStageUnits;   // stages per row
     const int64_t row_bytes = a.ld * 2;
 
     if (tid == 0) {
         for (int s = 0; s < kFwdStages; ++s) { mbar_init(full0 + 8u * s, 1); mbar_init(empty0 + 8u * s, kFwdWarps); }
+        for (int s = 0; s < kFwdSlots; ++s) { mbar_init(done0 + 8u * s, kFwdWarps); mbar_init(freed0 + 8u * s, 1); }
         fence_mbar_init();
     }
     __syncthreads();
@@ -84,14 +97,55 @@ rows_fwd_kernel(RowArgs a, int units_per_row) {
         return;
     }
 
+    if (warp == kFwdWarps + 1) {
+        // ===================== a3: one warp, a row behind the consumers
+        int slot = 0;
+        uint32_t sphase = 0;
+        RowHeader h, hn;
+        bool valid = false, validn = false;
+        if (lane == 0 && blockIdx.x < a.n_tok) hn = load_row_header(a, blockIdx.x, validn, true);
+        for (int64_t row = blockIdx.x; row < a.n_tok; row += gridDim.x) {
+            h = hn; valid = validn;
+            {   // the next row's header: its loads are in flight while this row is waited for
+                const int64_t nrow = row + gridDim.x;
+                if (lane == 0 && nrow < a.n_tok) hn = load_row_header(a, nrow, validn, true);
+            }
+            mbar_wait(done0 + 8u * slot, sphase);
+            const bool mine = lane < kFwdWarps;
+            const float2 st = ctrl->stats[slot][lane & (kFwdWarps - 1)];
+            const float stz = ENT ? ctrl->statz[slot][lane & (kFwdWarps - 1)] : 0.f;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(freed0 + 8u * slot);
+            float M = mine ? st.x : -INFINITY;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(kFull, M, o));
+            const float rs = (!mine || st.x == -INFINITY) ? 0.f : ex2_approx((st.x - M) * kLog2e);
+            float S = st.y * rs;
+            float SZ = stz * rs;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                S += __shfl_xor_sync(kFull, S, o);
+                if (ENT) SZ += __shfl_xor_sync(kFull, SZ, o);
+            }
+            if (lane == 0) {
+                const float lse_rest = M + logf(S);                      // -inf: nothing but the target
+                const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
+                store_token_outputs(a, row, h, ts, valid);
+                if (ENT) a.token_entropy[row] = valid ? row_entropy(ts.lse, M, SZ, ts.lp, h.zy) : 0.f;
+            }
+            if (++slot == kFwdSlots) { slot = 0; sphase ^= 1u; }
+        }
+        return;
+    }
+
     // ===================== consumers
     int stage = 0;
     uint32_t phase = 0;
-    int par = 0;
-    int fin = 0;                                         // the warp that finalises this row
+    int slot = 0;
+    uint32_t sphase = 0;
     int y_next = -1;
     if (blockIdx.x < a.n_tok) y_next = a.target_ids[blockIdx.x];
-    for (int64_t row = blockIdx.x; row < a.n_tok; row += gridDim.x, par ^= 1) {
+    for (int64_t row = blockIdx.x; row < a.n_tok; row += gridDim.x) {
         const int y = y_next;
         {
             const int64_t nrow = row + gridDim.x;
@@ -162,7 +216,8 @@ rows_fwd_kernel(RowArgs a, int units_per_row) {
             if (ENT) sz += accz[0] + accz[1];
         }
 
-        // ---- merge the 32 lanes, publish the warp's state, meet the other warps
+        // ---- merge the 32 lanes and publish the warp's state of this row; no waiting for the
+        // other warps (only for the a3 warp to have read this slot 8 rows ago)
         float wm = m;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) wm = fmaxf(wm, __shfl_xor_sync(kFull, wm, o));
@@ -175,36 +230,12 @@ rows_fwd_kernel(RowArgs a, int units_per_row) {
             if (ENT) wz += __shfl_xor_sync(kFull, wz, o);
         }
         if (lane == 0) {
-            ctrl->stats[par][warp] = make_float2(wm, ws);
-            if (ENT) ctrl->statz[par][warp] = wz;
+            mbar_wait(freed0 + 8u * slot, sphase ^ 1u);
+            ctrl->stats[slot][warp] = make_float2(wm, ws);
+            if (ENT) ctrl->statz[slot][warp] = wz;
+            mbar_arrive(done0 + 8u * slot);                              // release: the stores above
         }
-        asm volatile("bar.sync 1, %0;" ::"n"(kFwdConsumers) : "memory");
-
-        // ---- a3 on one warp (rotating), while the others go on to the next row
-        if (warp == fin) {
-            const float2 st = ctrl->stats[par][lane & (kFwdWarps - 1)];
-            const bool mine = lane < kFwdWarps;
-            float M = mine ? st.x : -INFINITY;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(kFull, M, o));
-            const float rs = (!mine || st.x == -INFINITY) ? 0.f : ex2_approx((st.x - M) * kLog2e);
-            float S = st.y * rs;
-            float SZ = ENT ? ctrl->statz[par][lane & (kFwdWarps - 1)] * rs : 0.f;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                S += __shfl_xor_sync(kFull, S, o);
-                if (ENT) SZ += __shfl_xor_sync(kFull, SZ, o);
-            }
-            if (lane == 0) {
-                bool v2 = false;
-                const RowHeader h = load_row_header(a, row, v2, true);
-                const float lse_rest = M + logf(S);                      // -inf: nothing but the target
-                const TokenScalars ts = token_scalars(h, lse_rest, v2, a.clip_eps, a.stale_cap, a.dual_c);
-                store_token_outputs(a, row, h, ts, v2);
-                if (ENT) a.token_entropy[row] = v2 ? row_entropy(ts.lse, M, SZ, ts.lp, h.zy) : 0.f;
-            }
-        }
-        if (++fin == kFwdWarps) fin = 0;
+        if (++slot == kFwdSlots) { slot = 0; sphase ^= 1u; }
     }
 }
 

@@ -31,6 +31,7 @@ def _f64(t):
 
 
 HEAD_KERNELS = [A.KERNEL_HEAD_1CTA, A.KERNEL_HEAD_2CTA]
+HEAD_PANEL_KERNELS = [A.KERNEL_HEAD_2CTA_STORED, A.KERNEL_HEAD_2CTA_E16]   # keep one row panel of logits / E
 
 
 # ------------------------------------------------------------------ the GEMM engine alone
@@ -114,7 +115,7 @@ def _check_head(gpu, ora, w_layout):
         assert not gpu["dhidden"][torch.from_numpy(zero_rows).to(DEV)].any()
 
 
-@pytest.mark.parametrize("kernel", HEAD_KERNELS + [A.KERNEL_HEAD_2CTA_STORED])
+@pytest.mark.parametrize("kernel", HEAD_KERNELS + HEAD_PANEL_KERNELS)
 @pytest.mark.parametrize("w_layout", [A.W_K_BY_V, A.W_V_BY_K])
 @pytest.mark.parametrize("n_tok,K,V", [(300, 128, 1000), (128, 64, 256), (517, 192, 2056)])
 def test_head_vs_oracle(n_tok, K, V, w_layout, kernel):
@@ -129,7 +130,8 @@ def test_head_vs_oracle(n_tok, K, V, w_layout, kernel):
 
 @pytest.mark.parametrize("kernel,n_tok,panels", [(A.KERNEL_HEAD_1CTA, 9700, 3),
                                                  (A.KERNEL_HEAD_2CTA, 19300, 3),
-                                                 (A.KERNEL_HEAD_2CTA_STORED, 19300, 3)])
+                                                 (A.KERNEL_HEAD_2CTA_STORED, 19300, 3),
+                                                 (A.KERNEL_HEAD_2CTA_E16, 19300, 3)])
 @pytest.mark.parametrize("norm", [A.NORM_CONST_K, A.NORM_PER_TRAJ])
 def test_head_several_panels(norm, kernel, n_tok, panels):
     """More rows than one dS panel (4,736 rows, 9,472 for CTA pairs): dw_head accumulates
@@ -138,10 +140,10 @@ def test_head_several_panels(norm, kernel, n_tok, panels):
     gpu = _run_head(batch, A.W_K_BY_V, normalizer=norm, kernel=kernel)
     ora = _oracle_head(batch, normalizer=norm)
     _check_head(gpu, ora, A.W_K_BY_V)
-    per_call = 5 * panels if kernel == A.KERNEL_HEAD_2CTA_STORED else 2 + 3 * panels
+    per_call = 5 * panels if kernel in HEAD_PANEL_KERNELS else 2 + 3 * panels
     assert A.head_launches_per_call(n_tok, 512, 64, kernel) == 3 + per_call
     assert A.head_launches_per_call(n_tok, 512, 64) == A.head_launches_per_call(
-        n_tok, 512, 64, A.KERNEL_HEAD_2CTA_STORED)          # AUTO resolves to the stored mode
+        n_tok, 512, 64, A.KERNEL_HEAD_2CTA_E16)             # AUTO resolves to the E16 mode
 
 
 def test_head_stored_logits_same_bits_as_recompute():
@@ -255,14 +257,14 @@ def test_head_random_shapes(n_tok, K, V, seed):
     (V a multiple of 64 or not), all three kernel modes."""
     batch = _head_batch(max(n_tok, 16), K, V, seed=seed, lp_mode="drift", masked_frac=0.02)
     ora = _oracle_head(batch, stale_cap=2.0)
-    for kernel in HEAD_KERNELS + [A.KERNEL_HEAD_2CTA_STORED]:
+    for kernel in HEAD_KERNELS + HEAD_PANEL_KERNELS:
         gpu = _run_head(batch, kernel=kernel, stale_cap=2.0)
         _check_head(gpu, ora, A.W_K_BY_V)
     gpu = _run_head(batch, A.W_V_BY_K, stale_cap=2.0)
     _check_head(gpu, ora, A.W_V_BY_K)
 
 
-@pytest.mark.parametrize("kernel", HEAD_KERNELS + [A.KERNEL_HEAD_2CTA_STORED])
+@pytest.mark.parametrize("kernel", HEAD_KERNELS + HEAD_PANEL_KERNELS)
 def test_head_token_entropy(kernel):
     """Per-token entropy from the fused head: a third per-tile partial (sum e^{z-m} z) merged
     across the vocabulary tiles; |dH| <= 1e-4 against the oracle, 0 for masked tokens, and the
@@ -290,7 +292,7 @@ def test_head_wide_dhidden_tiles(K, n_tok):
     batch = _head_batch(n_tok, K, 1512, seed=44, lp_mode="drift", masked_frac=0.02)
     ora = _oracle_head(batch, stale_cap=2.0)
     outs = {}
-    for kernel in HEAD_KERNELS + [A.KERNEL_HEAD_2CTA_STORED]:
+    for kernel in HEAD_KERNELS + HEAD_PANEL_KERNELS:
         outs[kernel] = _run_head(batch, kernel=kernel, stale_cap=2.0)
         _check_head(outs[kernel], ora, A.W_K_BY_V)
     d = (outs[A.KERNEL_HEAD_1CTA]["dhidden"].float() - outs[A.KERNEL_HEAD_2CTA]["dhidden"].float()).abs().max()
@@ -381,3 +383,13 @@ def test_head_host_buffer_entry():
         assert not out[k].is_cuda
         assert torch.equal(out[k], dev[k].cpu()), k
     assert call.h2d_bytes > 2 * (700 * 128 + 128 * 2056) and call.d2h_bytes > 2 * (700 * 128 + 128 * 2056)
+
+
+def test_head_workspace_is_mode_aware():
+    """include/awr.h: the workspace query takes the kernel; AUTO (E16) keeps 2 bytes per logit of one
+    row panel - BASELINE.json configs[4] fits in 5 GB - the stored-fp32 mode needs three times that."""
+    auto = A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16)
+    e16 = A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_HEAD_2CTA_E16)
+    stored = A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_HEAD_2CTA_STORED)
+    assert auto == e16 <= 5 * 10 ** 9 < stored
+    assert A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_CLUSTER_RF) == 0
