@@ -30,24 +30,6 @@ __device__ __forceinline__ float lg2_approx(float x) {
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// 2^t for t <= 0 on the FMA / ALU pipes instead of the special-function unit (the exp pass of the
-// register-file row kernel is MUFU-bound at 16 ex2 / clk / SM; a quarter of its exponentials go
-// through here so that both pipes work side by side).  Round-to-nearest split t = j + f with the
-// 1.5 * 2^23 magic number, f in [-0.5, 0.5]; degree-3 minimax polynomial for 2^f (max relative
-// error 9.4e-5, mean -2.7e-6: far below the bf16 rounding of the gradient and, averaged over a
-// row, below the 1e-4 bar on the log-prob); 2^j built in the exponent field and applied with one
-// multiply, so that t <= -127 (a -inf logit) gives exactly 0.
-__device__ __forceinline__ float ex2_poly(float t) {
-    t = fmaxf(t, -127.0f);
-    const float r = t + 12582912.0f;                         // j in the low mantissa bits
-    const float f = t - (r - 12582912.0f);
-    float p = fmaf(0.05522309988737106f, f, 0.2427525818347931f);
-    p = fmaf(p, f, 0.6932584643363953f);
-    p = fmaf(p, f, 0.9999087452888489f);
-    const float scale = __int_as_float((__float_as_int(r) << 23) + 0x3f800000);   // 2^j; 0 at j = -127
-    return p * scale;
-}
-
 // exp / log on the special-function unit (2 ulp ex2 / lg2 + one rounding of the scaled argument):
 // a3 runs redundantly in every thread between the passes of a row, so its latency is on the
 // critical path of every row; libm's expf / logf / log1pf cost ~1.2 k clocks there (measured).

@@ -20,9 +20,6 @@
 //   * Persistent: one cluster per SM pair, rows dealt round-robin to clusters (static schedule,
 //     deterministic results).  Rows with c_t = 0 (masked, zero advantage, clip triggered) skip
 //     pass 2 and are written as zeros.
-#include <stdio.h>
-#include <stdlib.h>
-
 #include "awr_common.cuh"
 #include "awr_kernels.h"
 #include "awr_ptx.cuh"
@@ -41,11 +38,6 @@ constexpr int kRfSlotBytes = kRfChunkUnits * 16;
 constexpr int kRfCtrlBytes = 2048;
 constexpr int kRfMinNU = 3, kRfMaxNU = 20;
 constexpr uint32_t kNegInf2 = 0xff80ff80u;  // bf16x2 (-inf, -inf)
-#ifndef AWR_RF_POLY_WORD
-#define AWR_RF_POLY_WORD 3
-#endif
-constexpr int kRfPolyWord = AWR_RF_POLY_WORD;   // word of every 16-byte unit whose two exponentials use
-                                            // ex2_poly (25 % of the row); -1: all on the MUFU
 
 // Two shapes of the same kernel (CL CTAs per cluster x WARPS warps per CTA = 32 parts per row):
 //   CL = 2, WARPS = 16: one CTA per SM, a row half per SM, 2 ring slots of 5 KB per warp (160 KB).
@@ -66,7 +58,6 @@ static_assert(2 * (RfShape<4>::kSmemBytes + 1024) <= 233472, "two CTAs in 228 KB
 struct RfPlan {
     int units_per_row;   // 16-byte units in one row (V / 8)
     int num_clusters;
-    int skew_clocks;     // CL = 4: the second half of the clusters starts this many clocks late
 };
 
 struct RfCtrl {
@@ -119,12 +110,6 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
     __syncwarp();
     cluster_arrive();     // both CTAs are resident before any distributed-shared-memory store
     cluster_wait();
-
-    if (p.skew_clocks > 0 && cluster >= (p.num_clusters + 1) / 2) {
-        // phase skew between the two CTAs that share an SM (they belong to different clusters)
-        const long long t0 = clock64();
-        while (clock64() - t0 < p.skew_clocks) {}
-    }
 
     // ---- TMA producer state (warp-uniform; lane 0 issues)
     int ld_seq = 0, ld_ch = 0, ld_slot = 0;
@@ -224,10 +209,8 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float z0 = bf16_lo(v[k][j]), z1 = bf16_hi(v[k][j]);
-                // one word in four on the FMA pipe (ex2_poly), the rest on the MUFU
-                const bool poly = kRfPolyWord >= 0 && j == kRfPolyWord;
-                const float e0 = poly ? ex2_poly(fmaf(z0, kLog2e, nref)) : ex2_approx(fmaf(z0, kLog2e, nref));
-                const float e1 = poly ? ex2_poly(fmaf(z1, kLog2e, nref)) : ex2_approx(fmaf(z1, kLog2e, nref));
+                const float e0 = ex2_approx(fmaf(z0, kLog2e, nref));
+                const float e1 = ex2_approx(fmaf(z1, kLog2e, nref));
                 acc[j] += e0;
                 acc[j] += e1;
                 if (want_ent) {
@@ -323,7 +306,6 @@ static bool make_rf_plan(int64_t V, int64_t ld, int dtype, RfPlan& p, int& nu) {
     if (n < kRfMinNU || n > kRfMaxNU) return false;
     p.units_per_row = (int)units;
     p.num_clusters = 0;
-    p.skew_clocks = 0;
     nu = (int)n;
     return true;
 }
@@ -364,8 +346,6 @@ static cudaError_t launch_nu(const RowArgs& a, RfPlan p, int num_sms, cudaStream
         max_clusters = n < 1 ? 1 : (n > want ? want : n);
         cached.set(dev, max_clusters);
     }
-    if (const char* sk = getenv("AWR_RF_SKEW")) p.skew_clocks = atoi(sk);       // experiment knob
-    if (getenv("AWR_RF_DEBUG")) fprintf(stderr, "rows_rf<%d,%d>: max_clusters %d skew %d\n", NU, CL, max_clusters, p.skew_clocks);
     int nc = max_clusters;
     if ((int64_t)nc > a.n_tok) nc = (int)a.n_tok;
     p.num_clusters = nc;
