@@ -511,7 +511,8 @@ def run_cuda(args):
               "rf": A.KERNEL_CLUSTER_RF, "rf4": A.KERNEL_CLUSTER_RF4}[args.kernel]
     leg, batch, call, local_ms = rows_leg(torch, A, W, dev, args.config, args.steps, args.warmup,
                                           seed=1000 + rank, normalizer=args.normalizer, kernel=kernel,
-                                          n_tok=args.n_tok or None, leg="config%d" % args.config,
+                                          n_tok=args.n_tok or None, backward=not args.forward_only,
+                                          leg=("config%d_fwd" if args.forward_only else "config%d") % args.config,
                                           rank_barrier=lambda: barrier(world))
     w = W.workload(args.config)
     n_tok, V = batch["n_tok"], batch["V"]
@@ -528,7 +529,7 @@ def run_cuda(args):
 
     # ---- end-to-end leg: host buffers through awr_loss_fwd_bwd_host
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.forward_only:
         e2e_steps = args.e2e_steps or args.steps
         host_in = {}
         for k in ("logits", "target_ids", "behave_lp", "prox_lp", "step_off", "traj_off",
@@ -572,11 +573,13 @@ def run_cuda(args):
 
     # ---- the other configs and the forward-only entry (N = 1, default workload only)
     others = None
-    if rank == 0 and world == 1 and args.config == 1 and not args.no_others and not args.n_tok:
+    if rank == 0 and world == 1 and args.config == 1 and not args.no_others and not args.n_tok \
+            and not args.forward_only:
         others = other_legs(torch, A, W, dev)
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
+        line = {"metric": METRIC if not args.forward_only else "forward-only tokens/s at V=151,936 bf16",
+                "value": value, "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "bf16 in/out, f32 math" if esz == 2 else "f32",
@@ -709,6 +712,8 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: --steps")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--forward-only", action="store_true",
+                    help="time awr_loss_fwd (PAPER.md:436 prox-lp recompute) instead of awr_loss_fwd_bwd")
     ap.add_argument("--no-others", action="store_true",
                     help="skip the legs for the other configs / the forward-only entry")
     args = ap.parse_args(argv)

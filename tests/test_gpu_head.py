@@ -393,3 +393,40 @@ def test_head_workspace_is_mode_aware():
     stored = A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_HEAD_2CTA_STORED)
     assert auto == e16 <= 5 * 10 ** 9 < stored
     assert A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_CLUSTER_RF) == 0
+
+
+@pytest.mark.parametrize("kernel", HEAD_KERNELS + HEAD_PANEL_KERNELS)
+def test_red_zones_fused_head(kernel):
+    """dhidden, dw_head and the workspace of the fused head between 4 KB zones of a byte pattern
+    that must survive the call (stands in for compute-sanitizer memcheck, closed on this pool)."""
+    PAT = 0x5A
+    batch = _head_batch(600, 128, 2056, seed=19, lp_mode="drift", masked_frac=0.02)
+    n_steps, n_traj, n_groups = (batch[k].numel() - 1 for k in ("step_off", "traj_off", "group_off"))
+    need = A.head_workspace_bytes(600, 2056, 128, n_steps, n_traj, n_groups, kernel)
+    need = (need + 255) // 256 * 256
+    wsbuf = torch.empty(need + 8192, dtype=torch.uint8, device=DEV)
+    wsbuf.fill_(PAT)
+    off = 4096 + ((-(wsbuf.data_ptr() + 4096)) % 256)
+    call = A.HeadLossCall(batch["hidden"], batch["w_head"], batch["target_ids"], batch["behave_lp"],
+                          batch["prox_lp"], batch["step_off"], batch["traj_off"], batch["group_off"],
+                          batch["rewards"], workspace=wsbuf[off:off + need],
+                          **dict(batch["params"], kernel=kernel))
+    guarded = {}
+    for k in ("dhidden", "dw_head", "token_lp"):
+        t = call.out[k]
+        buf = torch.empty(t.numel() + 4096, dtype=t.dtype, device=DEV)
+        buf.view(torch.uint8).fill_(PAT)
+        view = buf[2048:2048 + t.numel()].view(t.shape)
+        call.out[k] = view
+        setattr(call.outs, k, view.data_ptr())
+        guarded[k] = (buf, t.numel())
+    call.run()
+    torch.cuda.synchronize()
+    assert int(call.out["err_word"][0]) == 0
+    for k, (buf, n) in guarded.items():
+        raw = buf.view(torch.uint8)
+        esz = buf.element_size()
+        assert bool((raw[:2048 * esz] == PAT).all()) and bool((raw[(2048 + n) * esz:] == PAT).all()), k
+    assert bool((wsbuf[:off] == PAT).all()) and bool((wsbuf[off + need:] == PAT).all()), "workspace"
+    ora = _oracle_head(batch)
+    _check_head(call.out, ora, A.W_K_BY_V)

@@ -612,3 +612,70 @@ def test_host_buffer_entry(n_tok, V, dtype):
     P.check_scalars({k: v for k, v in out.items() if k != "dlogits"}, ora)
     P.check_dlogits(out["dlogits"].to(DEV), ora, V)
     assert np.abs(out["token_entropy"].numpy() - ora["token_entropy"]).max() <= 1e-4
+
+
+# ------------------------------------------------------------------ red zones (compute-sanitizer is closed on this pool)
+def _guarded(shape, dtype, pattern, pad=4096):
+    """A tensor of `shape` carved out of a larger buffer whose head and tail hold a byte pattern."""
+    n = int(np.prod(shape))
+    esz = torch.empty(0, dtype=dtype).element_size()
+    pad_e = pad // esz
+    buf = torch.empty(n + 2 * pad_e, dtype=dtype, device=DEV)
+    buf.view(torch.uint8).fill_(pattern)
+    return buf, buf[pad_e:pad_e + n].view(shape), pad_e
+
+
+def _zones_intact(buf, pad_e, n, pattern):
+    raw = buf.view(torch.uint8)
+    esz = buf.element_size()
+    return bool((raw[:pad_e * esz] == pattern).all()) and bool((raw[(pad_e + n) * esz:] == pattern).all())
+
+
+@pytest.mark.parametrize("kernel,backward", [(A.KERNEL_GENERIC, True), (A.KERNEL_CLUSTER, True),
+                                             (A.KERNEL_CLUSTER_RF, True), (A.KERNEL_CLUSTER_RF4, True),
+                                             (A.KERNEL_FWD_STREAM, False)])
+@pytest.mark.parametrize("V,ld", [(151_936, 151_936), (40_000, 40_008)])
+def test_red_zones_row_kernels(kernel, backward, V, ld):
+    """No kernel writes outside its outputs or its workspace, and none writes the columns
+    >= V of a padded gradient row: every output (and the workspace) sits between two 4 KB zones
+    of a byte pattern that must survive; the gradient buffer is pre-filled with the pattern and
+    its padding columns must still hold it.  (Stands in for compute-sanitizer memcheck, which
+    is closed on this pool: profiles/r2_sanitizer.md.)"""
+    w = W.workload(3, n_groups=6, group_size=4, n_tok=333, V=V)
+    b = W.make_batch(w, seed=21, device=DEV, ld=ld, masked_frac=0.03)
+    n, n_traj = b["n_tok"], b["rewards"].numel()
+    PAT = 0xA5
+    spec = dict(loss=((1,), torch.float32), token_lp=((n,), torch.float32), clip_count=((1,), torch.int64),
+                dual_clip_count=((1,), torch.int64), adv=((n_traj,), torch.float32),
+                tok_traj=((n,), torch.int32), target_logit=((n,), torch.float32),
+                tok_term=((n,), torch.float32), tok_coef=((n,), torch.float32),
+                err_word=((1,), torch.int32), token_entropy=((n,), torch.float32))
+    bufs, out = {}, {}
+    for k, (shape, dt) in spec.items():
+        bufs[k], out[k], _ = _guarded(shape, dt, PAT)
+    if backward:
+        bufs["dlogits"], out["dlogits"], _ = _guarded((n, ld), torch.bfloat16, PAT)
+    need = A.workspace_bytes(n, V, b["step_off"].numel() - 1, n_traj, b["group_off"].numel() - 1)
+    need = (need + 255) // 256 * 256
+    wsbuf = torch.empty(need + 8192, dtype=torch.uint8, device=DEV)
+    off = 4096 + ((-(wsbuf.data_ptr() + 4096)) % 256)       # 256-byte aligned, >= 4 KB in
+    wsbuf.fill_(PAT)
+    ws = wsbuf[off:off + need]
+    call = A.LossCall(b["logits"], b["target_ids"], b["behave_lp"], b["prox_lp"], b["step_off"], b["traj_off"],
+                      b["group_off"], b["rewards"], V=V, backward=backward, out=out, workspace=ws,
+                      **dict(b["params"], kernel=kernel, dual_clip_c=3.0))
+    if kernel == A.KERNEL_CLUSTER:
+        call.outs.token_entropy = None                   # not offered by the shared-memory cluster kernel
+    call.run()
+    torch.cuda.synchronize()
+    assert int(out["err_word"][0]) == 0
+    for k, (shape, dt) in spec.items():
+        pad_e = 4096 // torch.empty(0, dtype=dt).element_size()
+        assert _zones_intact(bufs[k], pad_e, int(np.prod(shape)), PAT), k
+    assert bool((wsbuf[:off] == PAT).all()) and bool((wsbuf[off + need:] == PAT).all()), "workspace"
+    if backward:
+        assert _zones_intact(bufs["dlogits"], 2048, n * ld, PAT), "dlogits"
+        if ld > V:
+            padcols = out["dlogits"][:, V:].contiguous().view(torch.uint8)
+            assert bool((padcols == PAT).all()), "columns >= V of the gradient rows were written"
+        assert np.isfinite(out["dlogits"][:, :V].float().cpu().numpy()).all()
