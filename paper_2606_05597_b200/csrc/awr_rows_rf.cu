@@ -35,6 +35,7 @@ constexpr int kRfParts = 32;                // warps per row (over the whole clu
 constexpr int kRfChunkRounds = 10;          // rounds (32 units each) per slot / per TMA copy
 constexpr int kRfChunkUnits = 32 * kRfChunkRounds;
 constexpr int kRfSlotBytes = kRfChunkUnits * 16;
+constexpr int kRfStageRounds = 4;           // rounds (512 B each) per staging buffer / per TMA store
 constexpr int kRfCtrlBytes = 2048;
 constexpr int kRfMinNU = 3, kRfMaxNU = 20;
 constexpr uint32_t kNegInf2 = 0xff80ff80u;  // bf16x2 (-inf, -inf)
@@ -50,7 +51,12 @@ struct RfShape {
     static constexpr int kThreads = kWarps * 32;
     static constexpr int kSlots = 2;
     static constexpr int kCtasPerSm = CL == 2 ? 1 : 2;
-    static constexpr int kSmemBytes = kRfCtrlBytes + kWarps * kSlots * kRfSlotBytes;
+    // CL = 2: the gradient leaves through a per-warp staging area (two buffers of kRfStageRounds
+    // rounds) and TMA bulk stores instead of per-lane 16-byte global stores
+    static constexpr bool kStaged = CL == 2;
+    static constexpr int kStageBytes = kStaged ? 2 * kRfStageRounds * 512 : 0;      // per warp
+    static constexpr int kRingBytes = kWarps * kSlots * kRfSlotBytes;
+    static constexpr int kSmemBytes = kRfCtrlBytes + kRingBytes + kWarps * kStageBytes;
 };
 static_assert(RfShape<2>::kSmemBytes <= 232448, "227 KB of dynamic shared memory per CTA");
 static_assert(2 * (RfShape<4>::kSmemBytes + 1024) <= 233472, "two CTAs in 228 KB per SM");
@@ -87,6 +93,8 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
     const int cluster = (int)cluster_id_x();
     const uint32_t ring = smem_u32(smem + kRfCtrlBytes) + (uint32_t)warp * (kRfSlots * kRfSlotBytes);
     const uint32_t bar0 = smem_u32(&ctrl->full[warp * 8]);
+    const uint32_t stage = smem_u32(smem + kRfCtrlBytes + RfShape<CL>::kRingBytes) +
+                           (uint32_t)warp * RfShape<CL>::kStageBytes;
 
     // this warp's part of the row, in 16-byte units: [part0, part0 + part_units)
     const int part_idx = (int)rank * kRfWarps + warp;
@@ -136,6 +144,7 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
     int y_next = -1, traj_next = -1;
     if (cluster < a.n_tok) { y_next = a.target_ids[cluster]; traj_next = a.tok_traj[cluster]; }
     int par = 0;
+    uint32_t stage_par = 0;               // staging buffers handed to the TMA so far (parity = next buffer)
     for (int64_t row = cluster; row < a.n_tok; row += p.num_clusters, par ^= 1) {
         // ---- row header: every thread loads the same words (one sector each).  Only the raw
         // loads are issued here; nothing consumes them before the cluster barrier (the selects
@@ -261,27 +270,66 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
 
         // ---- pass 2 (a4): dlogits = e * (c_t exp(m - lse)), straight from registers
         if (backward) {
-            uint8_t* g = gbase + row * row_bytes;
-            if (ts.coef == 0.f) {
+            // e was taken relative to m (0 if the part held nothing finite); c_t = 0 (masked, zero
+            // advantage, clip triggered): F = +0 and e >= 0 give all-bits-zero products
+            const float F = ts.coef == 0.f ? 0.f : ts.coef * ex2_approx(fmaf(-ts.lse, kLog2e, -nref));
+            const __nv_bfloat16 fh = __float2bfloat16_rn(F);
+            const __nv_bfloat16 fl = __float2bfloat16_rn(F - __bfloat162float(fh));
+            const uint32_t Fh = (uint32_t)__bfloat16_as_ushort(fh) * 0x00010001u;
+            const uint32_t Fl = (uint32_t)__bfloat16_as_ushort(fl) * 0x00010001u;
+            const uint32_t gy_bits = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(ts.gy));
+            const uint32_t gy2 = (h.y & 1) ? (gy_bits << 16) : gy_bits;
+            const bool patch = owner && ts.coef != 0.f;
+            if constexpr (RfShape<CL>::kStaged) {
+                // The SM's path for per-lane global stores takes 32 B/clk: 148 KB of gradient per row
+                // half held every warp ~5 k clocks in this pass.  Instead the warp writes its part to
+                // a staging buffer in shared memory (128 B/clk) and lane 0 hands each buffer to a TMA
+                // bulk store, which drains it to global memory while the warp is already in the next
+                // row; the registers are free as soon as the shared-memory write has been issued.
+                uint8_t* g = reinterpret_cast<uint8_t*>(a.dlogits) + (int64_t)part0 * 16 + row * row_bytes;
 #pragma unroll
-                for (int k = 0; k < NU; ++k)
-                    if (k < NU - 1 || k * 32 + lane < part_units)
-                        stg128_cs(g + k * (32 * 16), 0u, 0u, 0u, 0u);
+                for (int k = 0; k < NU; ++k) {
+                    const int kk = k % kRfStageRounds;
+                    const uint32_t buf = stage + (((uint32_t)(k / kRfStageRounds) + stage_par) & 1u) * (kRfStageRounds * 512);
+                    if (kk == 0) {
+                        // the bulk store issued two buffers ago has read this buffer out
+                        if (lane == 0) bulk_wait_read<1>();
+                        __syncwarp();
+                    }
+                    uint4 o;
+                    o.x = fma_bf16x2(v[k][0], Fh, mul_bf16x2(v[k][0], Fl));
+                    o.y = fma_bf16x2(v[k][1], Fh, mul_bf16x2(v[k][1], Fl));
+                    o.z = fma_bf16x2(v[k][2], Fh, mul_bf16x2(v[k][2], Fl));
+                    o.w = fma_bf16x2(v[k][3], Fh, mul_bf16x2(v[k][3], Fl));
+                    if (patch && k * 32 + lane == y_unit) {     // target entry: c (p_y - 1)
+                        o.x = y_word == 0 ? ((o.x & y_keep) | gy2) : o.x;
+                        o.y = y_word == 1 ? ((o.y & y_keep) | gy2) : o.y;
+                        o.z = y_word == 2 ? ((o.z & y_keep) | gy2) : o.z;
+                        o.w = y_word == 3 ? ((o.w & y_keep) | gy2) : o.w;
+                    }
+                    sts128(buf + (uint32_t)kk * 512u + (uint32_t)lane * 16u, o);
+                    if (kk == kRfStageRounds - 1 || k == NU - 1) {
+                        const int k0 = k - kk;                                  // first round of the buffer
+                        const int units = min(part_units, (k + 1) * 32) - k0 * 32;
+                        fence_proxy_async();                                    // generic writes -> TMA read
+                        __syncwarp();
+                        if (lane == 0 && units > 0) {
+                            bulk_store(g + (int64_t)k0 * 512, buf, (uint32_t)units * 16u);
+                            bulk_commit();
+                        }
+                    }
+                }
+                // the two buffers alternate across rows as well (a row has an odd number of pieces
+                // for most V): the next row starts with the buffer this row did not end on
+                stage_par += (uint32_t)((NU + kRfStageRounds - 1) / kRfStageRounds);
             } else {
-                // e was taken relative to m (0 if the part held nothing finite)
-                const float F = ts.coef * ex2_approx(fmaf(-ts.lse, kLog2e, -nref));
-                const __nv_bfloat16 fh = __float2bfloat16_rn(F);
-                const __nv_bfloat16 fl = __float2bfloat16_rn(F - __bfloat162float(fh));
-                const uint32_t Fh = (uint32_t)__bfloat16_as_ushort(fh) * 0x00010001u;
-                const uint32_t Fl = (uint32_t)__bfloat16_as_ushort(fl) * 0x00010001u;
-                const uint32_t gy_bits = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(ts.gy));
-                const uint32_t gy2 = (h.y & 1) ? (gy_bits << 16) : gy_bits;
+                uint8_t* g = gbase + row * row_bytes;
 #pragma unroll
                 for (int k = 0; k < NU; ++k) {
                     uint32_t o[4];
 #pragma unroll
                     for (int j = 0; j < 4; ++j) o[j] = fma_bf16x2(v[k][j], Fh, mul_bf16x2(v[k][j], Fl));
-                    if (owner && k * 32 + lane == y_unit) {     // target entry: c (p_y - 1)
+                    if (patch && k * 32 + lane == y_unit) {     // target entry: c (p_y - 1)
 #pragma unroll
                         for (int j = 0; j < 4; ++j)
                             o[j] = (j == y_word) ? ((o[j] & y_keep) | gy2) : o[j];
@@ -292,6 +340,7 @@ rows_rf_kernel(RowArgs a, RfPlan p) {
             }
         }
     }
+    if (lane == 0) bulk_wait_all();       // staged gradient writes complete before the CTA ends
     cluster_arrive();
     cluster_wait();
 }
