@@ -299,7 +299,7 @@ def measured_peaks():
 
 
 KERNEL_NAMES = {1: "rows_generic_kernel", 2: "rows_cluster_kernel", 3: "rows_rf_kernel<NU,2>",
-                4: "rows_rf_kernel<NU,4>", 8: "rows_fwd_kernel"}
+                4: "rows_rf_kernel<NU,4>", 8: "rows_fwd_kernel", 10: "rows_rfs_kernel<NU>"}
 
 
 def load_traffic(leg: str):
@@ -508,7 +508,7 @@ def run_cuda(args):
     init_dist("nccl")
 
     kernel = {"auto": A.KERNEL_AUTO, "generic": A.KERNEL_GENERIC, "cluster": A.KERNEL_CLUSTER,
-              "rf": A.KERNEL_CLUSTER_RF, "rf4": A.KERNEL_CLUSTER_RF4}[args.kernel]
+              "rf": A.KERNEL_CLUSTER_RF, "rf4": A.KERNEL_CLUSTER_RF4, "rfs": A.KERNEL_CLUSTER_RFS}[args.kernel]
     leg, batch, call, local_ms = rows_leg(torch, A, W, dev, args.config, args.steps, args.warmup,
                                           seed=1000 + rank, normalizer=args.normalizer, kernel=kernel,
                                           n_tok=args.n_tok or None, backward=not args.forward_only,
@@ -705,7 +705,7 @@ def main(argv=None):
                     help="BASELINE.json configs[i]; 5 = the Thinking-variant shapes (SURVEY 8(f) rank 4)")
     ap.add_argument("--n-tok", type=int, default=0, help="override the config's token count")
     ap.add_argument("--normalizer", type=int, default=None, choices=[0, 1])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4", "rfs"])
     ap.add_argument("--head-kernel", default="auto", choices=["auto", "1cta", "2cta", "stored"],
                     help="config 4: tcgen05 shape / backward mode (auto = stored: CTA pairs, fp32 "
                          "logits of one row panel kept for the dS pass; 1cta / 2cta recompute)")

@@ -107,7 +107,12 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_HEAD_2CTA_E16 = 9 /* fused head, CTA pairs: the forward epilogue leaves E = bf16(exp(z -
                                     tile row max)) of ONE row panel (<= 9,472 rows) in the dS buffer and one
                                     in-place pass rescales it to dS: 6 K V flops/token, 2 bytes of
-                                    transient per logit of the panel, no side stream */ };
+                                    transient per logit of the panel, no side stream */,
+       AWR_KERNEL_CLUSTER_RFS = 10 /* row resident in the register files of a 2-CTA cluster, 15 data
+                                    warps + one service warp per CTA: whole-slot TMA loads, gradient
+                                    through shared-memory staging and TMA bulk stores, (max, sum)
+                                    exchange by st.async, a3 on the service warp (bf16, 15,368 <= V
+                                    <= 153,600; AUTO's choice for awr_loss_fwd_bwd there) */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u };
 
@@ -285,7 +290,8 @@ AWR_API const char* awr_status_string(int status);
 AWR_API int awr_version(void);
 
 /* Introspection for benchmarks and tests: which row kernel AWR_KERNEL_AUTO resolves to for
- * this shape (AWR_KERNEL_GENERIC, AWR_KERNEL_CLUSTER or AWR_KERNEL_CLUSTER_RF), and the number of kernel launches one
+ * this shape in awr_loss_fwd_bwd (AWR_KERNEL_GENERIC, AWR_KERNEL_CLUSTER, AWR_KERNEL_CLUSTER_RF or
+ * AWR_KERNEL_CLUSTER_RFS), and the number of kernel launches one
  * awr_loss_fwd_bwd call enqueues. */
 AWR_API int awr_select_kernel(int64_t V, int64_t ld, int32_t logits_dtype);
 AWR_API int awr_launches_per_call(void);

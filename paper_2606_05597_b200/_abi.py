@@ -27,6 +27,7 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_CLUSTER, KERNEL_CLUSTER_RF, KERNEL_CLUSTER_R
 KERNEL_HEAD_1CTA, KERNEL_HEAD_2CTA, KERNEL_HEAD_2CTA_STORED = 5, 6, 7
 KERNEL_FWD_STREAM = 8
 KERNEL_HEAD_2CTA_E16 = 9
+KERNEL_CLUSTER_RFS = 10
 ERRBIT_STEP_OFF, ERRBIT_TRAJ_OFF, ERRBIT_GROUP_OFF, ERRBIT_TARGET_RANGE = 1, 2, 4, 8
 
 _vp = C.c_void_p

@@ -68,7 +68,7 @@ static int check_params(const awr_params* p) {
     if (p->flags & ~(uint32_t)(AWR_FLAG_SAMPLE_STD | AWR_FLAG_SUCCESS_FILTER | AWR_FLAG_COUPLED |
                                AWR_FLAG_SKIP_UNIFORM))
         return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_E16) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER_RFS) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -94,6 +94,7 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool 
                           bool backward = true) {
     if (requested == AWR_KERNEL_FWD_STREAM)                   // forward only, bf16, 16-byte units
         return (!backward && rows_fwd_supported(V, ld, dtype)) ? AWR_KERNEL_FWD_STREAM : -1;
+    if (requested == AWR_KERNEL_CLUSTER_RFS) return rows_rfs_supported(V, ld, dtype) ? AWR_KERNEL_CLUSTER_RFS : -1;
     if (requested > AWR_KERNEL_CLUSTER_RF4) return -1;        // a fused-head kernel id
     // forward only: nothing has to stay on chip for a second pass, so whole rows are streamed
     // (config 1: see DESIGN.md section 4 for the measured rates of all the kernels on this path)
@@ -101,7 +102,8 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool 
         return AWR_KERNEL_FWD_STREAM;
     // token_entropy is produced by the generic and the register-file kernels
     if (want_entropy && requested == AWR_KERNEL_CLUSTER) return -1;
-    if (want_entropy && requested == AWR_KERNEL_AUTO && V * 2 >= 65536 && !rows_rf_supported(V, ld, dtype))
+    if (want_entropy && requested == AWR_KERNEL_AUTO && V * 2 >= 65536 && !rows_rf_supported(V, ld, dtype) &&
+        !rows_rfs_supported(V, ld, dtype))
         return AWR_KERNEL_GENERIC;
     const bool ok = rows_cluster_supported(V, ld, dtype);
     const bool ok_rf = rows_rf_supported(V, ld, dtype);
@@ -111,6 +113,7 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool 
     if (requested == AWR_KERNEL_GENERIC) return AWR_KERNEL_GENERIC;
     // auto: the cluster kernels pay off once a row is a sizeable fraction of shared memory
     if (V * 2 < 65536) return AWR_KERNEL_GENERIC;
+    if (rows_rfs_supported(V, ld, dtype)) return AWR_KERNEL_CLUSTER_RFS;
     if (ok_rf) return AWR_KERNEL_CLUSTER_RF;
     return ok ? AWR_KERNEL_CLUSTER : AWR_KERNEL_GENERIC;
 }
@@ -118,6 +121,7 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool 
 static cudaError_t launch_rows(int kernel, const RowArgs& a, int dtype, int num_sms,
                                cudaStream_t st) {
     if (kernel == AWR_KERNEL_FWD_STREAM) return launch_rows_fwd(a, num_sms, st);
+    if (kernel == AWR_KERNEL_CLUSTER_RFS) return launch_rows_rfs(a, num_sms, st);
     if (kernel == AWR_KERNEL_CLUSTER_RF) return launch_rows_rf(a, num_sms, 2, st);
     if (kernel == AWR_KERNEL_CLUSTER_RF4) return launch_rows_rf(a, num_sms, 4, st);
     if (kernel == AWR_KERNEL_CLUSTER) return launch_rows_cluster(a, num_sms, st);

@@ -151,6 +151,17 @@ __device__ __forceinline__ void st_cluster_f32(uint32_t local_addr, uint32_t ran
                  : "memory");
 }
 
+// 16 bytes to the shared memory of CTA `rank` of the cluster, completing 16 bytes of the transaction
+// count of the mbarrier at `local_bar`'s offset in THAT CTA: data and signal travel together, so
+// the sender needs no fence and no barrier (both addresses are CTA-local, mapped here).
+__device__ __forceinline__ void st_async_f32x4(uint32_t local_addr, uint32_t local_bar, uint32_t rank,
+                                               float a, float b, float c, float d) {
+    asm volatile(
+        "st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];"
+        ::"r"(map_to_cta(local_addr, rank)), "f"(a), "f"(b), "f"(c), "f"(d), "r"(map_to_cta(local_bar, rank))
+        : "memory");
+}
+
 // ------------------------------------------------------------------ 16-byte shared / global accesses
 __device__ __forceinline__ void lds128(uint32_t (&v)[4], uint32_t addr) {
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"

@@ -78,7 +78,7 @@ def test_host_side_status_codes():
     assert f(C.byref(B), C.byref(P), C.byref(Oo), None, 0, None) == _abi.AWR_ERR_DTYPE
     B.logits_dtype = 0
     for bad in (dict(k_norm=0.0), dict(clip_eps=1.0), dict(clip_eps=-0.1), dict(normalizer=3),
-                dict(flags=16), dict(dual_clip_c=float("nan")), dict(kernel=10),
+                dict(flags=16), dict(dual_clip_c=float("nan")), dict(kernel=11),
                 dict(stale_cap=float("nan"))):
         Q = _abi.awr_params(10.0, 0.2, 0.0, 1.0, 0.0, 0, 0, 0)
         for k, v in bad.items():
@@ -88,7 +88,7 @@ def test_host_side_status_codes():
     assert lib.awr_status_string(_abi.AWR_ERR_ARCH).decode().startswith("device is not sm_100")
     assert lib.awr_workspace_bytes(1000, 151936, 10, 8, 2) % 256 == 0
     assert lib.awr_workspace_bytes(-1, 1, 1, 1, 1) == 0
-    assert lib.awr_select_kernel(151936, 151936, 0) in (_abi.KERNEL_CLUSTER, _abi.KERNEL_CLUSTER_RF)
+    assert lib.awr_select_kernel(151936, 151936, 0) == _abi.KERNEL_CLUSTER_RFS
     assert lib.awr_select_kernel(151936, 151936, 1) == _abi.KERNEL_GENERIC
     assert lib.awr_select_kernel(1024, 1024, 0) == _abi.KERNEL_GENERIC
 

@@ -109,7 +109,7 @@ def test_full_size_sampled(cfg, in_place, norm):
     print("config %d: oracle forward over all %d rows in %.1f s on %d host cores" % (
         cfg, n_tok, time.perf_counter() - t0, len(os.sched_getaffinity(0))))
 
-    assert A.select_kernel(V, batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RF
+    assert A.select_kernel(V, batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RFS
     kw = dict(dlogits=batch["logits"]) if in_place else {}
     if in_place:
         ref_lp = None

@@ -72,7 +72,7 @@ CLUSTER_SHAPES = [(151_936, 151_936), (40_000, 40_008), (32_768, 32_768), (65_54
                   (131_072, 131_072)]
 
 
-CLUSTER_KERNELS = [A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4]
+CLUSTER_KERNELS = [A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4, A.KERNEL_CLUSTER_RFS]
 
 
 @pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
@@ -266,7 +266,7 @@ def test_thinking_shapes_workload(horizon):
     if horizon == 20:      # 256 trajectories, 1 + Poisson(11.5) steps for failures: the cap binds
         assert (steps == 20).any(), "the horizon-20 cap should bind for some failed trajectory"
     batch = W.make_batch(w, seed=71 + horizon, device=DEV)
-    assert A.select_kernel(batch["V"], batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RF
+    assert A.select_kernel(batch["V"], batch["ld"], torch.bfloat16) == A.KERNEL_CLUSTER_RFS
     P.full_check(batch, dual_clip_c=3.0)
     P.full_check(batch, normalizer=A.NORM_PER_TRAJ, flags=A.FLAG_SKIP_UNIFORM)
 
@@ -310,7 +310,7 @@ def test_dynamic_sampling_flag():
 
 @pytest.mark.parametrize("flags", [A.FLAG_SUCCESS_FILTER, A.FLAG_COUPLED,
                                    A.FLAG_SUCCESS_FILTER | A.FLAG_COUPLED])
-@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER_RF])
+@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RFS])
 def test_baseline_variants(flags, kernel):
     """the paper's two comparison losses by flag - RAFT++ (advantage =
     1[R > 0]; run at group size 1 as in :462 and at 4) and the coupled-ratio
@@ -362,6 +362,8 @@ def test_dual_clip(kernel, norm):
                                             (A.KERNEL_CLUSTER_RF, 151_936, torch.bfloat16),
                                             (A.KERNEL_CLUSTER_RF4, 151_936, torch.bfloat16),
                                             (A.KERNEL_CLUSTER_RF, 40_000, torch.bfloat16),
+                                            (A.KERNEL_CLUSTER_RFS, 151_936, torch.bfloat16),
+                                            (A.KERNEL_CLUSTER_RFS, 40_000, torch.bfloat16),
                                             (A.KERNEL_AUTO, 151_936, torch.bfloat16)])
 @pytest.mark.parametrize("backward", [True, False])
 def test_token_entropy(kernel, V, dtype, backward):
@@ -574,7 +576,8 @@ def test_register_file_kernels_random_shapes(V, ld, n_tok, seed):
     (fewer rows than clusters included), both cluster shapes, entropy on."""
     w = W.workload(3, n_groups=3, group_size=4, n_tok=max(n_tok, 12), V=V)
     batch = W.make_batch(w, seed=seed % 1000, device=DEV, ld=ld, masked_frac=0.05)
-    for kernel in (A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4):
+    kernels = [A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4] + ([A.KERNEL_CLUSTER_RFS] if V <= 153_600 else [])
+    for kernel in kernels:
         batch["params"]["kernel"] = kernel
         gpu, ora = P.full_check(batch, dual_clip_c=3.0)
     out = A.awr_loss_fwd(batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
@@ -633,6 +636,7 @@ def _zones_intact(buf, pad_e, n, pattern):
 
 @pytest.mark.parametrize("kernel,backward", [(A.KERNEL_GENERIC, True), (A.KERNEL_CLUSTER, True),
                                              (A.KERNEL_CLUSTER_RF, True), (A.KERNEL_CLUSTER_RF4, True),
+                                             (A.KERNEL_CLUSTER_RFS, True),
                                              (A.KERNEL_FWD_STREAM, False)])
 @pytest.mark.parametrize("V,ld", [(151_936, 151_936), (40_000, 40_008)])
 def test_red_zones_row_kernels(kernel, backward, V, ld):
