@@ -212,8 +212,13 @@ AWR_API size_t awr_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t ld, in
                                 int32_t n_steps, int32_t n_traj, int32_t n_groups);
 
 /* a5 (BASELINE.json config 4): hidden states + LM head instead of logits.  logits = hidden
- * [n_tok, K] x w_head, never written to memory, fp32 accumulation fed straight to the
- * log-sum-exp (A17).  Outputs dhidden = dS W^T and dw_head = H^T dS (bf16, overwritten). */
+ * [n_tok, K] x w_head are produced tile by tile in tensor memory and fed from there to the
+ * log-sum-exp with fp32 accumulation (A17); the full [n_tok, V] matrix never exists.  What the modes
+ * keep, for ONE row panel (<= 9,472 rows) at a time, between the panel's forward GEMM and its dS
+ * pass:  E16 (AUTO): bf16(exp(z - tile row max)), 2 bytes per logit of the panel, in the dS buffer;
+ * STORED: the fp32 logits of the panel (two buffers, a side stream);  HEAD_1CTA / HEAD_2CTA: nothing
+ * (the tile is recomputed, 8 K V instead of 6 K V flops per token).  awr_head_workspace_bytes()
+ * gives the bytes per mode.  Outputs dhidden = dS W^T and dw_head = H^T dS (bf16, overwritten). */
 typedef struct awr_head_batch {
     int64_t n_tok;
     int64_t V;
@@ -267,10 +272,10 @@ AWR_API int awr_loss_fwd_bwd_fused_head_host(const awr_head_batch* host_batch, c
 AWR_API size_t awr_head_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
                                      int32_t n_traj, int32_t n_groups, int32_t kernel);
 
-/* Note: in the stored-logits mode the call forks the dS pass of each row panel onto a library-owned
- * side stream (created once per device) and joins it back before the panel's dhidden GEMM; from
- * the caller's point of view all work is still ordered on `stream`, and the call can be captured
- * into a CUDA graph.  Workspace: two fp32 logits panels.
+/* Note: only AWR_KERNEL_HEAD_2CTA_STORED uses a side stream: it forks the dS pass of each row panel
+ * onto a library-owned side stream (pool keyed by the caller's stream, see "Thread safety / state")
+ * and joins it back before the panel's dhidden GEMM; from the caller's point of view all work is
+ * still ordered on `stream`, and the call can be captured into a CUDA graph.
  *
  * Kernel launches one awr_loss_fwd_bwd_fused_head call enqueues for this shape. */
 AWR_API int awr_head_launches_per_call(int64_t n_tok, int64_t V, int64_t K, int32_t kernel);

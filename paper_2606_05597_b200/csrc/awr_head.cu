@@ -1,12 +1,16 @@
 // a5: fused LM-head variant (BASELINE.json config 4, readings A17).
 //
-//   logits Z = H W_head are produced tile by tile in tensor memory and never stored:
-//   pass F   Z tile -> per-row (max, sum exp) partials + target gather          (GEMM, kEpiLse)
-//   scalars  partials -> lse, l_t, ratio / clip / normalizer (a3), c_t           (one warp per row)
-//   per panel of P rows (P x V bf16 transient, 1.4 GB at the default P):
-//     pass G1  recompute the Z tile -> dS = c_t (softmax - onehot) in bf16       (GEMM, kEpiDs)
-//     pass G2  dhidden[panel] = dS W_head^T                                      (GEMM, kEpiStoreBf16)
-//     pass G3  dw_head += H[panel]^T dS   (fp32 running sum, bf16 at the end)    (GEMM, kEpiAccum)
+//   logits Z = H W_head are produced tile by tile in tensor memory; the full matrix never exists.
+//   Per panel of P <= 9,472 rows (E16 mode, the default; DESIGN.md section 5 for the other modes):
+//     pass F   Z tile -> per-row (max, sum exp) partials + target gather, and E = bf16(exp(z - tile
+//              row max)) into the dS panel (2 bytes per logit of the panel, 2.9 GB at the default P)
+//                                                                              (GEMM, kEpiLse16)
+//     scalars  partials -> lse, l_t, ratio / clip / normalizer (a3), c_t          (one warp per row)
+//     dS       E -> dS = c_t (softmax - onehot) in place, bf16                    (streaming pass)
+//     pass G2  dhidden[panel] = dS W_head^T                                       (GEMM, kEpiStoreBf16)
+//     pass G3  dw_head += H[panel]^T dS   (fp32 running sum, bf16 at the end)     (GEMM, kEpiAccum)
+//   Stored mode keeps the fp32 tile instead (kEpiLse + head_ds_kernel on a side stream); the
+//   recompute modes form dS with a second logits GEMM (kEpiDs).
 // Every GEMM is the tcgen05 kernel below; see awr_head_gemm.cuh for the engine.
 #include <mutex>
 

@@ -2,9 +2,10 @@
 //
 //   C[M, N] = A[M, Kc] * B[Kc, N],  bf16 x bf16 -> fp32 accumulators in tensor memory,
 //
-// with the epilogue applied to the accumulator tile while it is still on chip, so the logits
-// Z = H * W_head are never written to memory (reading A17: the fp32
-// accumulators go straight into the log-sum-exp).
+// with the epilogue applied to the accumulator tile while it is still on chip: the log-sum-exp of
+// Z = H * W_head is taken from the fp32 accumulators in tensor memory (reading
+// A17); what an epilogue writes out of the tile besides the per-row partials depends on the mode
+// (nothing / bf16 exp(z - max) / the fp32 tile of one row panel: awr_head.cu).
 //
 // One persistent CTA per SM, 256 threads, warp-specialised:
 //   warp 0    TMA producer: cp.async.bulk.tensor (128-byte swizzle) into a smem ring
