@@ -143,9 +143,13 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
             mbar_wait(stats_full0 + 8u * par, ph2);
             const bool mine = lane < 2 * kSvConsumers;
             const float4 st = ctrl->stats[par][mine ? lane : 0];
-            float M = mine ? st.x : -INFINITY;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(kFull, M, o));
+            // max over the warp in ONE instruction: floats order like their bits once the negative
+            // ones are flipped (this chain is on the critical path of every data warp of the cluster)
+            int mi = __float_as_int(mine ? st.x : -INFINITY);
+            mi ^= (mi >> 31) & 0x7fffffff;
+            mi = __reduce_max_sync(kFull, mi);
+            mi ^= (mi >> 31) & 0x7fffffff;
+            const float M = __int_as_float(mi);
             const float rs = (!mine || st.x == -INFINITY) ? 0.f : ex2_approx((st.x - M) * kLog2e);
             float S = st.y * rs;
             float SZ = ENT ? st.z * rs : 0.f;
@@ -268,7 +272,7 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 s += __shfl_xor_sync(kFull, s, o);
-                if (want_ent) accz += __shfl_xor_sync(kFull, accz, o);
+                if (ENT) accz += __shfl_xor_sync(kFull, accz, o);     // merged only if it is an output
             }
             // ---- exchange: (m_w, s_w, sz_w) to both CTAs, data and signal in one st.async each
             if (lane < 2)
