@@ -199,51 +199,60 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
         const int my_unit0 = warp * 32 + lane;                           // unit of round 0
         uint32_t v[NU][4];
         uint32_t gpiece = 0;
-        int y_n = a.target_ids[cluster];          // target id of the next row, fetched a row ahead
-        int it = 0;
-        for (int row = cluster; row < n_tok; row += nc, ++it) {
-            const int par = it & 1;
-            const uint32_t ph1 = (uint32_t)it & 1u, ph2 = (uint32_t)(it >> 1) & 1u;
-            const int y = y_n;
-            if (row + nc < n_tok) y_n = a.target_ids[row + nc];
-            // The target entry is left out of the (max, sum) state (token_scalars works from
-            // lse_rest): the thread that holds it masks it to -inf on the way to registers.
+        uint32_t mx2 = kSvNegInf2;
+
+        // One ring slot of row index `it` -> registers (rounds [10 s, 10 s + 10)), target entry masked
+        // to -inf (token_scalars works from lse_rest), packed running max; then the slot is released.
+        auto load_slot = [&](int s, int it, int y_round, int y_word, uint32_t y_keep) {
+            const bool have = s * kSvSlotRounds < nr;                                   // warp-uniform
+            if (have) mbar_wait(full0 + 8u * s, (uint32_t)it & 1u);
+            const uint32_t src = ring + (uint32_t)s * kSvSlotBytes + my_off;
+#pragma unroll
+            for (int kk = 0; kk < kSvSlotRounds; ++kk) {
+                const int k = s * kSvSlotRounds + kk;
+                if (k < NU) {
+                    if (k * kSvRoundUnits + my_unit0 < half_units) {
+                        lds128(v[k], src + (uint32_t)kk * kSvRoundBytes);
+                    } else {
+                        v[k][0] = v[k][1] = v[k][2] = v[k][3] = kSvNegInf2;
+                    }
+                    if (k == y_round) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            v[k][j] = (j == y_word) ? ((v[k][j] & y_keep) | (kSvNegInf2 & ~y_keep)) : v[k][j];
+                    }
+                    mx2 = max_bf16x2(mx2, max_bf16x2(max_bf16x2(v[k][0], v[k][1]), max_bf16x2(v[k][2], v[k][3])));
+                }
+            }
+            if (have) {
+                __syncwarp();                                 // the slot has been read out by the warp
+                if (lane == 0) mbar_arrive(empty0 + 8u * s);
+            }
+        };
+        // where the target of a row sits for this thread: its round (or -1), word and the OTHER half
+        auto locate = [&](int y, int& y_round, int& y_word, uint32_t& y_keep) {
             const bool valid = (y >= 0) && (y < a.V);
             const int y_unit = valid ? (y >> 3) - half_base : -1;                       // unit inside this half
             const bool holder = y_unit >= 0 && y_unit < half_units && (y_unit % kSvRoundUnits) == my_unit0;
-            const int y_round = holder ? y_unit / kSvRoundUnits : -1;
-            const int y_word = (y & 7) >> 1;
-            const uint32_t y_keep = (y & 1) ? 0x0000ffffu : 0xffff0000u;                // the OTHER half
+            y_round = holder ? y_unit / kSvRoundUnits : -1;
+            y_word = (y & 7) >> 1;
+            y_keep = (y & 1) ? 0x0000ffffu : 0xffff0000u;
+        };
 
-            // ---- pass 0: ring -> registers, packed running max
-            uint32_t mx2 = kSvNegInf2;
+        int y = a.target_ids[cluster];
+        int y_round, y_word;
+        uint32_t y_keep;
+        locate(y, y_round, y_word, y_keep);
 #pragma unroll
-            for (int s = 0; s < NCH; ++s) {
-                const bool have = s * kSvSlotRounds < nr;                               // warp-uniform
-                if (have) mbar_wait(full0 + 8u * s, ph1);
-                const uint32_t src = ring + (uint32_t)s * kSvSlotBytes + my_off;
-#pragma unroll
-                for (int kk = 0; kk < kSvSlotRounds; ++kk) {
-                    const int k = s * kSvSlotRounds + kk;
-                    if (k < NU) {
-                        if (k * kSvRoundUnits + my_unit0 < half_units) {
-                            lds128(v[k], src + (uint32_t)kk * kSvRoundBytes);
-                        } else {
-                            v[k][0] = v[k][1] = v[k][2] = v[k][3] = kSvNegInf2;
-                        }
-                        if (k == y_round) {
-#pragma unroll
-                            for (int j = 0; j < 4; ++j)
-                                v[k][j] = (j == y_word) ? ((v[k][j] & y_keep) | (kSvNegInf2 & ~y_keep)) : v[k][j];
-                        }
-                        mx2 = max_bf16x2(mx2, max_bf16x2(max_bf16x2(v[k][0], v[k][1]), max_bf16x2(v[k][2], v[k][3])));
-                    }
-                }
-                if (have) {
-                    __syncwarp();                             // the slot has been read out by the warp
-                    if (lane == 0) mbar_arrive(empty0 + 8u * s);
-                }
-            }
+        for (int s = 0; s < NCH; ++s) load_slot(s, 0, y_round, y_word, y_keep);     // pass 0 of the first row
+
+        int it = 0;
+        for (int row = cluster; row < n_tok; row += nc, ++it) {
+            const int par = it & 1;
+            const uint32_t ph2 = (uint32_t)(it >> 1) & 1u;
+            const bool have_next = row + nc < n_tok;
+            const int y_nx = have_next ? a.target_ids[row + nc] : -1;     // in flight behind the exp pass
+
             float m = fmaxf(bf16_lo(mx2), bf16_hi(mx2));
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(kFull, m, o));
@@ -279,14 +288,21 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
                 st_async_f32x4(smem_u32(&ctrl->stats[par][(int)rank * kSvConsumers + warp]),
                                stats_full0 + 8u * par, (uint32_t)lane, m, s, accz, 0.f);
 
+            // where the next row's target sits (for its pass 0, interleaved below)
+            int yn_round, yn_word;
+            uint32_t yn_keep;
+            locate(y_nx, yn_round, yn_word, yn_keep);
+
             // ---- a3 runs on the service warp; wait for (c_t, lse, c_t (p_y - 1))
             mbar_wait(ready0 + 8u * par, ph2);
             const float4 ri = ctrl->rowinfo[par];
-            if (!backward) continue;
 
-            // ---- pass 2 (a4): dlogits = e * (c_t exp(m - lse)) through the staging buffers.  e was
-            // taken relative to m (0 if the part held nothing finite); c_t = 0 (masked, zero
-            // advantage, clip triggered): F = +0 and e >= 0 give all-bits-zero products
+            // ---- pass 2 (a4): dlogits = e * (c_t exp(m - lse)) through the staging buffers, with pass
+            // 0 of the NEXT row slot by slot in between: after ten rounds both staging buffers are
+            // full and the warp would wait for the TMA store to drain one (32 B/clk); the registers
+            // of those ten rounds are free, so the next row's first ring slot is moved into them
+            // meanwhile.  e was taken relative to m (0 if the part held nothing finite); c_t = 0
+            // (masked, zero advantage, clip triggered): F = +0 and e >= 0 give all-bits-zero products
             const float F = ri.x == 0.f ? 0.f : ri.x * ex2_approx(fmaf(-ri.y, kLog2e, -nref));
             const __nv_bfloat16 fh = __float2bfloat16_rn(F);
             const __nv_bfloat16 fl = __float2bfloat16_rn(F - __bfloat162float(fh));
@@ -295,33 +311,42 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
             const uint32_t gy_bits = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(ri.z));
             const uint32_t gy2 = (y & 1) ? (gy_bits << 16) : gy_bits;
             const int y_patch = ri.x != 0.f ? y_round : -1;
+            mx2 = kSvNegInf2;
 #pragma unroll
-            for (int k = 0; k < NU; ++k) {
-                if (k < nr) {                                                 // warp-uniform
-                    const int kk = k % kSvStageRounds;
-                    const uint32_t gp = gpiece + (uint32_t)(k / kSvStageRounds);
-                    const uint32_t buf = stage + (gp & 1u) * kSvStageBytes;
-                    if (kk == 0) mbar_wait(sfree0 + 8u * (gp & 1u), ((gp >> 1) & 1u) ^ 1u);
-                    uint4 o;
-                    o.x = fma_bf16x2(v[k][0], Fh, mul_bf16x2(v[k][0], Fl));
-                    o.y = fma_bf16x2(v[k][1], Fh, mul_bf16x2(v[k][1], Fl));
-                    o.z = fma_bf16x2(v[k][2], Fh, mul_bf16x2(v[k][2], Fl));
-                    o.w = fma_bf16x2(v[k][3], Fh, mul_bf16x2(v[k][3], Fl));
-                    if (k == y_patch) {                                       // target entry: c (p_y - 1)
-                        o.x = y_word == 0 ? ((o.x & y_keep) | gy2) : o.x;
-                        o.y = y_word == 1 ? ((o.y & y_keep) | gy2) : o.y;
-                        o.z = y_word == 2 ? ((o.z & y_keep) | gy2) : o.z;
-                        o.w = y_word == 3 ? ((o.w & y_keep) | gy2) : o.w;
-                    }
-                    sts128(buf + (uint32_t)kk * kSvRoundBytes + my_off, o);
-                    if (kk == kSvStageRounds - 1 || k == nr - 1) {
-                        fence_proxy_async();                                  // generic writes -> TMA read
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(sfull0 + 8u * (gp & 1u));
+            for (int sl = 0; sl < NCH; ++sl) {
+                if (backward) {
+#pragma unroll
+                    for (int kk2 = 0; kk2 < kSvSlotRounds; ++kk2) {
+                        const int k = sl * kSvSlotRounds + kk2;
+                        if (k < NU && k < nr) {                                   // k < nr: warp-uniform
+                            const int kk = k % kSvStageRounds;
+                            const uint32_t gp = gpiece + (uint32_t)(k / kSvStageRounds);
+                            const uint32_t buf = stage + (gp & 1u) * kSvStageBytes;
+                            if (kk == 0) mbar_wait(sfree0 + 8u * (gp & 1u), ((gp >> 1) & 1u) ^ 1u);
+                            uint4 o;
+                            o.x = fma_bf16x2(v[k][0], Fh, mul_bf16x2(v[k][0], Fl));
+                            o.y = fma_bf16x2(v[k][1], Fh, mul_bf16x2(v[k][1], Fl));
+                            o.z = fma_bf16x2(v[k][2], Fh, mul_bf16x2(v[k][2], Fl));
+                            o.w = fma_bf16x2(v[k][3], Fh, mul_bf16x2(v[k][3], Fl));
+                            if (k == y_patch) {                                   // target entry: c (p_y - 1)
+                                o.x = y_word == 0 ? ((o.x & y_keep) | gy2) : o.x;
+                                o.y = y_word == 1 ? ((o.y & y_keep) | gy2) : o.y;
+                                o.z = y_word == 2 ? ((o.z & y_keep) | gy2) : o.z;
+                                o.w = y_word == 3 ? ((o.w & y_keep) | gy2) : o.w;
+                            }
+                            sts128(buf + (uint32_t)kk * kSvRoundBytes + my_off, o);
+                            if (kk == kSvStageRounds - 1 || k == nr - 1) {
+                                fence_proxy_async();                              // generic writes -> TMA read
+                                __syncwarp();
+                                if (lane == 0) mbar_arrive(sfull0 + 8u * (gp & 1u));
+                            }
+                        }
                     }
                 }
+                if (have_next) load_slot(sl, it + 1, yn_round, yn_word, yn_keep);
             }
-            gpiece += (uint32_t)npieces;
+            if (backward) gpiece += (uint32_t)npieces;
+            y = y_nx; y_round = yn_round; y_word = yn_word; y_keep = yn_keep;
         }
     }
     cluster_arrive();     // nobody leaves while the peer may still send to its shared memory
