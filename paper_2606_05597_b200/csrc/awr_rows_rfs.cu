@@ -16,7 +16,10 @@
 //     speed (128 B/clk) and go on; the service lane hands each full buffer to a TMA bulk store.
 //     An SM writes to L2 at 32 B/clk whatever the instruction (measured for per-lane stores and for
 //     TMA stores alike), so the 148 KB of a row half need 4.7 k clocks of that port; what staging
-//     buys is that the last 75 KB drain while the warps are already in the next row.
+//     buys is that the last 75 KB drain while the warps are already in the next row - and the
+//     first 75 KB too: the waits for a free staging buffer are filled with pass 0 (ring ->
+//     registers, max) of the NEXT row, slot by slot, into the registers whose gradient has just
+//     been staged.  With that the kernel is HBM-bound (config 1: 3.87 ms, 0.99 of the copy peak).
 //   * Exchange: every consumer warp sends its (max, sum[, sum e z]) with st.async to BOTH CTAs; the
 //     16 bytes complete a transaction count on the receiver's mbarrier - no cluster barrier, no
 //     fence.  The service warp of each CTA merges the 30 states, evaluates a3 once (header loads
