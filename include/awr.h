@@ -71,7 +71,9 @@ typedef enum awr_status {
     AWR_ERR_PARAM = -5,     /* k_norm <= 0, clip_eps outside [0,1), NaN scalars, bad enum */
     AWR_ERR_WORKSPACE = -6, /* workspace NULL, misaligned (256 B) or too small */
     AWR_ERR_ARCH = -7,      /* current device is not sm_100 */
-    AWR_ERR_CUDA = -8       /* a CUDA runtime call / launch failed (cudaGetLastError cleared) */
+    AWR_ERR_CUDA = -8,      /* a CUDA runtime call / launch failed (cudaGetLastError cleared) */
+    AWR_ERR_STATIC_LIMIT = -9 /* awr_loss_fwd_bwd_static: the batch needs more scratch than
+                                 AWR_STATIC_WS_BYTES; use awr_loss_fwd_bwd with a workspace */
 } awr_status;
 
 enum { AWR_DTYPE_BF16 = 0, AWR_DTYPE_F32 = 1 };
@@ -198,6 +200,25 @@ AWR_API int awr_group_advantage(const float* rewards, const int32_t* group_off, 
 /* Bytes of device workspace awr_loss_fwd_bwd / awr_loss_fwd need (256-B aligned pointer). */
 AWR_API size_t awr_workspace_bytes(int64_t n_tok, int64_t V, int32_t n_steps, int32_t n_traj,
                            int32_t n_groups);
+
+/* awr_loss_fwd_bwd for callers that cannot allocate (code under CUDA-graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the same checks, kernels and results, with the workspace in
+ * a fixed device array inside the library instead of a caller buffer.  The call itself never
+ * allocates: no cudaMalloc / cudaFree / allocating library routine; inputs and outputs are still
+ * the caller's.
+ *   Limit: awr_workspace_bytes(n_tok, V, n_steps, n_traj, n_groups) <= AWR_STATIC_WS_BYTES
+ *   (1 MiB: 8 + 8 bytes per trajectory and 9 bytes per token, each array rounded up to 256 B -
+ *   e.g. 110,000 tokens with 1,024 trajectories); a larger batch returns AWR_ERR_STATIC_LIMIT and
+ *   nothing is launched.  The array costs 1 MiB of device memory on every GPU that loads the
+ *   library, until the process exits.
+ *   Sharing: every call on a device uses the SAME array, and it keeps the previous call's
+ *   contents; the part that must start at zero (error word, advantages, trajectory scales) is
+ *   cleared on `stream` at the start of every call.  Two calls that overlap on one GPU (different
+ *   streams, or several host threads) RACE on it: order them on one stream or with events.
+ *   Back-to-back calls on one stream are safe. */
+#define AWR_STATIC_WS_BYTES ((size_t)1 << 20)
+AWR_API int awr_loss_fwd_bwd_static(const awr_batch* batch, const awr_params* params,
+                                    const awr_outputs* out, void* stream);
 
 /* Same path with HOST buffers: every pointer in `batch` and `out` is a host pointer (pinned
  * memory gives full PCIe speed; pageable works).  Rows are staged through `dev_workspace` in

@@ -16,6 +16,8 @@ from . import build as _build
 AWR_OK = 0
 AWR_ERR_NULL, AWR_ERR_SHAPE, AWR_ERR_DTYPE, AWR_ERR_ALIGN = -1, -2, -3, -4
 AWR_ERR_PARAM, AWR_ERR_WORKSPACE, AWR_ERR_ARCH, AWR_ERR_CUDA = -5, -6, -7, -8
+AWR_ERR_STATIC_LIMIT = -9
+STATIC_WS_BYTES = 1 << 20
 DTYPE_BF16, DTYPE_F32 = 0, 1
 NORM_CONST_K, NORM_PER_TRAJ = 0, 1
 FLAG_SAMPLE_STD = 1
@@ -76,6 +78,8 @@ SYMBOLS = {
                                    C.POINTER(awr_outputs), _vp, C.c_size_t, _vp]),
     "awr_loss_fwd": (C.c_int, [C.POINTER(awr_batch), C.POINTER(awr_params),
                                C.POINTER(awr_outputs), _vp, C.c_size_t, _vp]),
+    "awr_loss_fwd_bwd_static": (C.c_int, [C.POINTER(awr_batch), C.POINTER(awr_params),
+                                          C.POINTER(awr_outputs), _vp]),
     "awr_group_advantage": (C.c_int, [_vp, _vp, C.c_int32, C.c_int32, C.c_uint32, _vp, _vp]),
     "awr_workspace_bytes": (C.c_size_t, [C.c_int64, C.c_int64, C.c_int32, C.c_int32, C.c_int32]),
     "awr_loss_fwd_bwd_host": (C.c_int, [C.POINTER(awr_batch), C.POINTER(awr_params),

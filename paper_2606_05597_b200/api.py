@@ -171,6 +171,46 @@ def awr_loss_fwd_bwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off,
                     rewards, backward=True, **kw).run()
 
 
+class StaticLossCall:
+    """include/awr.h awr_loss_fwd_bwd_static: awr_loss_fwd_bwd with the library's fixed 1 MiB
+    device array as workspace (``STATIC_WS_BYTES``), for callers that cannot allocate.  Outputs
+    are the caller's (``out=`` / ``dlogits=``; allocated here, once, if not given); ``run()``
+    allocates nothing.  Every call on a GPU shares the array: calls that overlap on the GPU race."""
+
+    def __init__(self, logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off,
+                 rewards, *, V=None, dlogits=None, out=None, want=OPTIONAL_OUTPUTS, **params):
+        self.lib = load()
+        self.batch = _batch_struct(logits, target_ids, behave_lp, prox_lp, step_off, traj_off,
+                                   group_off, rewards, V)
+        self.params = make_params(**params)
+        self.device = logits.device
+        n_tok, n_traj = self.batch.n_tok, self.batch.n_traj
+        self.out = out if out is not None else alloc_outputs(n_tok, n_traj, self.device, None, want)
+        if dlogits is not None:
+            if dlogits.dtype != logits.dtype or dlogits.stride() != logits.stride():
+                raise TypeError("dlogits must match logits in dtype and strides")
+            self.out["dlogits"] = dlogits
+        elif "dlogits" not in self.out:
+            self.out["dlogits"] = torch.empty_strided(logits.shape, logits.stride(),
+                                                      dtype=logits.dtype, device=self.device)
+        self.outs = _out_struct(self.out)
+        self._keep = (logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off,
+                      rewards)
+
+    def run(self, stream=None):
+        check(self.lib.awr_loss_fwd_bwd_static(C.byref(self.batch), C.byref(self.params),
+                                               C.byref(self.outs), _stream_ptr(stream, self.device)),
+              "awr_loss_fwd_bwd_static")
+        return self.out
+
+
+def awr_loss_fwd_bwd_static(logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off,
+                            rewards, **kw):
+    """include/awr.h awr_loss_fwd_bwd_static (no workspace argument, no allocation in the call)."""
+    return StaticLossCall(logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off,
+                          rewards, **kw).run()
+
+
 def awr_loss_fwd(logits, target_ids, behave_lp, prox_lp, step_off, traj_off, group_off, rewards,
                  **kw):
     """include/awr.h awr_loss_fwd (no gradient; each row is read once)."""

@@ -204,6 +204,27 @@ static int run(const awr_batch* b, const awr_params* p, const awr_outputs* o, vo
     return AWR_OK;
 }
 
+// ---------------------------------------------------------------- no-allocation entry point
+// Scratch of awr_loss_fwd_bwd_static: one fixed array per GPU that loads the library.  In host code
+// the name is only a handle of the symbol, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_static_ws[AWR_STATIC_WS_BYTES];
+
+static int static_workspace(void** out) {
+    constexpr int kMax = 64;
+    static void* cache[kMax];                 // per device ordinal; written once with one value
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return AWR_ERR_CUDA; }
+    void* ptr = (dev >= 0 && dev < kMax) ? __atomic_load_n(&cache[dev], __ATOMIC_ACQUIRE) : nullptr;
+    if (!ptr) {
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_ws);
+        if (e != cudaSuccess || !ptr) { cudaGetLastError(); return AWR_ERR_CUDA; }
+        if (dev >= 0 && dev < kMax) __atomic_store_n(&cache[dev], ptr, __ATOMIC_RELEASE);
+    }
+    *out = ptr;
+    return AWR_OK;
+}
+
 }  // namespace awr
 
 using namespace awr;
@@ -223,6 +244,8 @@ const char* awr_status_string(int s) {
         case AWR_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
         case AWR_ERR_ARCH: return "device is not sm_100 (B200); no fallback exists";
         case AWR_ERR_CUDA: return "CUDA runtime error";
+        case AWR_ERR_STATIC_LIMIT:
+            return "batch needs more scratch than AWR_STATIC_WS_BYTES (1 MiB): use awr_loss_fwd_bwd with a workspace";
         default: return "unknown status";
     }
 }
@@ -243,6 +266,21 @@ int awr_launches_per_call(void) { return 4; }
 int awr_loss_fwd_bwd(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
                      void* workspace, size_t workspace_bytes, void* stream) {
     return run(batch, params, out, workspace, workspace_bytes, stream, true);
+}
+
+int awr_loss_fwd_bwd_static(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
+                            void* stream) {
+    if (!batch || !params || !out) return AWR_ERR_NULL;
+    const int rc = check_segments(batch->n_tok, batch->n_steps, batch->n_traj, batch->n_groups);
+    if (rc) return rc;
+    if (awr_workspace_bytes(batch->n_tok, batch->V, batch->n_steps, batch->n_traj, batch->n_groups) >
+        AWR_STATIC_WS_BYTES)
+        return AWR_ERR_STATIC_LIMIT;
+    void* ws = nullptr;
+    const int rs = static_workspace(&ws);
+    if (rs) return rs;
+    // run() clears the zero-initialised prefix of the workspace on `stream` before anything reads it
+    return run(batch, params, out, ws, AWR_STATIC_WS_BYTES, stream, true);
 }
 
 int awr_loss_fwd(const awr_batch* batch, const awr_params* params, const awr_outputs* out,
