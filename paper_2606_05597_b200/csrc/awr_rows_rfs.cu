@@ -54,12 +54,15 @@ struct SvCtrl {
     uint64_t stats_full[2];                              // [row parity] 30 x 16 bytes have arrived
     uint64_t row_ready[2];                               // [row parity] rowinfo is valid
     float4 stats[2][2 * kSvConsumers + 2];               // [row parity][cluster-wide warp] (m, s, sz, -)
-    float4 rowinfo[2];                                   // [row parity] (c_t, lse, c_t (p_y - 1), y as bits)
+    float4 rowinfo[2];                                   // [row parity] (c_t, lse, c_t (p_y - 1), place of the NEXT row's target)
 };
 static_assert(sizeof(SvCtrl) <= kSvCtrlBytes, "control block");
 
 struct SvPlan {
     int half_units[2];   // 16-byte units of the row held by CTA rank 0 / 1
+    int half_base[2];    // first unit of each half
+    int nr[2];           // rounds of each half: ceil(half_units / 480) (NU or NU - 1)
+    int npieces[2];      // staging buffers per row of each half: ceil(nr / 5)
     int num_clusters;
 };
 
@@ -77,10 +80,12 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
     const int warp = tid >> 5;
     const uint32_t rank = cluster_ctarank();
     const int cluster = (int)cluster_id_x();
-    const int half_units = p.half_units[rank];
-    const int half_base = rank ? p.half_units[0] : 0;                      // first unit of this half
-    const int nr = (half_units + kSvRoundUnits - 1) / kSvRoundUnits;       // rounds of THIS half (<= NU)
-    const int npieces = (nr + kSvStageRounds - 1) / kSvStageRounds;        // staging buffers per row
+    // derived sizes come from the plan: kernel parameters cost no registers (selects, not indexing,
+    // so that the parameter struct is not copied to local memory)
+    const int half_units = rank ? p.half_units[1] : p.half_units[0];
+    const int half_base = rank ? p.half_base[1] : p.half_base[0];          // first unit of this half
+    const int nr = rank ? p.nr[1] : p.nr[0];                               // rounds of THIS half (<= NU)
+    const int npieces = rank ? p.npieces[1] : p.npieces[0];                // staging buffers per row
     const uint32_t ring = smem_u32(smem + kSvCtrlBytes);
     const uint32_t stage = ring + 2u * kSvSlotBytes;
     const uint32_t full0 = smem_u32(&ctrl->full[0]), empty0 = smem_u32(&ctrl->empty[0]);
@@ -107,249 +112,318 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
 
     if (warp == kSvConsumers) {
         // =============================================================== service warp
+        // An event loop over the three things the data warps hand over - a ring slot read out, the
+        // 30 (max, sum) states of a row, a full staging buffer - so that a refill is issued the moment
+        // its slot is free, whatever the stores are doing (polling with mbarrier.test_wait; the tests
+        // are taken by the whole warp on one address and are warp-uniform).
         const uint8_t* lbase = reinterpret_cast<const uint8_t*>(a.logits) + (int64_t)half_base * 16;
         uint8_t* gbase = reinterpret_cast<uint8_t*>(a.dlogits) + (int64_t)half_base * 16;
-        auto load_slot = [&](int s, int row) {            // lane 0: one bulk copy fills the slot
+        const int nrows = (n_tok - cluster + nc - 1) / nc;            // rows of this cluster
+        auto issue_load = [&](int s, int j) {                          // lane 0: one bulk copy fills the slot
             const int u0 = s * kSvSlotRounds * kSvRoundUnits;
             const int units = min(kSvSlotRounds * kSvRoundUnits, half_units - u0);
             if (lane == 0 && units > 0) {
                 mbar_expect_tx(full0 + 8u * s, (uint32_t)units * 16u);
-                bulk_load(ring + (uint32_t)s * kSvSlotBytes, lbase + (int64_t)row * row_bytes + (int64_t)u0 * 16,
+                bulk_load(ring + (uint32_t)s * kSvSlotBytes,
+                          lbase + (int64_t)(cluster + j * nc) * row_bytes + (int64_t)u0 * 16,
                           (uint32_t)units * 16u, full0 + 8u * s);
             }
         };
+        int ld_j[NCH];                                    // next row index to load into each slot
 #pragma unroll
-        for (int s = 0; s < NCH; ++s) load_slot(s, cluster);
+        for (int s = 0; s < NCH; ++s) {
+            issue_load(s, 0);
+            ld_j[s] = (s * kSvSlotRounds < nr) ? 1 : nrows;           // a slot this half never uses
+        }
         RowHeader h, hn;
         bool valid = false, validn = false;
-        if (lane == 0) hn = load_row_header(a, cluster, validn, true);
+        int yq = -1;                                      // lane 0: target of the row after the next a3
+        if (lane == 0) {
+            hn = load_row_header(a, cluster, validn, true);
+            if (nrows > 1) yq = a.target_ids[cluster + nc];
+            mbar_expect_tx(stats_full0, 2u * kSvConsumers * 16u);
+            if (nrows > 1) mbar_expect_tx(stats_full0 + 8u, 2u * kSvConsumers * 16u);
+        }
+        int a3_j = 0;                                     // next row index to merge
+        int st_j = backward ? 0 : nrows, st_pc = 0;       // next staging buffer to store: row index, piece
         uint32_t gpiece = 0;                              // staging buffers handed to the TMA so far
-        int it = 0;
-        for (int row = cluster; row < n_tok; row += nc, ++it) {
-            const int par = it & 1;
-            const uint32_t ph2 = (uint32_t)(it >> 1) & 1u;      // phase of the per-parity barriers
-            h = hn; valid = validn;
-            const int next = row + nc;
-            if (lane == 0) {
-                mbar_expect_tx(stats_full0 + 8u * par, 2u * kSvConsumers * 16u);
-                if (next < n_tok) hn = load_row_header(a, next, validn, true);   // in flight behind this row
-            }
-            // ---- ring: refill each slot with the next row as soon as the 15 warps have read it out
-            if (next < n_tok) {
+        for (;;) {
+            bool pending = false;
+            // ---- a3: merge the 30 (max, sum) states, token scalars, publish (c_t, lse, gy, next target)
+            if (a3_j < nrows) {
+                pending = true;
+                const int par = a3_j & 1;
+                if (__all_sync(kFull, mbar_test(stats_full0 + 8u * par, (uint32_t)(a3_j >> 1) & 1u))) {
+                    const int row = cluster + a3_j * nc;
+                    h = hn; valid = validn;
+                    // where the NEXT row's target sits in this half (the data warps mask it out of the
+                    // row): holder thread << 16 | round * 8 + element of the unit, or -1
+                    int hn_code = -1;
+                    {
+                        const int yu = (yq >= 0 && yq < a.V) ? (yq >> 3) - half_base : -1;
+                        if (yu >= 0 && yu < half_units)
+                            hn_code = ((yu % kSvRoundUnits) << 16) | ((yu / kSvRoundUnits) * 8 + (yq & 7));
+                    }
+                    const bool mine = lane < 2 * kSvConsumers;
+                    const float4 st = ctrl->stats[par][mine ? lane : 0];
+                    // max over the warp in ONE instruction: floats order like their bits once the
+                    // negative ones are flipped (this chain is on the critical path of every data warp)
+                    int mi = __float_as_int(mine ? st.x : -INFINITY);
+                    mi ^= (mi >> 31) & 0x7fffffff;
+                    mi = __reduce_max_sync(kFull, mi);
+                    mi ^= (mi >> 31) & 0x7fffffff;
+                    const float M = __int_as_float(mi);
+                    const float rs = (!mine || st.x == -INFINITY) ? 0.f : ex2_approx((st.x - M) * kLog2e);
+                    float S = st.y * rs;
+                    float SZ = ENT ? st.z * rs : 0.f;
 #pragma unroll
-                for (int s = 0; s < NCH; ++s) {
-                    if (s * kSvSlotRounds < nr) mbar_wait(empty0 + 8u * s, (uint32_t)it & 1u);
-                    load_slot(s, next);
-                }
-            }
-            // ---- a3: merge the 30 (max, sum) states, token scalars, publish (c_t, lse, gy)
-            mbar_wait(stats_full0 + 8u * par, ph2);
-            const bool mine = lane < 2 * kSvConsumers;
-            const float4 st = ctrl->stats[par][mine ? lane : 0];
-            // max over the warp in ONE instruction: floats order like their bits once the negative
-            // ones are flipped (this chain is on the critical path of every data warp of the cluster)
-            int mi = __float_as_int(mine ? st.x : -INFINITY);
-            mi ^= (mi >> 31) & 0x7fffffff;
-            mi = __reduce_max_sync(kFull, mi);
-            mi ^= (mi >> 31) & 0x7fffffff;
-            const float M = __int_as_float(mi);
-            const float rs = (!mine || st.x == -INFINITY) ? 0.f : ex2_approx((st.x - M) * kLog2e);
-            float S = st.y * rs;
-            float SZ = ENT ? st.z * rs : 0.f;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                S += __shfl_xor_sync(kFull, S, o);
-                if (ENT) SZ += __shfl_xor_sync(kFull, SZ, o);
-            }
-            if (lane == 0) {
-                const float lse_rest = M + fast_log(S);               // -inf if nothing but the target
-                const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
-                ctrl->rowinfo[par] = make_float4(ts.coef, ts.lse, ts.gy, 0.f);
-                mbar_arrive(ready0 + 8u * par);                       // release: rowinfo is visible
-                if (rank == 0) {
-                    store_token_outputs(a, row, h, ts, valid);
-                    if (ENT) a.token_entropy[row] = valid ? row_entropy(ts.lse, M, SZ, ts.lp, h.zy) : 0.f;
-                }
-            }
-            __syncwarp();
-            // ---- gradient: every full staging buffer goes out with one TMA bulk store
-            if (backward) {
-                uint8_t* g = gbase + (int64_t)row * row_bytes;
-                for (int pc = 0; pc < npieces; ++pc, ++gpiece) {
-                    const uint32_t b = gpiece & 1u;
-                    mbar_wait(sfull0 + 8u * b, (gpiece >> 1) & 1u);
+                    for (int o = 16; o > 0; o >>= 1) {
+                        S += __shfl_xor_sync(kFull, S, o);
+                        if (ENT) SZ += __shfl_xor_sync(kFull, SZ, o);
+                    }
                     if (lane == 0) {
-                        const int u0 = pc * kSvStageRounds * kSvRoundUnits;
+                        const float lse_rest = M + fast_log(S);           // -inf if nothing but the target
+                        const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
+                        ctrl->rowinfo[par] = make_float4(ts.coef, ts.lse, ts.gy, __int_as_float(hn_code));
+                        mbar_arrive(ready0 + 8u * par);                   // release: rowinfo is visible
+                        if (a3_j + 2 < nrows) mbar_expect_tx(stats_full0 + 8u * par, 2u * kSvConsumers * 16u);
+                        // prefetches for the next a3, AFTER the publish: the header is a chain of
+                        // dependent global loads (target -> its logit, trajectory -> its advantage)
+                        // and in-order issue would hold the publish behind it (measured: 1.1-3.5 k
+                        // clocks of every row with the loads in front, 530 behind)
+                        if (a3_j + 1 < nrows) hn = load_row_header(a, row + nc, validn, true);
+                        if (a3_j + 2 < nrows) yq = a.target_ids[row + 2 * nc];
+                        if (rank == 0) {
+                            store_token_outputs(a, row, h, ts, valid);
+                            if (ENT) a.token_entropy[row] = valid ? row_entropy(ts.lse, M, SZ, ts.lp, h.zy) : 0.f;
+                        }
+                    }
+                    __syncwarp();
+                    ++a3_j;
+                }
+            }
+            // ---- ring: refill a slot with its next row as soon as the 15 warps have read it out
+#pragma unroll
+            for (int s = 0; s < NCH; ++s) {
+                if (ld_j[s] < nrows) {
+                    pending = true;
+                    if (__all_sync(kFull, mbar_test(empty0 + 8u * s, (uint32_t)(ld_j[s] - 1) & 1u))) {
+                        issue_load(s, ld_j[s]);
+                        ++ld_j[s];
+                    }
+                }
+            }
+            // ---- gradient: every full staging buffer goes out with one TMA bulk store
+            if (st_j < nrows) {
+                pending = true;
+                const uint32_t b = gpiece & 1u;
+                if (__all_sync(kFull, mbar_test(sfull0 + 8u * b, (gpiece >> 1) & 1u))) {
+                    if (lane == 0) {
+                        const int u0 = st_pc * kSvStageRounds * kSvRoundUnits;
                         const int units = min(kSvStageRounds * kSvRoundUnits, half_units - u0);
-                        bulk_store(g + (int64_t)u0 * 16, stage + b * kSvStageBytes, (uint32_t)units * 16u);
+                        bulk_store(gbase + (int64_t)(cluster + st_j * nc) * row_bytes + (int64_t)u0 * 16,
+                                   stage + b * kSvStageBytes, (uint32_t)units * 16u);
                         bulk_commit();
                         // all but this newest store have read their buffer out: the other buffer is free
                         bulk_wait_read<1>();
                         if (gpiece > 0) mbar_arrive(sfree0 + 8u * (b ^ 1u));
                     }
                     __syncwarp();
+                    ++gpiece;
+                    if (++st_pc == npieces) { st_pc = 0; ++st_j; }
                 }
             }
+            if (!pending) break;
         }
         if (lane == 0) bulk_wait_all();                   // gradient writes complete before the CTA ends
     } else {
         // =============================================================== consumer warps
-        // The entropy sum (sum e z) is always accumulated: its serial FMA chain costs nothing in the
-        // MUFU-bound exp pass and keeps ptxas from hoisting the exponentials of the fully unrolled
-        // loop ahead of their consumers (without it the same code spilled part of the row).
-        constexpr bool want_ent = true;
+        // Software pipeline over rows in GROUPS of five rounds (= one staging buffer, half a ring
+        // slot): iteration `it` stages the gradient of row `it` out of a group's 20 registers
+        // (pass 2), refills them at once with the same group of row it + 1 (pass 0) and
+        // exponentiates it (pass 1).  Every group of every thread carries its own exp reference
+        // (the thread's max over the group, a bf16 value), so nothing in the loop body but the
+        // hand-over barriers orders one group after another: the MUFU-bound pass of the next row
+        // runs while the TMA stores of this row drain through the SM's 32 B/clk write port.
+        // The kernel holds 80 data registers of its 128: all bookkeeping is packed (one int for the
+        // place of a row's target, bf16 pairs for the exp references, rowinfo re-read from shared
+        // memory) and the file is compiled with ptxas -O1 (build.py), where nothing spills.
+        constexpr int NG = (NU + kSvStageRounds - 1) / kSvStageRounds;            // groups per row half
+        constexpr int kGroupsPerSlot = kSvSlotRounds / kSvStageRounds;
         const uint32_t my_off = (uint32_t)(warp * 32 + lane) * 16u;      // byte offset inside a round
-        const int my_unit0 = warp * 32 + lane;                           // unit of round 0
         uint32_t v[NU][4];
-        uint32_t gpiece = 0;
-        uint32_t mx2 = kSvNegInf2;
-
-        // One ring slot of row index `it` -> registers (rounds [10 s, 10 s + 10)), target entry masked
-        // to -inf (token_scalars works from lse_rest), packed running max; then the slot is released.
-        auto load_slot = [&](int s, int it, int y_round, int y_word, uint32_t y_keep) {
-            const bool have = s * kSvSlotRounds < nr;                                   // warp-uniform
-            if (have) mbar_wait(full0 + 8u * s, (uint32_t)it & 1u);
-            const uint32_t src = ring + (uint32_t)s * kSvSlotBytes + my_off;
+        uint32_t mref2[(NG + 1) / 2];                     // exp reference of each group's registers: bf16 pairs
 #pragma unroll
-            for (int kk = 0; kk < kSvSlotRounds; ++kk) {
-                const int k = s * kSvSlotRounds + kk;
-                if (k < NU) {
-                    if (k * kSvRoundUnits + my_unit0 < half_units) {
-                        lds128(v[k], src + (uint32_t)kk * kSvRoundBytes);
-                    } else {
-                        v[k][0] = v[k][1] = v[k][2] = v[k][3] = kSvNegInf2;
-                    }
-                    if (k == y_round) {
-#pragma unroll
-                        for (int j = 0; j < 4; ++j)
-                            v[k][j] = (j == y_word) ? ((v[k][j] & y_keep) | (kSvNegInf2 & ~y_keep)) : v[k][j];
-                    }
-                    mx2 = max_bf16x2(mx2, max_bf16x2(max_bf16x2(v[k][0], v[k][1]), max_bf16x2(v[k][2], v[k][3])));
-                }
-            }
-            if (have) {
-                __syncwarp();                                 // the slot has been read out by the warp
-                if (lane == 0) mbar_arrive(empty0 + 8u * s);
-            }
+        for (int g = 0; g < (NG + 1) / 2; ++g) mref2[g] = kSvNegInf2;
+        auto get_mref = [&](int g) { return (g & 1) ? bf16_hi(mref2[g >> 1]) : bf16_lo(mref2[g >> 1]); };
+        auto set_mref = [&](int g, float m) {            // m is a bf16 value: its high half, exactly
+            const uint32_t b = __float_as_uint(m);
+            mref2[g >> 1] = (g & 1) ? ((mref2[g >> 1] & 0x0000ffffu) | (b & 0xffff0000u))
+                                    : ((mref2[g >> 1] & 0xffff0000u) | (b >> 16));
         };
-        // where the target of a row sits for this thread: its round (or -1), word and the OTHER half
-        auto locate = [&](int y, int& y_round, int& y_word, uint32_t& y_keep) {
-            const bool valid = (y >= 0) && (y < a.V);
-            const int y_unit = valid ? (y >> 3) - half_base : -1;                       // unit inside this half
-            const bool holder = y_unit >= 0 && y_unit < half_units && (y_unit % kSvRoundUnits) == my_unit0;
-            y_round = holder ? y_unit / kSvRoundUnits : -1;
-            y_word = (y & 7) >> 1;
-            y_keep = (y & 1) ? 0x0000ffffu : 0xffff0000u;
-        };
-
-        int y = a.target_ids[cluster];
-        int y_round, y_word;
-        uint32_t y_keep;
-        locate(y, y_round, y_word, y_keep);
-#pragma unroll
-        for (int s = 0; s < NCH; ++s) load_slot(s, 0, y_round, y_word, y_keep);     // pass 0 of the first row
-
-        int it = 0;
-        for (int row = cluster; row < n_tok; row += nc, ++it) {
+        // where the target of a row sits for this thread: round * 8 + element inside the unit, or -1 if
+        // another thread holds it.  First row: computed here; later rows: the service warp hands
+        // (holder thread, place) over with rowinfo
+        int ypos = -1;                                    // row being staged
+        int ynpos;                                        // row being filled
+        {
+            const int y0 = a.target_ids[cluster];
+            const int yu = (y0 >= 0 && y0 < a.V) ? (y0 >> 3) - half_base : -1;
+            const bool holder = yu >= 0 && yu < half_units && (yu % kSvRoundUnits) == (int)(my_off >> 4);
+            ynpos = holder ? (yu / kSvRoundUnits) * 8 + (y0 & 7) : -1;
+        }
+        int it = -1;                                      // iteration -1 only fills the first row
+        for (int row = cluster - nc; row < n_tok; row += nc, ++it) {
             const int par = it & 1;
-            const uint32_t ph2 = (uint32_t)(it >> 1) & 1u;
+            const bool have_cur = it >= 0;
             const bool have_next = row + nc < n_tok;
-            const int y_nx = have_next ? a.target_ids[row + nc] : -1;     // in flight behind the exp pass
 
-            float m = fmaxf(bf16_lo(mx2), bf16_hi(mx2));
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(kFull, m, o));
-
-            // ---- pass 1: z -> e = exp2((z - m) log2 e) as bf16, in registers; f32 sum
-            const float nref = (m == -INFINITY) ? 0.f : -m * kLog2e;
-            float acc[4] = {0.f, 0.f, 0.f, 0.f};
-            float accz = 0.f;                          // sum e z (entropy output; the pass is MUFU-bound)
-#pragma unroll
-            for (int k = 0; k < NU; ++k) {
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const float z0 = bf16_lo(v[k][j]), z1 = bf16_hi(v[k][j]);
-                    const float e0 = ex2_approx(fmaf(z0, kLog2e, nref));
-                    const float e1 = ex2_approx(fmaf(z1, kLog2e, nref));
-                    acc[j] += e0;
-                    acc[j] += e1;
-                    if (want_ent) {
-                        accz = fmaf(e0, fmaxf(z0, kZFloor), accz);
-                        accz = fmaf(e1, fmaxf(z1, kZFloor), accz);
-                    }
-                    v[k][j] = pack_bf16x2(e0, e1);
-                }
+            // ---- a3 of this row ran on the service warp: (c_t, lse, c_t (p_y - 1), place of the next
+            // row's target).  rowinfo[par] stays valid for the whole iteration and is re-read where
+            // it is needed instead of being held in registers
+            const float4* rinfo = &ctrl->rowinfo[par];
+            if (have_cur) {
+                mbar_wait_hint(ready0 + 8u * par, (uint32_t)(it >> 1) & 1u, 1000u);
+                const int code = __float_as_int(rinfo->w);
+                ynpos = (code >> 16) == (int)(my_off >> 4) ? (code & 0xffff) : -1;
             }
-            float s = (acc[0] + acc[1]) + (acc[2] + acc[3]);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                s += __shfl_xor_sync(kFull, s, o);
-                if (ENT) accz += __shfl_xor_sync(kFull, accz, o);     // merged only if it is an output
-            }
-            // ---- exchange: (m_w, s_w, sz_w) to both CTAs, data and signal in one st.async each
-            if (lane < 2)
-                st_async_f32x4(smem_u32(&ctrl->stats[par][(int)rank * kSvConsumers + warp]),
-                               stats_full0 + 8u * par, (uint32_t)lane, m, s, accz, 0.f);
 
-            // where the next row's target sits (for its pass 0, interleaved below)
-            int yn_round, yn_word;
-            uint32_t yn_keep;
-            locate(y_nx, yn_round, yn_word, yn_keep);
-
-            // ---- a3 runs on the service warp; wait for (c_t, lse, c_t (p_y - 1))
-            mbar_wait(ready0 + 8u * par, ph2);
-            const float4 ri = ctrl->rowinfo[par];
-
-            // ---- pass 2 (a4): dlogits = e * (c_t exp(m - lse)) through the staging buffers, with pass
-            // 0 of the NEXT row slot by slot in between: after ten rounds both staging buffers are
-            // full and the warp would wait for the TMA store to drain one (32 B/clk); the registers
-            // of those ten rounds are free, so the next row's first ring slot is moved into them
-            // meanwhile.  e was taken relative to m (0 if the part held nothing finite); c_t = 0
-            // (masked, zero advantage, clip triggered): F = +0 and e >= 0 give all-bits-zero products
-            const float F = ri.x == 0.f ? 0.f : ri.x * ex2_approx(fmaf(-ri.y, kLog2e, -nref));
-            const __nv_bfloat16 fh = __float2bfloat16_rn(F);
-            const __nv_bfloat16 fl = __float2bfloat16_rn(F - __bfloat162float(fh));
-            const uint32_t Fh = (uint32_t)__bfloat16_as_ushort(fh) * 0x00010001u;
-            const uint32_t Fl = (uint32_t)__bfloat16_as_ushort(fl) * 0x00010001u;
-            const uint32_t gy_bits = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(ri.z));
-            const uint32_t gy2 = (y & 1) ? (gy_bits << 16) : gy_bits;
-            const int y_patch = ri.x != 0.f ? y_round : -1;
-            mx2 = kSvNegInf2;
+            float mrun = -INFINITY, st = 0.f, szt = 0.f;  // this thread's (max, sum, sum e z) of the next row
 #pragma unroll
-            for (int sl = 0; sl < NCH; ++sl) {
-                if (backward) {
+            for (int g = 0; g < NG; ++g) {
+                const int sl = g / kGroupsPerSlot;
+                const bool slot_used = sl * kSvSlotRounds < nr;                       // warp-uniform
+                // ---- pass 2 (a4) of this row, group g: dlogits = e * (c_t exp(m_g - lse)) into a
+                // staging buffer.  c_t = 0 (masked, zero advantage, clip triggered): F = +0 and
+                // e >= 0 give all-bits-zero products
+                if (backward && have_cur && g * kSvStageRounds < nr) {
+                    const float2 cl = *reinterpret_cast<const float2*>(rinfo);            // (c_t, lse)
+                    const float F = cl.x == 0.f ? 0.f : cl.x * ex2_approx((get_mref(g) - cl.y) * kLog2e);
+                    const __nv_bfloat16 fh = __float2bfloat16_rn(F);
+                    const __nv_bfloat16 fl = __float2bfloat16_rn(F - __bfloat162float(fh));
+                    const uint32_t Fh = (uint32_t)__bfloat16_as_ushort(fh) * 0x00010001u;
+                    const uint32_t Fl = (uint32_t)__bfloat16_as_ushort(fl) * 0x00010001u;
+                    const uint32_t gp = (uint32_t)(it * npieces + g);          // staging buffers filled so far
+                    const uint32_t buf = stage + (gp & 1u) * kSvStageBytes + my_off;
+                    mbar_wait(sfree0 + 8u * (gp & 1u), ((gp >> 1) & 1u) ^ 1u);
 #pragma unroll
-                    for (int kk2 = 0; kk2 < kSvSlotRounds; ++kk2) {
-                        const int k = sl * kSvSlotRounds + kk2;
-                        if (k < NU && k < nr) {                                   // k < nr: warp-uniform
-                            const int kk = k % kSvStageRounds;
-                            const uint32_t gp = gpiece + (uint32_t)(k / kSvStageRounds);
-                            const uint32_t buf = stage + (gp & 1u) * kSvStageBytes;
-                            if (kk == 0) mbar_wait(sfree0 + 8u * (gp & 1u), ((gp >> 1) & 1u) ^ 1u);
+                    for (int kk = 0; kk < kSvStageRounds; ++kk) {
+                        const int k = g * kSvStageRounds + kk;
+                        if (k < NU && (k < NU - 1 || k < nr)) {               // nr >= NU - 1; warp-uniform
                             uint4 o;
                             o.x = fma_bf16x2(v[k][0], Fh, mul_bf16x2(v[k][0], Fl));
                             o.y = fma_bf16x2(v[k][1], Fh, mul_bf16x2(v[k][1], Fl));
                             o.z = fma_bf16x2(v[k][2], Fh, mul_bf16x2(v[k][2], Fl));
                             o.w = fma_bf16x2(v[k][3], Fh, mul_bf16x2(v[k][3], Fl));
-                            if (k == y_patch) {                                   // target entry: c (p_y - 1)
-                                o.x = y_word == 0 ? ((o.x & y_keep) | gy2) : o.x;
-                                o.y = y_word == 1 ? ((o.y & y_keep) | gy2) : o.y;
-                                o.z = y_word == 2 ? ((o.z & y_keep) | gy2) : o.z;
-                                o.w = y_word == 3 ? ((o.w & y_keep) | gy2) : o.w;
-                            }
-                            sts128(buf + (uint32_t)kk * kSvRoundBytes + my_off, o);
-                            if (kk == kSvStageRounds - 1 || k == nr - 1) {
-                                fence_proxy_async();                              // generic writes -> TMA read
-                                __syncwarp();
-                                if (lane == 0) mbar_arrive(sfull0 + 8u * (gp & 1u));
+                            sts128(buf + (uint32_t)kk * kSvRoundBytes, o);
+                        }
+                    }
+                    // target entry: c (p_y - 1), patched into the staged unit by the one thread that
+                    // holds it (its own 16-byte store above is earlier in program order)
+                    if (ypos >= g * kSvStageRounds * 8 && ypos < (g + 1) * kSvStageRounds * 8 && cl.x != 0.f) {
+                        const uint32_t at = buf + (uint32_t)((ypos >> 3) - g * kSvStageRounds) * kSvRoundBytes +
+                                            (uint32_t)(ypos & 7) * 2u;
+                        const unsigned short gy = __bfloat16_as_ushort(__float2bfloat16_rn(rinfo->z));
+                        asm volatile("st.shared.u16 [%0], %1;" ::"r"(at), "h"(gy) : "memory");
+                    }
+                    fence_proxy_async();                                          // generic writes -> TMA read
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(sfull0 + 8u * (gp & 1u));
+                }
+                if (!have_next) continue;
+                // ---- pass 0 of the next row, group g: ring -> registers, target entry masked to -inf
+                // (token_scalars works from lse_rest), packed max; the slot is released after its
+                // last group
+                if (g % kGroupsPerSlot == 0 && slot_used) mbar_wait(full0 + 8u * sl, (uint32_t)(it + 1) & 1u);
+                const uint32_t src = ring + my_off;                  // the two slots are contiguous
+#pragma unroll
+                for (int kk = 0; kk < kSvStageRounds; ++kk) {
+                    const int k = g * kSvStageRounds + kk;
+                    if (k < NU) {
+                        // rounds below NU - 2 are full on both ranks; a stale read of the ring is harmless
+                        lds128(v[k], src + (uint32_t)k * kSvRoundBytes);
+                        if (k >= NU - 2 && k * kSvRoundUnits + (int)(my_off >> 4) >= half_units)
+                            v[k][0] = v[k][1] = v[k][2] = v[k][3] = kSvNegInf2;
+                    }
+                }
+                if ((g % kGroupsPerSlot == kGroupsPerSlot - 1 || g == NG - 1) && slot_used) {
+                    __syncwarp();                                 // the slot has been read out by the warp
+                    if (lane == 0) mbar_arrive(empty0 + 8u * sl);
+                }
+                // one thread of the cluster holds the target: a warp-uniform branch around its masking
+                if (__any_sync(kFull, ynpos >= g * kSvStageRounds * 8 && ynpos < (g + 1) * kSvStageRounds * 8)) {
+                    const uint32_t half = (ynpos & 1) ? 0xffff0000u : 0x0000ffffu;     // the target's half of its word
+#pragma unroll
+                    for (int kk = 0; kk < kSvStageRounds; ++kk) {
+                        const int k = g * kSvStageRounds + kk;
+                        if (k < NU) {
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {      // every word by name: v must stay in registers
+                                const uint32_t mk = (k * 4 + j == (ynpos >> 1)) ? half : 0u;
+                                v[k][j] = (v[k][j] & ~mk) | (kSvNegInf2 & mk);
                             }
                         }
                     }
                 }
-                if (have_next) load_slot(sl, it + 1, yn_round, yn_word, yn_keep);
+                uint32_t mx2 = kSvNegInf2;
+#pragma unroll
+                for (int kk = 0; kk < kSvStageRounds; ++kk) {
+                    const int k = g * kSvStageRounds + kk;
+                    if (k < NU)
+                        mx2 = max_bf16x2(mx2, max_bf16x2(max_bf16x2(v[k][0], v[k][1]), max_bf16x2(v[k][2], v[k][3])));
+                }
+                // ---- pass 1 of the next row, group g: z -> e = exp2((z - m) log2 e) as bf16, in
+                // registers, m = this thread's max over the group; f32 sums.  FFMA2 / FADD2: the (low,
+                // high) elements of a word are one packed f32x2 operation (half the issue slots)
+                const float m = fmaxf(bf16_lo(mx2), bf16_hi(mx2));
+                const float nref = (m == -INFINITY) ? 0.f : -m * kLog2e;
+                const float2 l2 = make_float2(kLog2e, kLog2e), nref2 = make_float2(nref, nref);
+                float2 acc[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+                float2 accz = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int kk = 0; kk < kSvStageRounds; ++kk) {
+                    const int k = g * kSvStageRounds + kk;
+                    if (k < NU) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const float2 z = make_float2(bf16_lo(v[k][j]), bf16_hi(v[k][j]));
+                            const float2 x = fma_f32x2(z, l2, nref2);
+                            const float2 e = make_float2(ex2_approx(x.x), ex2_approx(x.y));
+                            acc[j & 1] = add_f32x2(acc[j & 1], e);
+                            if (ENT)
+                                accz = fma_f32x2(e, make_float2(fmaxf(z.x, kZFloor), fmaxf(z.y, kZFloor)), accz);
+                            v[k][j] = pack_bf16x2(e.x, e.y);
+                        }
+                    }
+                }
+                // fold the group into the thread's state of the row
+                const float M = fmaxf(mrun, m);
+                const float f_old = (mrun == -INFINITY) ? 0.f : ex2_approx((mrun - M) * kLog2e);
+                const float f_new = (m == -INFINITY) ? 0.f : ex2_approx((m - M) * kLog2e);
+                st = st * f_old + ((acc[0].x + acc[0].y) + (acc[1].x + acc[1].y)) * f_new;
+                if (ENT) szt = szt * f_old + (accz.x + accz.y) * f_new;
+                mrun = M;
+                set_mref(g, m);
             }
-            if (backward) gpiece += (uint32_t)npieces;
-            y = y_nx; y_round = yn_round; y_word = yn_word; y_keep = yn_keep;
+            if (have_next) {
+                // ---- the warp's state, then the exchange: (m_w, s_w, sz_w) of the next row to both
+                // CTAs, data and signal in one st.async each
+                float wm = mrun;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) wm = fmaxf(wm, __shfl_xor_sync(kFull, wm, o));
+                const float sc = (mrun == -INFINITY) ? 0.f : ex2_approx((mrun - wm) * kLog2e);
+                st *= sc;
+                if (ENT) szt *= sc;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    st += __shfl_xor_sync(kFull, st, o);
+                    if (ENT) szt += __shfl_xor_sync(kFull, szt, o);
+                }
+                if (lane < 2)
+                    st_async_f32x4(smem_u32(&ctrl->stats[par ^ 1][(int)rank * kSvConsumers + warp]),
+                                   stats_full0 + 8u * (uint32_t)(par ^ 1), (uint32_t)lane, wm, st, szt, 0.f);
+            }
+            ypos = ynpos;
         }
     }
     cluster_arrive();     // nobody leaves while the peer may still send to its shared memory
@@ -366,6 +440,12 @@ static bool make_sv_plan(int64_t V, int64_t ld, int dtype, SvPlan& p, int& nu) {
     if (n < kSvMinNU || n > kSvMaxNU) return false;
     p.half_units[0] = (int)h0;
     p.half_units[1] = (int)(units - h0);
+    p.half_base[0] = 0;
+    p.half_base[1] = (int)h0;
+    for (int r = 0; r < 2; ++r) {
+        p.nr[r] = (p.half_units[r] + kSvRoundUnits - 1) / kSvRoundUnits;
+        p.npieces[r] = (p.nr[r] + kSvStageRounds - 1) / kSvStageRounds;
+    }
     p.num_clusters = 0;
     nu = (int)n;
     return true;
