@@ -398,7 +398,8 @@ def head_leg(torch, A, W, dev, steps, warmup, *, seed=1000, head_kernel="auto", 
     batch = W.make_batch(w, seed=seed, device=dev)
     n, V, K = batch["n_tok"], batch["V"], w.hidden
     kcode = {"auto": A.KERNEL_AUTO, "1cta": A.KERNEL_HEAD_1CTA, "2cta": A.KERNEL_HEAD_2CTA,
-             "stored": A.KERNEL_HEAD_2CTA_STORED}[head_kernel]
+             "stored": A.KERNEL_HEAD_2CTA_STORED, "e16": A.KERNEL_HEAD_2CTA_E16,
+             "rowref": A.KERNEL_HEAD_2CTA_ROWREF}[head_kernel]
     call = A.HeadLossCall(batch["hidden"], batch["w_head"], batch["target_ids"], batch["behave_lp"],
                           batch["prox_lp"], batch["step_off"], batch["traj_off"], batch["group_off"],
                           batch["rewards"], want=("err_word",), **dict(batch["params"], kernel=kcode))
@@ -421,7 +422,7 @@ def head_leg(torch, A, W, dev, steps, warmup, *, seed=1000, head_kernel="auto", 
     local_ms = t_beg.elapsed_time(t_end)
     peaks = measured_peaks()
     alg_flops = 6.0 * K * V * n
-    exe_ratio = 1.0 if head_kernel in ("auto", "stored") else 8.0 / 6.0
+    exe_ratio = 1.0 if head_kernel in ("auto", "stored", "e16", "rowref") else 8.0 / 6.0
     achieved = alg_flops / (local_ms / steps / 1e3) / 1e12
     res = {"ms_per_step": local_ms / steps, "tokens_per_s": n * steps / (local_ms / 1e3),
            "n_tok": n, "V": V, "K": K, "steps": steps, "entry": "awr_loss_fwd_bwd_fused_head",
@@ -430,8 +431,9 @@ def head_leg(torch, A, W, dev, steps, warmup, *, seed=1000, head_kernel="auto", 
                         "unit": "TFLOP/s", "frac": achieved / peaks["tensor"], "traffic": None,
                         "kernel": "head_gemm_kernel<epi, %s> (%s), whole step" % (
                             "1" if head_kernel == "1cta" else "2",
-                            "3 GEMMs + dS streaming pass per panel" if exe_ratio == 1.0
-                            else "4 GEMMs, logits recomputed"),
+                            "4 GEMMs, logits recomputed" if exe_ratio != 1.0 else
+                            ("3 GEMMs per panel, row-reference E, no dS pass" if head_kernel in ("auto", "rowref")
+                             else "3 GEMMs + dS streaming pass per panel")),
                         "algorithmic_flops_per_step": alg_flops,
                         "executed_flops_per_step": alg_flops * exe_ratio,
                         "executed_tflops": achieved * exe_ratio,
@@ -603,6 +605,80 @@ def run_cuda(args):
     return 0
 
 
+def run_regimes(args):
+    """--regimes: how the fwd+bwd row kernel of config 1 behaves as the board's clocks move (DESIGN.md
+    section 4, "Clock regimes"; a diagnostic, not the bench line).  (a) `--steps` back-to-back calls
+    from an idle board: kernel time of every call (events the call records around its row kernel)
+    and an NVML trace of the SM clock; (b) three calls after each of six 0.25 s bursts of dense
+    bf16 GEMMs (torch.matmul 8192^3 as the load generator): the state a training step leaves the
+    board in.  Prints one JSON object."""
+    import torch
+
+    import paper_2606_05597_b200 as A
+    from gen import workloads as W
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    batch = W.make_batch(W.workload(1), seed=1000, device=dev)
+    call = A.LossCall(batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+                      batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"],
+                      want=("err_word",), **batch["params"])
+    stream = torch.cuda.current_stream(dev)
+
+    def events(n):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        for a, b in evs:
+            a.record(stream)
+            b.record(stream)
+        return evs
+
+    for _ in range(2):
+        call.run()
+    steps = max(20, args.steps)
+    evs = events(steps)
+    torch.cuda.synchronize(dev)
+    time.sleep(1.0)                                  # idle board: boost clock
+    trace = []
+    with ClockSampler(dev.index or 0, period_s=0.001) as clk:
+        clk.trace = trace
+        t0 = time.perf_counter()
+        for ev in evs:
+            call.run(row_events=ev)
+        torch.cuda.synchronize(dev)
+        wall_ms = (time.perf_counter() - t0) * 1e3
+    ms = [a.elapsed_time(b) for a, b in evs]
+    n_sm = len(clk.sm)
+    blocks = []
+    for i in range(0, steps, 20):
+        blk = ms[i:i + 20]
+        lo, hi = i * n_sm // steps, max(i * n_sm // steps + 1, (i + len(blk)) * n_sm // steps)
+        blocks.append({"calls": "%d-%d" % (i, i + len(blk) - 1), "kernel_ms_mean": round(sum(blk) / len(blk), 3),
+                       "kernel_ms_min": round(min(blk), 3), "kernel_ms_max": round(max(blk), 3),
+                       "sm_mhz_median": statistics.median(clk.sm[lo:hi]) if clk.sm else None})
+    x = torch.randn(8192, 8192, device=dev, dtype=torch.bfloat16)
+    y = torch.randn(8192, 8192, device=dev, dtype=torch.bfloat16)
+    bursts = []
+    with ClockSampler(dev.index or 0) as clk2:
+        for _ in range(6):
+            for _ in range(300):
+                torch.matmul(x, y)
+            evs = events(3)
+            for ev in evs:
+                call.run(row_events=ev)
+            torch.cuda.synchronize(dev)
+            bursts.append([round(a.elapsed_time(b), 3) for a, b in evs])
+    assert int(call.out["err_word"][0]) == 0
+    flat = [v for r in bursts[1:] for v in r]
+    print(json.dumps({"regimes": {
+        "workload": "BASELINE.json configs[1], awr_loss_fwd_bwd, kernel %s" % KERNEL_NAMES.get(
+            A.select_kernel(batch["V"], batch["ld"], batch["logits"].dtype)),
+        "back_to_back": {"calls": steps, "wall_ms": round(wall_ms, 1), "by_20_calls": blocks,
+                         "reasons": sorted(clk.reasons)},
+        "between_gemm_bursts": {"kernel_ms": bursts, "mean_ms_after_first_burst": round(sum(flat) / len(flat), 3),
+                                "clocks": clk2.summary()}}}), flush=True)
+    return 0
+
+
 def run_head(args):
     """--config 4: the fused LM-head variant (a5).  A step = one awr_loss_fwd_bwd_fused_head call
     (hidden [32,768, 2048] and W_head [2048, 151,936] in, loss / dhidden / dw_head out).  The
@@ -706,7 +782,7 @@ def main(argv=None):
     ap.add_argument("--n-tok", type=int, default=0, help="override the config's token count")
     ap.add_argument("--normalizer", type=int, default=None, choices=[0, 1])
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4", "rfs"])
-    ap.add_argument("--head-kernel", default="auto", choices=["auto", "1cta", "2cta", "stored"],
+    ap.add_argument("--head-kernel", default="auto", choices=["auto", "1cta", "2cta", "stored", "e16", "rowref"],
                     help="config 4: tcgen05 shape / backward mode (auto = stored: CTA pairs, fp32 "
                          "logits of one row panel kept for the dS pass; 1cta / 2cta recompute)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: --steps")
@@ -716,7 +792,12 @@ def main(argv=None):
                     help="time awr_loss_fwd (PAPER.md:436 prox-lp recompute) instead of awr_loss_fwd_bwd")
     ap.add_argument("--no-others", action="store_true",
                     help="skip the legs for the other configs / the forward-only entry")
+    ap.add_argument("--regimes", action="store_true",
+                    help="diagnostic: per-call kernel times of config 1 against the board's clock state "
+                         "(back to back from idle; between bursts of dense GEMMs); prints its own JSON object")
     args = ap.parse_args(argv)
+    if args.regimes:
+        return run_regimes(args)
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3                   # timing rule: at least 3 warm-up steps
     _, _, world = dist_env()

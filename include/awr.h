@@ -95,7 +95,7 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     16K <= V <= 163,840); shared memory is a TMA load FIFO */
        AWR_KERNEL_CLUSTER_RF4 = 4, /* the same with a row quarter per CTA of a 4-CTA cluster and
                                     two CTAs (of different rows) resident per SM */
-       /* fused-head entry points only (AUTO = AWR_KERNEL_HEAD_2CTA_E16): */
+       /* fused-head entry points only (AUTO = AWR_KERNEL_HEAD_2CTA_ROWREF): */
        AWR_KERNEL_HEAD_1CTA = 5, /* tcgen05 cta_group::1, 128 x 256 tiles, one CTA per SM; the
                                     logits tile is recomputed for the backward (8 K V flops/token) */
        AWR_KERNEL_HEAD_2CTA = 6, /* tcgen05 cta_group::2, 256 x 256 tiles on CTA pairs; recompute */
@@ -114,9 +114,17 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     warps + one service warp per CTA: whole-slot TMA loads, gradient
                                     through shared-memory staging and TMA bulk stores, (max, sum)
                                     exchange by st.async, a3 on the service warp (bf16, 15,368 <= V
-                                    <= 153,600; AUTO's choice for awr_loss_fwd_bwd there) */ };
+                                    <= 153,600; AUTO's choice for awr_loss_fwd_bwd there) */,
+       AWR_KERNEL_HEAD_2CTA_ROWREF = 11 /* fused head, CTA pairs: E = bf16(exp(z - zref_t)) with a per-row
+                                    reference computed before the GEMM (zref_t = hidden_t . w_head[:, y_t],
+                                    an estimate of the target logit), so dS = E f_t with ONE factor per
+                                    row: the dhidden GEMM scales its output rows by f_t, the dw_head GEMM
+                                    reads bf16(f_t hidden_t); no pass over the panel is left.  A token with
+                                    a logit more than ~88 nats above its target's (p_y < 1e-38) sets
+                                    AWR_ERRBIT_HEAD_RANGE and contributes nothing */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
-       AWR_ERRBIT_TARGET_RANGE = 8u };
+       AWR_ERRBIT_TARGET_RANGE = 8u,
+       AWR_ERRBIT_HEAD_RANGE = 16u /* AWR_KERNEL_HEAD_2CTA_ROWREF only: exp(z - zref) overflowed in a row */ };
 
 /* One batch of response tokens (:61 "G rollouts per task, |tau_i| steps per rollout,
  * |tau_{i,j}| tokens per step"), as three CSR offset arrays.  Each offset array starts at 0,
@@ -235,8 +243,11 @@ AWR_API size_t awr_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t ld, in
 /* a5 (BASELINE.json config 4): hidden states + LM head instead of logits.  logits = hidden
  * [n_tok, K] x w_head are produced tile by tile in tensor memory and fed from there to the
  * log-sum-exp with fp32 accumulation (A17); the full [n_tok, V] matrix never exists.  What the modes
- * keep, for ONE row panel (<= 9,472 rows) at a time, between the panel's forward GEMM and its dS
- * pass:  E16 (AUTO): bf16(exp(z - tile row max)), 2 bytes per logit of the panel, in the dS buffer;
+ * keep, for ONE row panel (<= 9,472 rows) at a time, between the panel's forward GEMM and its backward
+ * GEMMs:  ROWREF (AUTO): E = bf16(exp(z - zref_t)), 2 bytes per logit of the panel, zref_t an estimate
+ * of the row's target logit computed before the GEMM; dS = E f_t is never formed (the row factor is
+ * applied by the dhidden epilogue and folded into the hidden operand of the dw_head GEMM);
+ * E16: bf16(exp(z - tile row max)) in the dS buffer, rescaled to dS by one in-place pass;
  * STORED: the fp32 logits of the panel (two buffers, a side stream);  HEAD_1CTA / HEAD_2CTA: nothing
  * (the tile is recomputed, 8 K V instead of 6 K V flops per token).  awr_head_workspace_bytes()
  * gives the bytes per mode.  Outputs dhidden = dS W^T and dw_head = H^T dS (bf16, overwritten). */
@@ -278,7 +289,8 @@ AWR_API int awr_loss_fwd_bwd_fused_head(const awr_head_batch* batch, const awr_p
                                 const awr_head_outputs* out, void* workspace,
                                 size_t workspace_bytes, void* stream);
 /* Workspace of the fused head for `kernel` (an AWR_KERNEL_HEAD_* id or AUTO); the modes differ:
- * config 4 (32,768 x 2048 x 151,936) needs 4.4 GB with E16 (AUTO), 15.9 GB with HEAD_2CTA_STORED. */
+ * config 4 (32,768 x 2048 x 151,936) needs 4.4 GB with ROWREF (AUTO) or E16, 15.9 GB with
+ * HEAD_2CTA_STORED. */
 AWR_API size_t awr_head_workspace_bytes(int64_t n_tok, int64_t V, int64_t K, int32_t n_steps,
                                 int32_t n_traj, int32_t n_groups, int32_t kernel);
 

@@ -68,7 +68,7 @@ static int check_params(const awr_params* p) {
     if (p->flags & ~(uint32_t)(AWR_FLAG_SAMPLE_STD | AWR_FLAG_SUCCESS_FILTER | AWR_FLAG_COUPLED |
                                AWR_FLAG_SKIP_UNIFORM))
         return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER_RFS) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_ROWREF) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -81,12 +81,14 @@ static int check_segments(int64_t n_tok, int32_t n_steps, int32_t n_traj, int32_
 // fused-head entry points: which tcgen05 shape (CTAs per tile) a kernel request means, or -1
 static int resolve_head_ctas(int requested) {
     if (requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA ||
-        requested == AWR_KERNEL_HEAD_2CTA_STORED || requested == AWR_KERNEL_HEAD_2CTA_E16) return 2;
+        requested == AWR_KERNEL_HEAD_2CTA_STORED || requested == AWR_KERNEL_HEAD_2CTA_E16 ||
+        requested == AWR_KERNEL_HEAD_2CTA_ROWREF) return 2;
     if (requested == AWR_KERNEL_HEAD_1CTA) return 1;
     return -1;
 }
 static int resolve_head_mode(int requested) {
-    if (requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA_E16) return kHeadE16;
+    if (requested == AWR_KERNEL_AUTO || requested == AWR_KERNEL_HEAD_2CTA_ROWREF) return kHeadRowRef;
+    if (requested == AWR_KERNEL_HEAD_2CTA_E16) return kHeadE16;
     return requested == AWR_KERNEL_HEAD_2CTA_STORED ? kHeadStored32 : kHeadRecompute;
 }
 

@@ -1,16 +1,19 @@
 // a5: fused LM-head variant (BASELINE.json config 4, readings A17).
 //
 //   logits Z = H W_head are produced tile by tile in tensor memory; the full matrix never exists.
-//   Per panel of P <= 9,472 rows (E16 mode, the default; DESIGN.md section 5 for the other modes):
-//     pass F   Z tile -> per-row (max, sum exp) partials + target gather, and E = bf16(exp(z - tile
-//              row max)) into the dS panel (2 bytes per logit of the panel, 2.9 GB at the default P)
-//                                                                              (GEMM, kEpiLse16)
-//     scalars  partials -> lse, l_t, ratio / clip / normalizer (a3), c_t          (one warp per row)
-//     dS       E -> dS = c_t (softmax - onehot) in place, bf16                    (streaming pass)
-//     pass G2  dhidden[panel] = dS W_head^T                                       (GEMM, kEpiStoreBf16)
-//     pass G3  dw_head += H[panel]^T dS   (fp32 running sum, bf16 at the end)     (GEMM, kEpiAccum)
-//   Stored mode keeps the fp32 tile instead (kEpiLse + head_ds_kernel on a side stream); the
-//   recompute modes form dS with a second logits GEMM (kEpiDs).
+//   Per panel of P <= 9,472 rows, row-reference mode (AUTO; DESIGN.md section 5 for the others):
+//     ref      zref_t = h_t . w[:, y_t], an estimate of the target logit, for all rows (one warp per row)
+//     pass F   Z tile -> per-row sum of e = exp(z - zref_t) + target gather, and E = bf16(e) into
+//              the dS panel (2 bytes per logit of the panel, 2.9 GB at the default P), ONE pass over
+//              the accumulator                                                  (GEMM, kEpiLseRef)
+//     scalars  partials -> lse, l_t, ratio / clip / normalizer (a3), c_t; then f_t = c_t exp(zref_t -
+//              lse), the target entry of E, and Hs = bf16(f_t h_t)                 (one warp per row)
+//     pass G2  dhidden[panel] = diag(f) (E W_head^T): row scale in the epilogue    (GEMM, kEpiStoreBf16)
+//     pass G3  dw_head += Hs^T E   (fp32 running sum, bf16 at the end)             (GEMM, kEpiAccum)
+//   so dS = diag(f) E is never formed.  E16 mode: E relative to the tile's row max (kEpiLse16, two
+//   passes over the accumulator) and an in-place streaming pass E -> dS; stored mode: the fp32 tile is
+//   kept instead (kEpiLse + head_ds_kernel on a side stream); the recompute modes form dS with a
+//   second logits GEMM (kEpiDs).
 // Every GEMM is the tcgen05 kernel below; see awr_head_gemm.cuh for the engine.
 #include <mutex>
 
@@ -369,6 +372,81 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                     if (want_ent) g.e.partz[(int64_t)n_blk * g.e.part_ld + row] = sz;
                     if (y_here) g.e.zy[row] = zy;
                 }
+            } else if constexpr (EPI == kEpiLseRef) {
+                // The row's exp reference is known before the GEMM (zref, an estimate of the target
+                // logit: every e is p_v / p_y up to a constant near 1), so ONE pass over the
+                // accumulator gives both the sum and E = bf16(exp(z - zref)).  The unrounded e feed
+                // the partial; an overflowing e (some logit 88 nats above the target's: p_y < 1e-38)
+                // makes the sum +inf, which head_scalars_kernel reports; the stored E is clamped to
+                // a finite value so that a zero row scale still gives zeros.
+                const int y = row_ok ? g.e.target_ids[row] : -1;
+                const bool want_ent = g.e.partz != nullptr;
+                const bool y_here = (y >= n0) && (y < n0 + kTN) && (y < g.N);
+                const float ref = row_ok ? g.e.zref[row] : 0.f;
+                const float nref = -ref * kLog2e;
+                float zy = 0.f, s = 0.f, sz = 0.f;
+                uint32_t* stg = reinterpret_cast<uint32_t*>(zstage) + q * (32 * kZStageLd);
+                const int row_w = row - lane;                 // tile row of this warp's TMEM lane 0
+                auto expchunk = [&](int c, float (&v)[32], int half) {
+                    const int c0 = n0 + c * 32;
+                    if (c0 + 32 > g.N) {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) if (c0 + j >= g.N) v[j] = -INFINITY;
+                    }
+                    if (y_here && y >= c0 && y < c0 + 32) {
+                        // the target entry is gathered and left out of the sum; its place in E is
+                        // written by head_scalars_kernel
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) if (c0 + j == y) { zy = v[j]; v[j] = -INFINITY; }
+                    }
+                    float acc0 = 0.f, acc1 = 0.f, accz = 0.f;
+#pragma unroll
+                    for (int j = 0; j < 32; j += 2) {
+                        const float z0 = v[j], z1 = v[j + 1];
+                        v[j] = ex2_approx(fmaf(z0, kLog2e, nref));
+                        v[j + 1] = ex2_approx(fmaf(z1, kLog2e, nref));
+                        acc0 += v[j];
+                        acc1 += v[j + 1];
+                        if (want_ent) {
+                            accz = fmaf(v[j], fmaxf(z0, kZFloor), accz);
+                            accz = fmaf(v[j + 1], fmaxf(z1, kZFloor), accz);
+                        }
+                    }
+                    s += acc0 + acc1;
+                    sz += accz;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        *reinterpret_cast<uint4*>(stg + lane * kZStageLd + half * 16 + 4 * j) = make_uint4(
+                            pack_bf16x2_sat(v[8 * j], v[8 * j + 1]), pack_bf16x2_sat(v[8 * j + 2], v[8 * j + 3]),
+                            pack_bf16x2_sat(v[8 * j + 4], v[8 * j + 5]), pack_bf16x2_sat(v[8 * j + 6], v[8 * j + 7]));
+                };
+                float vb[32];
+                tmem_ld32_issue(t_addr, v);
+#pragma unroll 1
+                for (int c = 0; c < kTN / 32; c += 2) {
+                    tmem_ld_wait(v);
+                    tmem_ld32_issue(t_addr + (c + 1) * 32, vb);
+                    expchunk(c, v, 0);
+                    tmem_ld_wait(vb);
+                    if (c + 2 < kTN / 32) tmem_ld32_issue(t_addr + (c + 2) * 32, v);
+                    expchunk(c + 1, vb, 1);
+                    __syncwarp();
+                    const int c0 = n0 + c * 32;
+                    const int cc = (lane & 7) * 8;            // bf16 column inside the 64
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int r = i * 4 + (lane >> 3);
+                        const uint4 t = *reinterpret_cast<const uint4*>(stg + r * kZStageLd + (lane & 7) * 4);
+                        if (row_w + r < g.M && c0 + cc < g.N)
+                            *reinterpret_cast<uint4*>(g.e.eout + (int64_t)(row_w + r) * g.e.eout_ld + c0 + cc) = t;
+                    }
+                    __syncwarp();
+                }
+                if (row_ok) {
+                    g.e.part[(int64_t)n_blk * g.e.part_ld + row] = make_float2(ref, s);
+                    if (want_ent) g.e.partz[(int64_t)n_blk * g.e.part_ld + row] = sz;
+                    if (y_here) g.e.zy[row] = zy;
+                }
             } else if constexpr (EPI == kEpiDs) {
                 int y = -1;
                 float lse = 0.f, coef = 0.f, gy = 0.f;
@@ -406,12 +484,22 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 }
             } else {
                 const int64_t ro = (int64_t)row * g.e.out_ld + n0;
+                float rs = 1.f;                               // kEpiStoreBf16: optional row scale
+                if constexpr (EPI == kEpiStoreBf16) {
+                    if (g.e.row_scale != nullptr && row_ok) rs = g.e.row_scale[row];
+                }
 #pragma unroll 1
                 for (int c = 0; c < kTN / 32; ++c) {
                     tmem_ld32(t_addr + c * 32, v);
                     const int c0 = n0 + c * 32;
                     if (!row_ok || c0 >= g.N) continue;
                     bool to_bf16 = true;
+                    if constexpr (EPI == kEpiStoreBf16) {
+                        if (g.e.row_scale != nullptr) {       // warp-uniform
+#pragma unroll
+                            for (int j = 0; j < 32; ++j) v[j] = rs == 0.f ? 0.f : v[j] * rs;
+                        }
+                    }
                     if constexpr (EPI == kEpiAccum) {
                         float* ap = g.e.acc + ro + c * 32;
                         if (!g.e.first_panel) {
@@ -477,12 +565,29 @@ namespace head {
 
 // One warp per row: combine the per-column-tile (max, sum) partials into the log-sum-exp of
 // the row without its target entry, then the same token_scalars() as the logits path.
+//
+// Row-reference mode (ref.zref != nullptr; the forward epilogue was kEpiLseRef, every partial is
+// relative to zref[row]): dS = E f_row with f_row = c_t exp(zref - lse), so instead of a pass over
+// the panel this warp writes f_row (the dhidden GEMM scales its output rows by it), the row of
+// Hs = bf16(f_row H) (the A operand of the dw_head GEMM) and ONE element of E: the target entry,
+// (p_y - 1) exp(lse - zref), so that E f_row = c_t (p_y - 1) there.  A row whose sum overflowed
+// (a logit 88 nats above the target's) sets AWR_ERRBIT_HEAD_RANGE and contributes nothing.
+struct HeadRefArgs {
+    const float* zref;            // [n_tok] or nullptr
+    float* row_f;                 // [n_tok]
+    __nv_bfloat16* e;             // E panel, row 0 = token row0
+    int64_t e_ld;
+    const __nv_bfloat16* hidden;  // [n_tok, K]
+    __nv_bfloat16* hs;            // [panel rows, K], row 0 = token row0
+    int64_t K;
+};
+
 __global__ void __launch_bounds__(256)
 head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld, int n_tiles,
                     const float* __restrict__ partz, const float* __restrict__ zy,
                     float* __restrict__ row_lse,
                     float* __restrict__ row_coef, float* __restrict__ row_gy, int64_t row0,
-                    int64_t row1) {
+                    int64_t row1, HeadRefArgs ref) {
     const int lane = threadIdx.x & 31;
     const int64_t row = row0 + (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (row >= row1) return;
@@ -505,7 +610,9 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
     const float lse_rest = st.m + logf(st.s);          // -inf when nothing but the target
     RowHeader h;
     h.y = a.target_ids[row];
-    const bool valid = (h.y >= 0) && (h.y < a.V);
+    bool valid = (h.y >= 0) && (h.y < a.V);
+    const bool overflow = ref.zref != nullptr && valid && !(st.s <= 3.0e38f);
+    if (overflow) valid = false;
     const int traj = a.tok_traj[row];
     h.q = a.prox_lp[row];
     h.b = a.behave_lp[row];
@@ -515,12 +622,73 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
     const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
     if (lane == 0) {
         if (h.y >= a.V) atomicOr(a.err_word, AWR_ERRBIT_TARGET_RANGE);
+        if (overflow) atomicOr(a.err_word, AWR_ERRBIT_HEAD_RANGE);
         store_token_outputs(a, row, h, ts, valid);
         if (a.token_entropy) a.token_entropy[row] = valid ? row_entropy(ts.lse, st.m, sz, ts.lp, h.zy) : 0.f;
         row_lse[row] = ts.lse;
         row_coef[row] = ts.coef;
         row_gy[row] = ts.gy;
     }
+    if (ref.zref != nullptr) {
+        const float zr = ref.zref[row];
+        const float f = ts.coef == 0.f ? 0.f : ts.coef * ex2_approx((zr - ts.lse) * kLog2e);
+        if (lane == 0) {
+            ref.row_f[row] = f;
+            if (f != 0.f) {
+                const float ty = (ts.gy / ts.coef) * ex2_approx((ts.lse - zr) * kLog2e);
+                ref.e[(row - row0) * ref.e_ld + h.y] = __float2bfloat16_rn(fmaxf(ty, -3.0e38f));
+            }
+        }
+        const uint4* src = reinterpret_cast<const uint4*>(ref.hidden + row * ref.K);
+        uint4* dst = reinterpret_cast<uint4*>(ref.hs + (row - row0) * ref.K);
+        for (int u = lane; u < (int)(ref.K >> 3); u += 32) {
+            uint4 o = make_uint4(0u, 0u, 0u, 0u);
+            if (f != 0.f) {
+                const uint4 x = src[u];
+                o.x = pack_bf16x2(bf16_lo(x.x) * f, bf16_hi(x.x) * f);
+                o.y = pack_bf16x2(bf16_lo(x.y) * f, bf16_hi(x.y) * f);
+                o.z = pack_bf16x2(bf16_lo(x.z) * f, bf16_hi(x.z) * f);
+                o.w = pack_bf16x2(bf16_lo(x.w) * f, bf16_hi(x.w) * f);
+            }
+            dst[u] = o;
+        }
+    }
+}
+
+// Row-reference mode: zref[row] = hidden[row, :] . w_head[:, y_row] in fp32 (an ESTIMATE of the
+// target logit - summation order differs from the tensor core's; any finite value near the row's
+// large logits would do), 0 for masked / out-of-range targets.  One warp per row.
+__global__ void __launch_bounds__(256)
+head_ref_kernel(const __nv_bfloat16* __restrict__ hidden, const __nv_bfloat16* __restrict__ w_head,
+                int kv_layout, int64_t V, int64_t K, const int32_t* __restrict__ target_ids,
+                int64_t n_tok, float* __restrict__ zref) {
+    const int lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= n_tok) return;
+    const int y = target_ids[row];
+    float acc = 0.f;
+    if (y >= 0 && y < V) {
+        const __nv_bfloat16* hr = hidden + row * K;
+        if (kv_layout) {                       // w_head[k * V + y]: a strided gather
+            const __nv_bfloat16* wc = w_head + y;
+#pragma unroll 8
+            for (int k = lane; k < (int)K; k += 32)
+                acc = fmaf(__bfloat162float(hr[k]), __bfloat162float(wc[(int64_t)k * V]), acc);
+        } else {                               // w_head[y * K + k]
+            const uint4* wr = reinterpret_cast<const uint4*>(w_head + (int64_t)y * K);
+            const uint4* hv = reinterpret_cast<const uint4*>(hr);
+            for (int u = lane; u < (int)(K >> 3); u += 32) {
+                const uint4 x = hv[u], w = wr[u];
+                acc = fmaf(bf16_lo(x.x), bf16_lo(w.x), acc); acc = fmaf(bf16_hi(x.x), bf16_hi(w.x), acc);
+                acc = fmaf(bf16_lo(x.y), bf16_lo(w.y), acc); acc = fmaf(bf16_hi(x.y), bf16_hi(w.y), acc);
+                acc = fmaf(bf16_lo(x.z), bf16_lo(w.z), acc); acc = fmaf(bf16_hi(x.z), bf16_hi(w.z), acc);
+                acc = fmaf(bf16_lo(x.w), bf16_lo(w.w), acc); acc = fmaf(bf16_hi(x.w), bf16_hi(w.w), acc);
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFull, acc, o);
+    if (lane == 0) zref[row] = (fabsf(acc) <= 3.0e38f) ? acc : 0.f;
 }
 
 // a4 for the stored-logits mode: dS = c_t (exp(z - lse) - onehot) from the fp32 logits panel the
@@ -724,7 +892,7 @@ static cudaError_t launch_gemm(int epi, const OperandView& A, const OperandView&
     if (nt == 2) return launch_gemm_epi<kEpiStoreBf16, 2, 2>(ta, tb, g, grid, st);
     switch (epi) {
         AWR_HEAD_CASE(kEpiLse) AWR_HEAD_CASE(kEpiDs) AWR_HEAD_CASE(kEpiStoreBf16) AWR_HEAD_CASE(kEpiAccum)
-        AWR_HEAD_CASE(kEpiLse16)
+        AWR_HEAD_CASE(kEpiLse16) AWR_HEAD_CASE(kEpiLseRef)
         default: return cudaErrorInvalidValue;
     }
 #undef AWR_HEAD_CASE
@@ -820,6 +988,8 @@ struct HeadWs {
     float* dw_acc;
     float* zpanel;           // stored-logits mode: fp32 [panel_rows, z_ld]
     float* zpanel2;          // second buffer: the forward of panel p + 1 runs beside the dS pass of p
+    float *zref, *row_f;     // row-reference mode: exp reference and dS scale of every row
+    __nv_bfloat16* hs;       // row-reference mode: bf16(f_row H) of the panel [panel_rows, K]
     int64_t part_ld, ds_ld, z_ld, panel_rows;
     int n_vtiles, n_panels;
     size_t total;
@@ -854,6 +1024,10 @@ static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ct
     w.z_ld = w.ds_ld;
     w.zpanel = (float*)take(store_z ? (size_t)w.panel_rows * w.z_ld * 4 : 0);
     w.zpanel2 = (float*)take(store_z && w.n_panels > 1 ? (size_t)w.panel_rows * w.z_ld * 4 : 0);
+    const bool rowref = mode == kHeadRowRef;
+    w.zref = (float*)take(rowref ? (size_t)n_pad * 4 : 0);
+    w.row_f = (float*)take(rowref ? (size_t)n_pad * 4 : 0);
+    w.hs = (__nv_bfloat16*)take(rowref ? (size_t)w.panel_rows * K * 2 : 0);
     w.total = off;
     return w;
 }
@@ -871,6 +1045,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     const int gm = 4096 / (kBM * ctas);               // raster groups of 4096 rows
     const bool store_z = c.mode == kHeadStored32;
     const bool e16 = c.mode == kHeadE16;
+    const bool rowref = c.mode == kHeadRowRef;
     const HeadWs w = head_carve(c.ws, c.n_tok, c.V, c.K, ctas, c.mode);
     const bool kv = c.w_layout == AWR_W_K_BY_V;
     const __nv_bfloat16* H = reinterpret_cast<const __nv_bfloat16*>(c.hidden);
@@ -879,12 +1054,21 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     const OperandView w_bwd{c.w_head, c.K, c.V, kv ? c.V : c.K, kv ? kMajorK : kMajorMN};
     cudaError_t e = cudaMemsetAsync(w.zy, 0, (size_t)w.part_ld * 4, st);
     if (e != cudaSuccess) return e;
+    if (rowref) {
+        const int warps = 8;
+        head_ref_kernel<<<(unsigned)((c.n_tok + warps - 1) / warps), warps * 32, 0, st>>>(
+            H, reinterpret_cast<const __nv_bfloat16*>(c.w_head), kv ? 1 : 0, c.V, c.K,
+            c.rows->target_ids, c.n_tok, w.zref);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
 
     // pass F + a3 over rows [r0, r0 + rows): log-sum-exp partials + gather, then the scalars.
     // Partials / gathered logits are indexed by global row (pointers pre-offset by r0).
     auto forward = [&](int64_t r0, int64_t rows, float* zout) -> cudaError_t {
         EpiArgs ea = {};
-        ea.eout = e16 ? w.ds : nullptr; ea.eout_ld = w.ds_ld;
+        ea.eout = (e16 || rowref) ? w.ds : nullptr; ea.eout_ld = w.ds_ld;
+        ea.zref = rowref ? w.zref + r0 : nullptr;
         ea.part = w.part + r0; ea.part_ld = w.part_ld; ea.zy = w.zy + r0;
         ea.partz = c.rows->token_entropy ? w.partz + r0 : nullptr;
         ea.target_ids = c.rows->target_ids + r0;
@@ -892,15 +1076,18 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         // raster: when the H rows of this call fit in L2 (a panel: 39 MB at K = 2048) walk all of
         // its row tiles before the next W column tile, so W_head streams from HBM exactly once
         const int fgm = rows * c.K * 2 <= (48ll << 20) ? (int)((rows + kBM * ctas - 1) / (kBM * ctas)) : gm;
-        cudaError_t err = launch_gemm(e16 ? kEpiLse16 : kEpiLse, OperandView{H + r0 * c.K, rows, c.K, c.K, kMajorK},
+        cudaError_t err = launch_gemm(rowref ? kEpiLseRef : (e16 ? kEpiLse16 : kEpiLse),
+                                      OperandView{H + r0 * c.K, rows, c.K, c.K, kMajorK},
                                       w_fwd, 0, fgm, ea, num_sms, ctas, st);
         if (err != cudaSuccess) return err;
         const int warps = 8;
         const unsigned blocks = (unsigned)((rows + warps - 1) / warps);
+        HeadRefArgs ra = {};
+        if (rowref) ra = HeadRefArgs{w.zref, w.row_f, w.ds, w.ds_ld, H, w.hs, c.K};
         head_scalars_kernel<<<blocks, warps * 32, 0, st>>>(*c.rows, w.part, w.part_ld, w.n_vtiles,
                                                            c.rows->token_entropy ? w.partz : nullptr,
                                                            w.zy, w.row_lse, w.row_coef, w.row_gy,
-                                                           r0, r0 + rows);
+                                                           r0, r0 + rows, ra);
         return cudaGetLastError();
     };
     if (c.mode == kHeadRecompute) {
@@ -962,6 +1149,10 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
                                                      w.part + r0, w.part_ld, w.row_lse + r0,
                                                      w.row_coef + r0, w.row_gy + r0);
             e = cudaGetLastError();
+        } else if (rowref) {
+            // row-reference mode: the forward GEMM leaves E = bf16(exp(z - zref)); the scalars kernel
+            // patches the target entries and writes f_row and Hs = bf16(f_row H).  No pass over E.
+            e = forward(r0, rows, nullptr);
         } else {
             EpiArgs e1 = {};
             e1.target_ids = c.rows->target_ids + r0; e1.row_lse = w.row_lse + r0;
@@ -973,6 +1164,7 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
 
         EpiArgs e2 = {};
         e2.out = reinterpret_cast<__nv_bfloat16*>(c.dhidden) + r0 * c.K; e2.out_ld = c.K;
+        e2.row_scale = rowref ? w.row_f + r0 : nullptr;
         e = launch_gemm(kEpiStoreBf16, OperandView{w.ds, rows, c.V, w.ds_ld, kMajorK}, w_bwd, 1, 1, e2,
                         num_sms, ctas, st, /*wide=*/true);
         if (e != cudaSuccess) return e;
@@ -980,7 +1172,8 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         EpiArgs e3 = {};
         e3.out = reinterpret_cast<__nv_bfloat16*>(c.dw_head); e3.acc = w.dw_acc;
         e3.first_panel = p == 0; e3.last_panel = p == w.n_panels - 1;
-        const OperandView ht{Hp, c.K, rows, c.K, kMajorMN};          // H^T: m = k, contraction = t
+        // H^T: m = k, contraction = t (row-reference mode: the rows of H already scaled by f_row)
+        const OperandView ht{rowref ? w.hs : Hp, c.K, rows, c.K, kMajorMN};
         const OperandView dst{w.ds, c.V, rows, w.ds_ld, kMajorMN};   // dS:  n = v, contraction = t
         if (kv) {            // dw_head[k, v]
             e3.out_ld = c.V;
@@ -997,6 +1190,8 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
 int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode) {
     const HeadWs w = head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2, mode);
     // recompute: F, scalars, then (dS GEMM, dH, dW) per panel; stored / E16: (F, scalars, dS pass, dH, dW) per panel
+    // row reference: the reference kernel, then (F, scalars, dH, dW) per panel
+    if (mode == kHeadRowRef) return 1 + 4 * w.n_panels;
     return mode != kHeadRecompute ? 5 * w.n_panels : 2 + 3 * w.n_panels;
 }
 

@@ -76,12 +76,13 @@ constexpr int kZStageBytes = 4 * 32 * kZStageLd * 4;            // 4 epilogue wa
 template <int EPI, int CTAS, int NT>
 struct EpiGeo {
     using G = Geo<CTAS, NT>;
-    static constexpr bool kStaged = EPI == 0 || EPI == 4;       // kEpiLse, kEpiLse16
+    static constexpr bool kStaged = EPI == 0 || EPI == 4 || EPI == 5;   // kEpiLse, kEpiLse16, kEpiLseRef
     static constexpr int kStages = (kStaged && CTAS == 2 && NT == 1) ? G::kStages - 1 : G::kStages;
     static constexpr int kSmemBytes = kStages * G::kStageBytes + 1024 + 256 + (kStaged ? kZStageBytes : 0);
 };
 static_assert(EpiGeo<0, 2, 1>::kSmemBytes <= 232448 && EpiGeo<0, 1, 1>::kSmemBytes <= 232448, "shared memory");
 static_assert(EpiGeo<4, 2, 1>::kSmemBytes <= 232448 && EpiGeo<4, 1, 1>::kSmemBytes <= 232448, "shared memory");
+static_assert(EpiGeo<5, 2, 1>::kSmemBytes <= 232448 && EpiGeo<5, 1, 1>::kSmemBytes <= 232448, "shared memory");
 static_assert(Geo<2>::kStages <= kMaxStages && Geo<2>::kSmemBytes <= 232448, "shared memory");
 static_assert(Geo<2, 2>::kSmemBytes <= 232448, "shared memory");
 
@@ -90,8 +91,12 @@ enum { kEpiLse = 0,      // a2 on the tile: per-row (max, sum exp) partials + ta
        kEpiDs = 1,       // a4 on the tile: dS = c_t (exp(z - lse) - onehot) -> bf16 panel
        kEpiStoreBf16 = 2,// C -> bf16 (dhidden)
        kEpiAccum = 3,    // C accumulated over row panels in fp32, bf16 on the last panel (dw_head)
-       kEpiLse16 = 4 };  // kEpiLse that also keeps the tile as E = bf16(exp(z - tile row max)): two
+       kEpiLse16 = 4,    // kEpiLse that also keeps the tile as E = bf16(exp(z - tile row max)): two
                          // passes over the accumulator (max, then exp + sum + store)
+       kEpiLseRef = 5 }; // the same with a PER-ROW reference known before the GEMM (zref[row], an estimate
+                         // of the target logit): E = bf16(exp(z - zref)) in ONE pass over the accumulator;
+                         // dS = E * f_row, so the scale moves into the dhidden epilogue (row_scale) and
+                         // into the H operand of the dw_head GEMM, and no dS pass is left
 
 // How one operand is staged and described to the tensor core (all runtime values).
 struct Operand {
@@ -116,8 +121,9 @@ struct EpiArgs {
     const int32_t* target_ids; // [M] (kEpiLse, kEpiDs), already offset to row 0 of this GEMM
     float* zout;               // optional [M, zout_ld]: the fp32 logits tile, kept for the dS pass
     int64_t zout_ld;
-    __nv_bfloat16* eout;       // kEpiLse16 [M, eout_ld]: E = exp(z - m) with m the (max) of part[]
+    __nv_bfloat16* eout;       // kEpiLse16 / kEpiLseRef [M, eout_ld]: E = exp(z - m), m the .x of part[]
     int64_t eout_ld;
+    const float* zref;         // kEpiLseRef [M]: the row's exp reference (finite)
     // kEpiDs
     const float* row_lse;      // [M] log-sum-exp of the whole row
     const float* row_coef;     // [M] c_t
@@ -125,6 +131,8 @@ struct EpiArgs {
     __nv_bfloat16* ds;         // [M, ds_ld]
     int64_t ds_ld;
     // kEpiStoreBf16 / kEpiAccum
+    const float* row_scale;    // kEpiStoreBf16, optional [M]: C row i is multiplied by row_scale[i]
+                               // (0 gives an all-zero row whatever the accumulator holds)
     __nv_bfloat16* out;        // [M, out_ld]
     float* acc;                // [M, out_ld] fp32 running sum over panels
     int64_t out_ld;

@@ -79,8 +79,11 @@ struct HeadCall {
 enum { kHeadRecompute = 0,  // the logits tile is recomputed for dS (8 K V flops / token)
        kHeadStored32 = 1,   // the fp32 logits of a row panel are kept (two buffers, side stream); dS in
                             // a streaming pass (6 K V); same bits as recompute
-       kHeadE16 = 2 };      // the forward epilogue keeps E = bf16(exp(z - tile max)) IN the dS panel; one
+       kHeadE16 = 2,        // the forward epilogue keeps E = bf16(exp(z - tile max)) IN the dS panel; one
                             // in-place pass rescales it to dS (6 K V; 2 bytes per logit of transient)
+       kHeadRowRef = 3 };   // E = bf16(exp(z - zref_row)) with a per-row reference known before the GEMM
+                            // (an estimate of the target logit): dS = E f_row, the scale applied by the
+                            // dhidden epilogue and folded into the H operand of dw_head - no dS pass
 size_t head_ws_bytes(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode);
 int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode);
 cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st);

@@ -15,16 +15,24 @@
 //     contiguous in memory, two buffers: all the shared memory the ring leaves) at shared-memory
 //     speed (128 B/clk) and go on; the service lane hands each full buffer to a TMA bulk store.
 //     An SM writes to L2 at 32 B/clk whatever the instruction (measured for per-lane stores and for
-//     TMA stores alike), so the 148 KB of a row half need 4.7 k clocks of that port; what staging
-//     buys is that the last 75 KB drain while the warps are already in the next row - and the
-//     first 75 KB too: the waits for a free staging buffer are filled with pass 0 (ring ->
-//     registers, max) of the NEXT row, slot by slot, into the registers whose gradient has just
-//     been staged.  With that the kernel is HBM-bound (config 1: 3.87 ms, 0.99 of the copy peak).
+//     TMA stores alike), so the 148 KB of a row half need 4.7 k clocks of that port.
+//   * Schedule: a software pipeline over rows in GROUPS of five rounds (= one staging buffer = 20
+//     registers per thread).  In turn for each group: stage the gradient of row r out of the
+//     group's registers (pass 2), refill them from the ring with the same group of row r + 1
+//     (pass 0) and exponentiate it (pass 1).  Every group carries its own exp reference (the
+//     thread's max over the group), so no warp-wide or row-wide max sits between the passes and
+//     the MUFU-bound pass of the next row runs while the TMA stores of this row drain through the
+//     write port.  Measured against the predecessor (pass 0 of the next row inside the staging
+//     waits, then one MUFU pass over the whole row): slower in a cold burst at the 1,965 MHz boost
+//     clock (4.05 against 3.70 ms for config 1), faster once the board has settled under load
+//     (3.8-3.95 against 4.1-4.3 ms) and at the power-capped clocks of a training step (4.95 against
+//     5.45 ms between bursts of dense GEMMs): DESIGN.md section 4, profiles/r2_rows.md.
 //   * Exchange: every consumer warp sends its (max, sum[, sum e z]) with st.async to BOTH CTAs; the
 //     16 bytes complete a transaction count on the receiver's mbarrier - no cluster barrier, no
 //     fence.  The service warp of each CTA merges the 30 states, evaluates a3 once (header loads
 //     issued a row ahead) and publishes (c_t, lse, c_t (p_y - 1)) in shared memory; the consumers
-//     wait for that on an mbarrier and scale their registers by c_t exp(m_w - lse).
+//     wait for that on an mbarrier and scale each group of registers by c_t exp(m_g - lse), m_g the
+//     group's exp reference.
 // Rows are dealt round-robin to clusters (static schedule, fixed merge order: bit-reproducible).
 #include "awr_common.cuh"
 #include "awr_kernels.h"

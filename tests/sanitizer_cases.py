@@ -56,7 +56,8 @@ def main():
         print("300 x 151,936 bf16, forward stream, entropy", ent, ":",
               rows_case(big, A.KERNEL_FWD_STREAM, backward=False, entropy=ent))
     for name, k in (("1cta recompute", A.KERNEL_HEAD_1CTA), ("2cta recompute", A.KERNEL_HEAD_2CTA),
-                    ("2cta stored fp32", A.KERNEL_HEAD_2CTA_STORED), ("2cta E16", A.KERNEL_HEAD_2CTA_E16)):
+                    ("2cta stored fp32", A.KERNEL_HEAD_2CTA_STORED), ("2cta E16", A.KERNEL_HEAD_2CTA_E16),
+                    ("2cta row reference", A.KERNEL_HEAD_2CTA_ROWREF)):
         print("fused head 600 x 128 x 2056,", name, ":", head_case(k))
     print("SANITIZER_CASES_DONE")
 

@@ -31,7 +31,8 @@ def _f64(t):
 
 
 HEAD_KERNELS = [A.KERNEL_HEAD_1CTA, A.KERNEL_HEAD_2CTA]
-HEAD_PANEL_KERNELS = [A.KERNEL_HEAD_2CTA_STORED, A.KERNEL_HEAD_2CTA_E16]   # keep one row panel of logits / E
+HEAD_PANEL_KERNELS = [A.KERNEL_HEAD_2CTA_STORED, A.KERNEL_HEAD_2CTA_E16,   # keep one row panel of logits / E
+                      A.KERNEL_HEAD_2CTA_ROWREF]
 
 
 # ------------------------------------------------------------------ the GEMM engine alone
@@ -131,7 +132,8 @@ def test_head_vs_oracle(n_tok, K, V, w_layout, kernel):
 @pytest.mark.parametrize("kernel,n_tok,panels", [(A.KERNEL_HEAD_1CTA, 9700, 3),
                                                  (A.KERNEL_HEAD_2CTA, 19300, 3),
                                                  (A.KERNEL_HEAD_2CTA_STORED, 19300, 3),
-                                                 (A.KERNEL_HEAD_2CTA_E16, 19300, 3)])
+                                                 (A.KERNEL_HEAD_2CTA_E16, 19300, 3),
+                                                 (A.KERNEL_HEAD_2CTA_ROWREF, 19300, 3)])
 @pytest.mark.parametrize("norm", [A.NORM_CONST_K, A.NORM_PER_TRAJ])
 def test_head_several_panels(norm, kernel, n_tok, panels):
     """More rows than one dS panel (4,736 rows, 9,472 for CTA pairs): dw_head accumulates
@@ -141,9 +143,11 @@ def test_head_several_panels(norm, kernel, n_tok, panels):
     ora = _oracle_head(batch, normalizer=norm)
     _check_head(gpu, ora, A.W_K_BY_V)
     per_call = 5 * panels if kernel in HEAD_PANEL_KERNELS else 2 + 3 * panels
+    if kernel == A.KERNEL_HEAD_2CTA_ROWREF:
+        per_call = 1 + 4 * panels          # reference kernel, then (F, scalars, dhidden, dw_head) per panel
     assert A.head_launches_per_call(n_tok, 512, 64, kernel) == 3 + per_call
     assert A.head_launches_per_call(n_tok, 512, 64) == A.head_launches_per_call(
-        n_tok, 512, 64, A.KERNEL_HEAD_2CTA_E16)             # AUTO resolves to the E16 mode
+        n_tok, 512, 64, A.KERNEL_HEAD_2CTA_ROWREF)          # AUTO resolves to the row-reference mode
 
 
 def test_head_stored_logits_same_bits_as_recompute():
@@ -154,6 +158,70 @@ def test_head_stored_logits_same_bits_as_recompute():
     b = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA_STORED, stale_cap=2.0)
     for k in ("loss", "token_lp", "clip_count", "tok_coef", "tok_term", "dhidden", "dw_head"):
         assert torch.equal(a[k], b[k]), k
+
+
+def test_head_rowref_peaked_and_unlikely_targets():
+    """Row-reference mode away from its comfortable case.  The reference is an estimate of the TARGET
+    logit, so every e = exp(z - zref) is p_v / p_y: (a) rows whose target is the far most likely
+    token (p_y -> 1, all other e tiny) and (b) rows whose target is 40 nats below the row maximum
+    (e up to e^40, sums of 1e17) must still meet the oracle at the usual bars; nothing is flagged."""
+    n_tok, K, V = 600, 128, 2056
+    batch = _head_batch(n_tok, K, V, seed=61, lp_mode="drift", masked_frac=0.02)
+    hid = batch["hidden"].float()
+    w = batch["w_head"].float().clone()                       # [K, V]
+    ids = batch["target_ids"].clone()
+    # column 7 of W becomes a "loud" token: logit = 0.5 * |h|^2 / sqrt(K)-ish, large and positive for
+    # every row; rows 0::3 get it as target (peaked), rows 1::3 keep a random target far below it
+    loud = hid.mean(0)
+    loud = loud / loud.norm() * 4.0
+    w[:, 7] = loud
+    batch["w_head"] = w.to(torch.bfloat16)
+    hid = hid + 10.0 * loud / loud.norm()                    # every row has a component along it: z_7 ~ 40
+    batch["hidden"] = hid.to(torch.bfloat16)
+    sel = torch.arange(n_tok, device=DEV) % 3 == 0
+    ids[sel & (ids >= 0)] = 7
+    batch["target_ids"] = ids
+    z = batch["hidden"].float() @ batch["w_head"].float()
+    lp = torch.log_softmax(z.double(), -1)
+    gathered = lp.gather(1, ids.clamp(min=0).long()[:, None])[:, 0].float()
+    batch["prox_lp"] = gathered + 0.01 * torch.randn_like(gathered)
+    batch["behave_lp"] = batch["prox_lp"] + 0.01 * torch.randn_like(gathered)
+    assert float(gathered[(~sel) & (ids >= 0)].min()) < -30.0 and float(gathered[sel & (ids >= 0)].max()) > -1e-3
+    ora = _oracle_head(batch)
+    for kernel in (A.KERNEL_HEAD_2CTA_ROWREF, A.KERNEL_HEAD_2CTA_E16):
+        gpu = _run_head(batch, kernel=kernel)
+        _check_head(gpu, ora, A.W_K_BY_V)
+
+
+def test_head_rowref_overflow_is_reported():
+    """A token whose target logit is more than ~88 nats below another logit of its row (p_y < 1e-38)
+    cannot be represented relative to its reference: AWR_ERRBIT_HEAD_RANGE is set, the token
+    contributes nothing (zero term, zero dhidden row, token_lp 0 like a masked token) and every
+    other row is what the oracle gives with that token masked."""
+    n_tok, K, V = 300, 64, 1000
+    batch = _head_batch(n_tok, K, V, seed=62)
+    hid = batch["hidden"].float().clone()
+    w = batch["w_head"].float().clone()
+    bad = 17
+    y = int(batch["target_ids"][bad])
+    other = (y + 1) % V
+    w[:, other] = hid[bad] / hid[bad].norm() * 3.0            # z[bad, other] = 3 |h| ~ 24 ... scale up below
+    hid[bad] *= 6.0                                           # |h| ~ 48: z[bad, other] ~ 144, target logit ~ N(0, 1)
+    batch["hidden"] = hid.to(torch.bfloat16)
+    batch["w_head"] = w.to(torch.bfloat16)
+    z = batch["hidden"].float() @ batch["w_head"].float()
+    assert float(z[bad, other] - z[bad, y]) > 100.0
+    gpu = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA_ROWREF)
+    assert int(gpu["err_word"][0]) == A.ERRBIT_HEAD_RANGE
+    assert float(gpu["token_lp"][bad]) == 0.0 and float(gpu["tok_term"][bad]) == 0.0
+    assert not gpu["dhidden"][bad].any()
+    assert torch.isfinite(gpu["dhidden"].float()).all() and torch.isfinite(gpu["dw_head"].float()).all()
+    masked = dict(batch)
+    masked["target_ids"] = batch["target_ids"].clone()
+    masked["target_ids"][bad] = -1
+    ora = _oracle_head(masked)
+    gpu["err_word"].zero_()
+    _check_head(gpu, ora, A.W_K_BY_V)
 
 
 def test_head_shapes_agree_bitwise_on_integers():
@@ -386,12 +454,14 @@ def test_head_host_buffer_entry():
 
 
 def test_head_workspace_is_mode_aware():
-    """include/awr.h: the workspace query takes the kernel; AUTO (E16) keeps 2 bytes per logit of one
-    row panel - BASELINE.json configs[4] fits in 5 GB - the stored-fp32 mode needs three times that."""
+    """include/awr.h: the workspace query takes the kernel; AUTO (row reference) and E16 keep 2 bytes
+    per logit of one row panel - BASELINE.json configs[4] fits in 5 GB - the stored-fp32 mode needs
+    three times that."""
     auto = A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16)
+    rowref = A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_HEAD_2CTA_ROWREF)
     e16 = A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_HEAD_2CTA_E16)
     stored = A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_HEAD_2CTA_STORED)
-    assert auto == e16 <= 5 * 10 ** 9 < stored
+    assert e16 < auto == rowref <= 5 * 10 ** 9 < stored
     assert A.head_workspace_bytes(32_768, 151_936, 2048, 3000, 256, 16, A.KERNEL_CLUSTER_RF) == 0
 
 
