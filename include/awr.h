@@ -116,12 +116,13 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     exchange by st.async, a3 on the service warp (bf16, 15,368 <= V
                                     <= 153,600; AUTO's choice for awr_loss_fwd_bwd there) */,
        AWR_KERNEL_HEAD_2CTA_ROWREF = 11 /* fused head, CTA pairs: E = bf16(exp(z - zref_t)) with a per-row
-                                    reference computed before the GEMM (zref_t = hidden_t . w_head[:, y_t],
-                                    an estimate of the target logit), so dS = E f_t with ONE factor per
-                                    row: the dhidden GEMM scales its output rows by f_t, the dw_head GEMM
-                                    reads bf16(f_t hidden_t); no pass over the panel is left.  A token with
-                                    a logit more than ~88 nats above its target's (p_y < 1e-38) sets
-                                    AWR_ERRBIT_HEAD_RANGE and contributes nothing */ };
+                                    reference computed before the GEMM (zref_t = the row's largest logit
+                                    among the first 256 vocabulary entries: one column tile), so dS =
+                                    E f_t with ONE factor per row: the dhidden GEMM scales its output rows
+                                    by f_t, the dw_head GEMM reads bf16(f_t hidden_t); no pass over the
+                                    panel is left.  A valid token whose row has a logit more than ~88 nats
+                                    above that reference sets AWR_ERRBIT_HEAD_RANGE and contributes
+                                    nothing (use AWR_KERNEL_HEAD_2CTA_E16 for such logits) */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u,
        AWR_ERRBIT_HEAD_RANGE = 16u /* AWR_KERNEL_HEAD_2CTA_ROWREF only: exp(z - zref) overflowed in a row */ };
@@ -244,8 +245,8 @@ AWR_API size_t awr_host_workspace_bytes(int64_t n_tok, int64_t V, int64_t ld, in
  * [n_tok, K] x w_head are produced tile by tile in tensor memory and fed from there to the
  * log-sum-exp with fp32 accumulation (A17); the full [n_tok, V] matrix never exists.  What the modes
  * keep, for ONE row panel (<= 9,472 rows) at a time, between the panel's forward GEMM and its backward
- * GEMMs:  ROWREF (AUTO): E = bf16(exp(z - zref_t)), 2 bytes per logit of the panel, zref_t an estimate
- * of the row's target logit computed before the GEMM; dS = E f_t is never formed (the row factor is
+ * GEMMs:  ROWREF (AUTO): E = bf16(exp(z - zref_t)), 2 bytes per logit of the panel, zref_t the row's
+ * largest logit among the first 256 vocabulary entries, computed before the GEMM; dS = E f_t is never formed (the row factor is
  * applied by the dhidden epilogue and folded into the hidden operand of the dw_head GEMM);
  * E16: bf16(exp(z - tile row max)) in the dS buffer, rescaled to dS by one in-place pass;
  * STORED: the fp32 logits of the panel (two buffers, a side stream);  HEAD_1CTA / HEAD_2CTA: nothing

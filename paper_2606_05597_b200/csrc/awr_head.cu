@@ -2,7 +2,8 @@
 //
 //   logits Z = H W_head are produced tile by tile in tensor memory; the full matrix never exists.
 //   Per panel of P <= 9,472 rows, row-reference mode (AUTO; DESIGN.md section 5 for the others):
-//     ref      zref_t = h_t . w[:, y_t], an estimate of the target logit, for all rows (one warp per row)
+//     ref      zref_t = the row's largest logit among the first 256 vocabulary entries: one column
+//              tile of the forward GEMM                                          (GEMM, kEpiRowMax)
 //     pass F   Z tile -> per-row sum of e = exp(z - zref_t) + target gather, and E = bf16(e) into
 //              the dS panel (2 bytes per logit of the panel, 2.9 GB at the default P), ONE pass over
 //              the accumulator                                                  (GEMM, kEpiLseRef)
@@ -373,12 +374,11 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                     if (y_here) g.e.zy[row] = zy;
                 }
             } else if constexpr (EPI == kEpiLseRef) {
-                // The row's exp reference is known before the GEMM (zref, an estimate of the target
-                // logit: every e is p_v / p_y up to a constant near 1), so ONE pass over the
-                // accumulator gives both the sum and E = bf16(exp(z - zref)).  The unrounded e feed
-                // the partial; an overflowing e (some logit 88 nats above the target's: p_y < 1e-38)
-                // makes the sum +inf, which head_scalars_kernel reports; the stored E is clamped to
-                // a finite value so that a zero row scale still gives zeros.
+                // The row's exp reference is known before the GEMM (zref: the largest of the row's
+                // first 256 logits), so ONE pass over the accumulator gives both the sum and
+                // E = bf16(exp(z - zref)).  The unrounded e feed the partial; an overflowing e (a logit
+                // 88 nats above the reference) makes the sum +inf, which head_scalars_kernel reports;
+                // the stored E is clamped to a finite value so that a zero row scale still gives zeros.
                 const int y = row_ok ? g.e.target_ids[row] : -1;
                 const bool want_ent = g.e.partz != nullptr;
                 const bool y_here = (y >= n0) && (y < n0 + kTN) && (y < g.N);
@@ -447,6 +447,17 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                     if (want_ent) g.e.partz[(int64_t)n_blk * g.e.part_ld + row] = sz;
                     if (y_here) g.e.zy[row] = zy;
                 }
+            } else if constexpr (EPI == kEpiRowMax) {
+                float m = -INFINITY;
+#pragma unroll 1
+                for (int c = 0; c < kTN / 32; ++c) {
+                    tmem_ld32(t_addr + c * 32, v);
+                    const int c0 = n0 + c * 32;
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) if (c0 + j < g.N) m = fmaxf(m, v[j]);
+                }
+                // a finite reference whatever the accumulators hold (NaN / inf logits: garbage in)
+                if (row_ok) g.e.zref_out[row] = (fabsf(m) <= 3.0e38f) ? m : 0.f;
             } else if constexpr (EPI == kEpiDs) {
                 int y = -1;
                 float lse = 0.f, coef = 0.f, gy = 0.f;
@@ -571,7 +582,7 @@ namespace head {
 // the panel this warp writes f_row (the dhidden GEMM scales its output rows by it), the row of
 // Hs = bf16(f_row H) (the A operand of the dw_head GEMM) and ONE element of E: the target entry,
 // (p_y - 1) exp(lse - zref), so that E f_row = c_t (p_y - 1) there.  A row whose sum overflowed
-// (a logit 88 nats above the target's) sets AWR_ERRBIT_HEAD_RANGE and contributes nothing.
+// (a logit 88 nats above the reference) sets AWR_ERRBIT_HEAD_RANGE and contributes nothing.
 struct HeadRefArgs {
     const float* zref;            // [n_tok] or nullptr
     float* row_f;                 // [n_tok]
@@ -653,42 +664,6 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
             dst[u] = o;
         }
     }
-}
-
-// Row-reference mode: zref[row] = hidden[row, :] . w_head[:, y_row] in fp32 (an ESTIMATE of the
-// target logit - summation order differs from the tensor core's; any finite value near the row's
-// large logits would do), 0 for masked / out-of-range targets.  One warp per row.
-__global__ void __launch_bounds__(256)
-head_ref_kernel(const __nv_bfloat16* __restrict__ hidden, const __nv_bfloat16* __restrict__ w_head,
-                int kv_layout, int64_t V, int64_t K, const int32_t* __restrict__ target_ids,
-                int64_t n_tok, float* __restrict__ zref) {
-    const int lane = threadIdx.x & 31;
-    const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (row >= n_tok) return;
-    const int y = target_ids[row];
-    float acc = 0.f;
-    if (y >= 0 && y < V) {
-        const __nv_bfloat16* hr = hidden + row * K;
-        if (kv_layout) {                       // w_head[k * V + y]: a strided gather
-            const __nv_bfloat16* wc = w_head + y;
-#pragma unroll 8
-            for (int k = lane; k < (int)K; k += 32)
-                acc = fmaf(__bfloat162float(hr[k]), __bfloat162float(wc[(int64_t)k * V]), acc);
-        } else {                               // w_head[y * K + k]
-            const uint4* wr = reinterpret_cast<const uint4*>(w_head + (int64_t)y * K);
-            const uint4* hv = reinterpret_cast<const uint4*>(hr);
-            for (int u = lane; u < (int)(K >> 3); u += 32) {
-                const uint4 x = hv[u], w = wr[u];
-                acc = fmaf(bf16_lo(x.x), bf16_lo(w.x), acc); acc = fmaf(bf16_hi(x.x), bf16_hi(w.x), acc);
-                acc = fmaf(bf16_lo(x.y), bf16_lo(w.y), acc); acc = fmaf(bf16_hi(x.y), bf16_hi(w.y), acc);
-                acc = fmaf(bf16_lo(x.z), bf16_lo(w.z), acc); acc = fmaf(bf16_hi(x.z), bf16_hi(w.z), acc);
-                acc = fmaf(bf16_lo(x.w), bf16_lo(w.w), acc); acc = fmaf(bf16_hi(x.w), bf16_hi(w.w), acc);
-            }
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFull, acc, o);
-    if (lane == 0) zref[row] = (fabsf(acc) <= 3.0e38f) ? acc : 0.f;
 }
 
 // a4 for the stored-logits mode: dS = c_t (exp(z - lse) - onehot) from the fp32 logits panel the
@@ -892,7 +867,7 @@ static cudaError_t launch_gemm(int epi, const OperandView& A, const OperandView&
     if (nt == 2) return launch_gemm_epi<kEpiStoreBf16, 2, 2>(ta, tb, g, grid, st);
     switch (epi) {
         AWR_HEAD_CASE(kEpiLse) AWR_HEAD_CASE(kEpiDs) AWR_HEAD_CASE(kEpiStoreBf16) AWR_HEAD_CASE(kEpiAccum)
-        AWR_HEAD_CASE(kEpiLse16) AWR_HEAD_CASE(kEpiLseRef)
+        AWR_HEAD_CASE(kEpiLse16) AWR_HEAD_CASE(kEpiLseRef) AWR_HEAD_CASE(kEpiRowMax)
         default: return cudaErrorInvalidValue;
     }
 #undef AWR_HEAD_CASE
@@ -1054,14 +1029,6 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
     const OperandView w_bwd{c.w_head, c.K, c.V, kv ? c.V : c.K, kv ? kMajorK : kMajorMN};
     cudaError_t e = cudaMemsetAsync(w.zy, 0, (size_t)w.part_ld * 4, st);
     if (e != cudaSuccess) return e;
-    if (rowref) {
-        const int warps = 8;
-        head_ref_kernel<<<(unsigned)((c.n_tok + warps - 1) / warps), warps * 32, 0, st>>>(
-            H, reinterpret_cast<const __nv_bfloat16*>(c.w_head), kv ? 1 : 0, c.V, c.K,
-            c.rows->target_ids, c.n_tok, w.zref);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-    }
 
     // pass F + a3 over rows [r0, r0 + rows): log-sum-exp partials + gather, then the scalars.
     // Partials / gathered logits are indexed by global row (pointers pre-offset by r0).
@@ -1076,6 +1043,17 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         // raster: when the H rows of this call fit in L2 (a panel: 39 MB at K = 2048) walk all of
         // its row tiles before the next W column tile, so W_head streams from HBM exactly once
         const int fgm = rows * c.K * 2 <= (48ll << 20) ? (int)((rows + kBM * ctas - 1) / (kBM * ctas)) : gm;
+        if (rowref) {
+            // the exp reference of every row of the panel: its largest logit among the first 256
+            // vocabulary entries (one column tile of the same GEMM, 1 / 594 of the forward flops)
+            EpiArgs er = {};
+            er.zref_out = w.zref + r0;
+            OperandView w_ref = w_fwd;
+            w_ref.mn = c.V < kBN ? c.V : kBN;
+            cudaError_t err = launch_gemm(kEpiRowMax, OperandView{H + r0 * c.K, rows, c.K, c.K, kMajorK},
+                                          w_ref, 0, fgm, er, num_sms, ctas, st);
+            if (err != cudaSuccess) return err;
+        }
         cudaError_t err = launch_gemm(rowref ? kEpiLseRef : (e16 ? kEpiLse16 : kEpiLse),
                                       OperandView{H + r0 * c.K, rows, c.K, c.K, kMajorK},
                                       w_fwd, 0, fgm, ea, num_sms, ctas, st);
@@ -1190,8 +1168,8 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
 int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode) {
     const HeadWs w = head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2, mode);
     // recompute: F, scalars, then (dS GEMM, dH, dW) per panel; stored / E16: (F, scalars, dS pass, dH, dW) per panel
-    // row reference: the reference kernel, then (F, scalars, dH, dW) per panel
-    if (mode == kHeadRowRef) return 1 + 4 * w.n_panels;
+    // row reference: (reference tile, F, scalars, dH, dW) per panel
+    if (mode == kHeadRowRef) return 5 * w.n_panels;
     return mode != kHeadRecompute ? 5 * w.n_panels : 2 + 3 * w.n_panels;
 }
 

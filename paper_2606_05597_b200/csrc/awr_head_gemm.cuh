@@ -93,10 +93,12 @@ enum { kEpiLse = 0,      // a2 on the tile: per-row (max, sum exp) partials + ta
        kEpiAccum = 3,    // C accumulated over row panels in fp32, bf16 on the last panel (dw_head)
        kEpiLse16 = 4,    // kEpiLse that also keeps the tile as E = bf16(exp(z - tile row max)): two
                          // passes over the accumulator (max, then exp + sum + store)
-       kEpiLseRef = 5 }; // the same with a PER-ROW reference known before the GEMM (zref[row], an estimate
-                         // of the target logit): E = bf16(exp(z - zref)) in ONE pass over the accumulator;
-                         // dS = E * f_row, so the scale moves into the dhidden epilogue (row_scale) and
-                         // into the H operand of the dw_head GEMM, and no dS pass is left
+       kEpiLseRef = 5,   // the same with a PER-ROW reference known before the GEMM (zref[row]):
+                         // E = bf16(exp(z - zref)) in ONE pass over the accumulator; dS = E * f_row, so
+                         // the scale moves into the dhidden epilogue (row_scale) and into the H operand
+                         // of the dw_head GEMM, and no dS pass is left
+       kEpiRowMax = 6 }; // zref[row] = max of the tile's row (one column tile only: the reference of
+                         // kEpiLseRef is the row's largest logit among the first 256 vocabulary entries)
 
 // How one operand is staged and described to the tensor core (all runtime values).
 struct Operand {
@@ -124,6 +126,7 @@ struct EpiArgs {
     __nv_bfloat16* eout;       // kEpiLse16 / kEpiLseRef [M, eout_ld]: E = exp(z - m), m the .x of part[]
     int64_t eout_ld;
     const float* zref;         // kEpiLseRef [M]: the row's exp reference (finite)
+    float* zref_out;           // kEpiRowMax [M]
     // kEpiDs
     const float* row_lse;      // [M] log-sum-exp of the whole row
     const float* row_coef;     // [M] c_t

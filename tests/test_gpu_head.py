@@ -143,8 +143,7 @@ def test_head_several_panels(norm, kernel, n_tok, panels):
     ora = _oracle_head(batch, normalizer=norm)
     _check_head(gpu, ora, A.W_K_BY_V)
     per_call = 5 * panels if kernel in HEAD_PANEL_KERNELS else 2 + 3 * panels
-    if kernel == A.KERNEL_HEAD_2CTA_ROWREF:
-        per_call = 1 + 4 * panels          # reference kernel, then (F, scalars, dhidden, dw_head) per panel
+    # row reference: (reference tile, F, scalars, dhidden, dw_head) per panel - also 5
     assert A.head_launches_per_call(n_tok, 512, 64, kernel) == 3 + per_call
     assert A.head_launches_per_call(n_tok, 512, 64) == A.head_launches_per_call(
         n_tok, 512, 64, A.KERNEL_HEAD_2CTA_ROWREF)          # AUTO resolves to the row-reference mode
@@ -160,26 +159,27 @@ def test_head_stored_logits_same_bits_as_recompute():
         assert torch.equal(a[k], b[k]), k
 
 
-def test_head_rowref_peaked_and_unlikely_targets():
-    """Row-reference mode away from its comfortable case.  The reference is an estimate of the TARGET
-    logit, so every e = exp(z - zref) is p_v / p_y: (a) rows whose target is the far most likely
-    token (p_y -> 1, all other e tiny) and (b) rows whose target is 40 nats below the row maximum
-    (e up to e^40, sums of 1e17) must still meet the oracle at the usual bars; nothing is flagged."""
+@pytest.mark.parametrize("loud_id", [7, 700])
+def test_head_rowref_peaked_and_unlikely_targets(loud_id):
+    """Row-reference mode away from its comfortable case.  The reference of a row is its largest logit
+    among the first 256 vocabulary entries.  One "loud" token gets a logit ~40 above all others in
+    every row; a third of the rows have it as target (p_y -> 1), the others keep a target 40 nats
+    below it.  loud_id = 7: the reference IS the loud logit, every stored e <= 1 and the unlikely
+    targets sit at e^-40; loud_id = 700: the reference is an ordinary logit, the loud entry is stored
+    as e^40 and the row sums are 1e17.  Both must meet the oracle at the usual bars, nothing flagged."""
     n_tok, K, V = 600, 128, 2056
     batch = _head_batch(n_tok, K, V, seed=61, lp_mode="drift", masked_frac=0.02)
     hid = batch["hidden"].float()
     w = batch["w_head"].float().clone()                       # [K, V]
     ids = batch["target_ids"].clone()
-    # column 7 of W becomes a "loud" token: logit = 0.5 * |h|^2 / sqrt(K)-ish, large and positive for
-    # every row; rows 0::3 get it as target (peaked), rows 1::3 keep a random target far below it
     loud = hid.mean(0)
     loud = loud / loud.norm() * 4.0
-    w[:, 7] = loud
+    w[:, loud_id] = loud
     batch["w_head"] = w.to(torch.bfloat16)
-    hid = hid + 10.0 * loud / loud.norm()                    # every row has a component along it: z_7 ~ 40
+    hid = hid + 10.0 * loud / loud.norm()                    # every row has a component along it: z_loud ~ 40
     batch["hidden"] = hid.to(torch.bfloat16)
     sel = torch.arange(n_tok, device=DEV) % 3 == 0
-    ids[sel & (ids >= 0)] = 7
+    ids[sel & (ids >= 0)] = loud_id
     batch["target_ids"] = ids
     z = batch["hidden"].float() @ batch["w_head"].float()
     lp = torch.log_softmax(z.double(), -1)
@@ -194,23 +194,23 @@ def test_head_rowref_peaked_and_unlikely_targets():
 
 
 def test_head_rowref_overflow_is_reported():
-    """A token whose target logit is more than ~88 nats below another logit of its row (p_y < 1e-38)
-    cannot be represented relative to its reference: AWR_ERRBIT_HEAD_RANGE is set, the token
-    contributes nothing (zero term, zero dhidden row, token_lp 0 like a masked token) and every
-    other row is what the oracle gives with that token masked."""
+    """A row with a logit more than ~88 nats above its reference (the largest of its first 256 logits)
+    cannot be represented relative to it: AWR_ERRBIT_HEAD_RANGE is set, the token contributes
+    nothing (zero term, zero dhidden row, token_lp 0 like a masked token) and every other row is
+    what the oracle gives with that token masked."""
     n_tok, K, V = 300, 64, 1000
     batch = _head_batch(n_tok, K, V, seed=62)
     hid = batch["hidden"].float().clone()
     w = batch["w_head"].float().clone()
     bad = 17
     y = int(batch["target_ids"][bad])
-    other = (y + 1) % V
-    w[:, other] = hid[bad] / hid[bad].norm() * 3.0            # z[bad, other] = 3 |h| ~ 24 ... scale up below
-    hid[bad] *= 6.0                                           # |h| ~ 48: z[bad, other] ~ 144, target logit ~ N(0, 1)
+    other = 500 if y != 500 else 501                          # beyond the reference tile
+    w[:, other] = hid[bad] / hid[bad].norm() * 3.0
+    hid[bad] *= 6.0                                           # |h| ~ 48: z[bad, other] ~ 144, the rest ~ N(0, 1)
     batch["hidden"] = hid.to(torch.bfloat16)
     batch["w_head"] = w.to(torch.bfloat16)
     z = batch["hidden"].float() @ batch["w_head"].float()
-    assert float(z[bad, other] - z[bad, y]) > 100.0
+    assert float(z[bad, other] - z[bad, :256].max()) > 100.0
     gpu = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA_ROWREF)
     assert int(gpu["err_word"][0]) == A.ERRBIT_HEAD_RANGE
     assert float(gpu["token_lp"][bad]) == 0.0 and float(gpu["tok_term"][bad]) == 0.0
@@ -222,6 +222,10 @@ def test_head_rowref_overflow_is_reported():
     ora = _oracle_head(masked)
     gpu["err_word"].zero_()
     _check_head(gpu, ora, A.W_K_BY_V)
+    # the other modes take the same row in their stride
+    e16 = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA_E16)
+    assert int(e16["err_word"][0]) == 0
+    _check_head(e16, _oracle_head(batch), A.W_K_BY_V)
 
 
 def test_head_shapes_agree_bitwise_on_integers():
