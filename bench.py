@@ -299,7 +299,8 @@ def measured_peaks():
 
 
 KERNEL_NAMES = {1: "rows_generic_kernel", 2: "rows_cluster_kernel", 3: "rows_rf_kernel<NU,2>",
-                4: "rows_rf_kernel<NU,4>", 8: "rows_fwd_kernel", 10: "rows_rfs_kernel<NU>"}
+                4: "rows_rf_kernel<NU,4>", 8: "rows_fwd_kernel", 10: "rows_rfs_kernel<NU>",
+                12: "rows_rfs_kernel<NU> (late statistics)"}
 
 
 def load_traffic(leg: str):
@@ -510,7 +511,8 @@ def run_cuda(args):
     init_dist("nccl")
 
     kernel = {"auto": A.KERNEL_AUTO, "generic": A.KERNEL_GENERIC, "cluster": A.KERNEL_CLUSTER,
-              "rf": A.KERNEL_CLUSTER_RF, "rf4": A.KERNEL_CLUSTER_RF4, "rfs": A.KERNEL_CLUSTER_RFS}[args.kernel]
+              "rf": A.KERNEL_CLUSTER_RF, "rf4": A.KERNEL_CLUSTER_RF4, "rfs": A.KERNEL_CLUSTER_RFS,
+              "rfs_late": A.KERNEL_CLUSTER_RFS_LATE}[args.kernel]
     leg, batch, call, local_ms = rows_leg(torch, A, W, dev, args.config, args.steps, args.warmup,
                                           seed=1000 + rank, normalizer=args.normalizer, kernel=kernel,
                                           n_tok=args.n_tok or None, backward=not args.forward_only,
@@ -620,9 +622,12 @@ def run_regimes(args):
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     batch = W.make_batch(W.workload(1), seed=1000, device=dev)
+    kern = {"auto": A.KERNEL_AUTO, "rfs": A.KERNEL_CLUSTER_RFS, "rfs_late": A.KERNEL_CLUSTER_RFS_LATE,
+            "rf": A.KERNEL_CLUSTER_RF, "rf4": A.KERNEL_CLUSTER_RF4, "cluster": A.KERNEL_CLUSTER,
+            "generic": A.KERNEL_GENERIC}[args.kernel]
     call = A.LossCall(batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
                       batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"],
-                      want=("err_word",), **batch["params"])
+                      want=("err_word",), **dict(batch["params"], kernel=kern))
     stream = torch.cuda.current_stream(dev)
 
     def events(n):
@@ -671,7 +676,7 @@ def run_regimes(args):
     flat = [v for r in bursts[1:] for v in r]
     print(json.dumps({"regimes": {
         "workload": "BASELINE.json configs[1], awr_loss_fwd_bwd, kernel %s" % KERNEL_NAMES.get(
-            A.select_kernel(batch["V"], batch["ld"], batch["logits"].dtype)),
+            kern if kern != A.KERNEL_AUTO else A.select_kernel(batch["V"], batch["ld"], batch["logits"].dtype)),
         "back_to_back": {"calls": steps, "wall_ms": round(wall_ms, 1), "by_20_calls": blocks,
                          "reasons": sorted(clk.reasons)},
         "between_gemm_bursts": {"kernel_ms": bursts, "mean_ms_after_first_burst": round(sum(flat) / len(flat), 3),
@@ -781,7 +786,7 @@ def main(argv=None):
                     help="BASELINE.json configs[i]; 5 = the Thinking-variant shapes (SURVEY 8(f) rank 4)")
     ap.add_argument("--n-tok", type=int, default=0, help="override the config's token count")
     ap.add_argument("--normalizer", type=int, default=None, choices=[0, 1])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4", "rfs"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4", "rfs", "rfs_late"])
     ap.add_argument("--head-kernel", default="auto", choices=["auto", "1cta", "2cta", "stored", "e16", "rowref"],
                     help="config 4: tcgen05 shape / backward mode (auto = stored: CTA pairs, fp32 "
                          "logits of one row panel kept for the dS pass; 1cta / 2cta recompute)")

@@ -113,8 +113,11 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_CLUSTER_RFS = 10 /* row resident in the register files of a 2-CTA cluster, 15 data
                                     warps + one service warp per CTA: whole-slot TMA loads, gradient
                                     through shared-memory staging and TMA bulk stores, (max, sum)
-                                    exchange by st.async, a3 on the service warp (bf16, 15,368 <= V
-                                    <= 153,600; AUTO's choice for awr_loss_fwd_bwd there) */,
+                                    exchange by st.async, a3 on the service warp; rows pipelined in
+                                    groups of 5 rounds, the row's (max, sum) sent for a3 BEFORE the last
+                                    group's gradient is staged (its statistics taken from the ring) so
+                                    that the a3 hand-over is hidden (bf16, 15,368 <= V <= 153,600; AUTO's
+                                    choice for awr_loss_fwd_bwd there) */,
        AWR_KERNEL_HEAD_2CTA_ROWREF = 11 /* fused head, CTA pairs: E = bf16(exp(z - zref_t)) with a per-row
                                     reference computed before the GEMM (zref_t = the row's largest logit
                                     among the first 256 vocabulary entries: one column tile), so dS =
@@ -122,7 +125,13 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     by f_t, the dw_head GEMM reads bf16(f_t hidden_t); no pass over the
                                     panel is left.  A valid token whose row has a logit more than ~88 nats
                                     above that reference sets AWR_ERRBIT_HEAD_RANGE and contributes
-                                    nothing (use AWR_KERNEL_HEAD_2CTA_E16 for such logits) */ };
+                                    nothing (use AWR_KERNEL_HEAD_2CTA_E16 for such logits) */,
+       AWR_KERNEL_CLUSTER_RFS_LATE = 12 /* AWR_KERNEL_CLUSTER_RFS with the row's (max, sum) sent for a3 after
+                                    the last register group has been exponentiated instead of before its
+                                    gradient is staged: the data warps wait ~2 k clocks per row for a3,
+                                    but 25 % fewer shared-memory sweeps.  Measured (config 1): ~8 % slower
+                                    than CLUSTER_RFS in a cold burst at the boost clock, ~5 % faster at
+                                    power-capped SM clocks (between dense GEMMs) - DESIGN.md section 4 */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u,
        AWR_ERRBIT_HEAD_RANGE = 16u /* AWR_KERNEL_HEAD_2CTA_ROWREF only: exp(z - zref) overflowed in a row */ };

@@ -31,6 +31,7 @@ KERNEL_FWD_STREAM = 8
 KERNEL_HEAD_2CTA_E16 = 9
 KERNEL_CLUSTER_RFS = 10
 KERNEL_HEAD_2CTA_ROWREF = 11
+KERNEL_CLUSTER_RFS_LATE = 12
 ERRBIT_STEP_OFF, ERRBIT_TRAJ_OFF, ERRBIT_GROUP_OFF, ERRBIT_TARGET_RANGE = 1, 2, 4, 8
 ERRBIT_HEAD_RANGE = 16
 

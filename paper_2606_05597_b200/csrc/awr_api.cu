@@ -68,7 +68,7 @@ static int check_params(const awr_params* p) {
     if (p->flags & ~(uint32_t)(AWR_FLAG_SAMPLE_STD | AWR_FLAG_SUCCESS_FILTER | AWR_FLAG_COUPLED |
                                AWR_FLAG_SKIP_UNIFORM))
         return AWR_ERR_PARAM;
-    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_HEAD_2CTA_ROWREF) return AWR_ERR_PARAM;
+    if (p->kernel < AWR_KERNEL_AUTO || p->kernel > AWR_KERNEL_CLUSTER_RFS_LATE) return AWR_ERR_PARAM;
     return AWR_OK;
 }
 
@@ -96,7 +96,8 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool 
                           bool backward = true) {
     if (requested == AWR_KERNEL_FWD_STREAM)                   // forward only, bf16, 16-byte units
         return (!backward && rows_fwd_supported(V, ld, dtype)) ? AWR_KERNEL_FWD_STREAM : -1;
-    if (requested == AWR_KERNEL_CLUSTER_RFS) return rows_rfs_supported(V, ld, dtype) ? AWR_KERNEL_CLUSTER_RFS : -1;
+    if (requested == AWR_KERNEL_CLUSTER_RFS || requested == AWR_KERNEL_CLUSTER_RFS_LATE)
+        return rows_rfs_supported(V, ld, dtype) ? requested : -1;
     if (requested > AWR_KERNEL_CLUSTER_RF4) return -1;        // a fused-head kernel id
     // forward only: nothing has to stay on chip for a second pass, so whole rows are streamed
     // (config 1: see DESIGN.md section 4 for the measured rates of all the kernels on this path)
@@ -123,7 +124,8 @@ static int resolve_kernel(int requested, int64_t V, int64_t ld, int dtype, bool 
 static cudaError_t launch_rows(int kernel, const RowArgs& a, int dtype, int num_sms,
                                cudaStream_t st) {
     if (kernel == AWR_KERNEL_FWD_STREAM) return launch_rows_fwd(a, num_sms, st);
-    if (kernel == AWR_KERNEL_CLUSTER_RFS) return launch_rows_rfs(a, num_sms, st);
+    if (kernel == AWR_KERNEL_CLUSTER_RFS) return launch_rows_rfs(a, num_sms, /*early_stats=*/true, st);
+    if (kernel == AWR_KERNEL_CLUSTER_RFS_LATE) return launch_rows_rfs(a, num_sms, /*early_stats=*/false, st);
     if (kernel == AWR_KERNEL_CLUSTER_RF) return launch_rows_rf(a, num_sms, 2, st);
     if (kernel == AWR_KERNEL_CLUSTER_RF4) return launch_rows_rf(a, num_sms, 4, st);
     if (kernel == AWR_KERNEL_CLUSTER) return launch_rows_cluster(a, num_sms, st);

@@ -54,7 +54,7 @@ cudaError_t launch_rows_rf(const RowArgs& a, int num_sms, int cluster_size, cuda
 // a2 + a3 + a4, the register-file design with a service warp per CTA (awr_rows_rfs.cu): whole-slot
 // TMA loads, staged TMA gradient stores, st.async exchange, a3 on the service warp.
 bool rows_rfs_supported(int64_t V, int64_t ld, int dtype);
-cudaError_t launch_rows_rfs(const RowArgs& a, int num_sms, cudaStream_t st);
+cudaError_t launch_rows_rfs(const RowArgs& a, int num_sms, bool early_stats, cudaStream_t st);
 
 // a2 + a3 forward only (awr_loss_fwd), bf16 rows streamed once through a TMA-filled ring; no
 // gradient, no row residency (awr_rows_fwd.cu).

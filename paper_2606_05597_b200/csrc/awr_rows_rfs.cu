@@ -22,11 +22,21 @@
 //     (pass 0) and exponentiate it (pass 1).  Every group carries its own exp reference (the
 //     thread's max over the group), so no warp-wide or row-wide max sits between the passes and
 //     the MUFU-bound pass of the next row runs while the TMA stores of this row drain through the
-//     write port.  Measured against the predecessor (pass 0 of the next row inside the staging
-//     waits, then one MUFU pass over the whole row): slower in a cold burst at the 1,965 MHz boost
-//     clock (4.05 against 3.70 ms for config 1), faster once the board has settled under load
-//     (3.8-3.95 against 4.1-4.3 ms) and at the power-capped clocks of a training step (4.95 against
-//     5.45 ms between bursts of dense GEMMs): DESIGN.md section 4, profiles/r2_rows.md.
+//     write port.
+//   * Statistics of the LAST group early (template parameter EARLY; AWR_KERNEL_CLUSTER_RFS, AUTO): the
+//     row's (max, sum) can leave for a3 only when every element has been exponentiated, and the next
+//     iteration needs a3's answer at once: st.async -> service warp -> publish is 1.5-2 k clocks that
+//     every data warp waited for at the top of every row (14.7 % of the warp samples of a capture).
+//     The last group's registers still hold the previous row at that point, so its statistics are
+//     taken straight from the ring - two sweeps over shared memory (max; then exp, sum, and e written
+//     back IN PLACE as bf16) - the statistics are sent, and only then is the previous row's last
+//     group staged (pass 2) and the e reloaded from the ring: the hand-over runs behind that work.
+//     EARLY = false (AWR_KERNEL_CLUSTER_RFS_LATE) keeps pass 2 / pass 0 / pass 1 for the last group
+//     too and sends afterwards.  Measured, config 1, same lease: EARLY 3.78 ms
+//     in the first 20 calls from an idle board (boost clock), 3.90-3.97 ms over the next 80, 4.05-4.15
+//     ms at 1.7 GHz, 5.16-5.35 ms between bursts of dense GEMMs (1.35 GHz); late 3.98-4.06 / 3.71-3.86 /
+//     3.84-3.98 / 4.97-5.05 ms; the predecessor schedule (pass 0 of the next row inside the staging
+//     waits, then one MUFU pass per row) 3.69 / 4.12 / 4.30 / 5.45 ms.
 //   * Exchange: every consumer warp sends its (max, sum[, sum e z]) with st.async to BOTH CTAs; the
 //     16 bytes complete a transaction count on the receiver's mbarrier - no cluster barrier, no
 //     fence.  The service warp of each CTA merges the 30 states, evaluates a3 once (header loads
@@ -76,7 +86,7 @@ struct SvPlan {
 
 // NU = rounds per row half = ceil(max half units / 480), compile time: the register array of a
 // consumer thread is v[NU][4] (one 16-byte unit per round).
-template <int NU, bool ENT>
+template <int NU, bool ENT, bool EARLY>
 __global__ void __launch_bounds__(kSvThreads, 1)
 rows_rfs_kernel(RowArgs a, SvPlan p) {
     using namespace ptx;
@@ -297,16 +307,107 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
             }
 
             float mrun = -INFINITY, st = 0.f, szt = 0.f;  // this thread's (max, sum, sum e z) of the next row
+            // the warp's state of the next row, then the exchange: (m_w, s_w, sz_w) to both CTAs, data
+            // and signal in one st.async each
+            auto send_stats = [&]() {
+                float wm = mrun;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) wm = fmaxf(wm, __shfl_xor_sync(kFull, wm, o));
+                const float sc = (mrun == -INFINITY) ? 0.f : ex2_approx((mrun - wm) * kLog2e);
+                st *= sc;
+                if (ENT) szt *= sc;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    st += __shfl_xor_sync(kFull, st, o);
+                    if (ENT) szt += __shfl_xor_sync(kFull, szt, o);
+                }
+                if (lane < 2)
+                    st_async_f32x4(smem_u32(&ctrl->stats[par ^ 1][(int)rank * kSvConsumers + warp]),
+                                   stats_full0 + 8u * (uint32_t)(par ^ 1), (uint32_t)lane, wm, st, szt, 0.f);
+            };
+            // fold a group's (m, sum, sum e z) into the thread's state of the row
+            auto fold = [&](float m, float gsum, float gsz) {
+                const float M = fmaxf(mrun, m);
+                const float f_old = (mrun == -INFINITY) ? 0.f : ex2_approx((mrun - M) * kLog2e);
+                const float f_new = (m == -INFINITY) ? 0.f : ex2_approx((m - M) * kLog2e);
+                st = st * f_old + gsum * f_new;
+                if (ENT) szt = szt * f_old + gsz * f_new;
+                mrun = M;
+            };
+            const uint32_t src = ring + my_off;                  // the ring slots are contiguous
+            // the last group's reference of THIS row: its slot in mref2 is overwritten (next row) before
+            // this row's pass 2 of that group reads it
+            const float mref_last = get_mref(NG - 1);
+            auto mref_cur = [&](int g) { return g == NG - 1 ? mref_last : get_mref(g); };
 #pragma unroll
             for (int g = 0; g < NG; ++g) {
                 const int sl = g / kGroupsPerSlot;
                 const bool slot_used = sl * kSvSlotRounds < nr;                       // warp-uniform
+                const bool last = g == NG - 1;                                        // compile time
+                // ---- LAST group of the next row, early: its (max, sum) straight from the ring while
+                // its registers still hold this row, e = exp2((z - m) log2 e) written back IN PLACE as
+                // bf16, so that the row's statistics leave for a3 before pass 2 of this group instead
+                // of after its pass 1: the a3 hand-over (st.async -> service warp -> publish, 1.5-2 k
+                // clocks that every data warp used to wait for at the top of the next row) runs
+                // behind that pass 2 and the reload.  Two sweeps over shared memory (max, then exp):
+                // every thread re-reads only the 16-byte units it wrote itself.
+                if (EARLY && last && have_next) {
+                    if (g % kGroupsPerSlot == 0 && slot_used) mbar_wait(full0 + 8u * sl, (uint32_t)(it + 1) & 1u);
+                    // the target entry is left out of the row's state: its holder overwrites it with
+                    // -inf in the ring (its own later loads of that unit follow in program order)
+                    if (ynpos >= g * kSvStageRounds * 8) {
+                        const uint32_t at = src + (uint32_t)(ynpos >> 3) * kSvRoundBytes + (uint32_t)(ynpos & 7) * 2u;
+                        asm volatile("st.shared.u16 [%0], %1;" ::"r"(at), "h"((unsigned short)0xff80) : "memory");
+                    }
+                    auto load_masked = [&](int k, uint32_t (&t)[4]) {
+                        lds128(t, src + (uint32_t)k * kSvRoundBytes);
+                        if (k >= NU - 2 && k * kSvRoundUnits + (int)(my_off >> 4) >= half_units)
+                            t[0] = t[1] = t[2] = t[3] = kSvNegInf2;
+                    };
+                    uint32_t mx2 = kSvNegInf2;
+#pragma unroll
+                    for (int kk = 0; kk < kSvStageRounds; ++kk) {
+                        const int k = g * kSvStageRounds + kk;
+                        if (k < NU) {
+                            uint32_t t[4];
+                            load_masked(k, t);
+                            mx2 = max_bf16x2(mx2, max_bf16x2(max_bf16x2(t[0], t[1]), max_bf16x2(t[2], t[3])));
+                        }
+                    }
+                    const float m = fmaxf(bf16_lo(mx2), bf16_hi(mx2));
+                    const float nref = (m == -INFINITY) ? 0.f : -m * kLog2e;
+                    const float2 l2 = make_float2(kLog2e, kLog2e), nref2 = make_float2(nref, nref);
+                    float2 acc[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+                    float2 accz = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int kk = 0; kk < kSvStageRounds; ++kk) {
+                        const int k = g * kSvStageRounds + kk;
+                        if (k < NU) {
+                            uint32_t t[4];
+                            load_masked(k, t);
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                const float2 z = make_float2(bf16_lo(t[j]), bf16_hi(t[j]));
+                                const float2 x = fma_f32x2(z, l2, nref2);
+                                const float2 e = make_float2(ex2_approx(x.x), ex2_approx(x.y));
+                                acc[j & 1] = add_f32x2(acc[j & 1], e);
+                                if (ENT)
+                                    accz = fma_f32x2(e, make_float2(fmaxf(z.x, kZFloor), fmaxf(z.y, kZFloor)), accz);
+                                t[j] = pack_bf16x2(e.x, e.y);
+                            }
+                            sts128(src + (uint32_t)k * kSvRoundBytes, make_uint4(t[0], t[1], t[2], t[3]));
+                        }
+                    }
+                    fold(m, (acc[0].x + acc[0].y) + (acc[1].x + acc[1].y), accz.x + accz.y);
+                    set_mref(g, m);
+                    send_stats();
+                }
                 // ---- pass 2 (a4) of this row, group g: dlogits = e * (c_t exp(m_g - lse)) into a
                 // staging buffer.  c_t = 0 (masked, zero advantage, clip triggered): F = +0 and
                 // e >= 0 give all-bits-zero products
                 if (backward && have_cur && g * kSvStageRounds < nr) {
                     const float2 cl = *reinterpret_cast<const float2*>(rinfo);            // (c_t, lse)
-                    const float F = cl.x == 0.f ? 0.f : cl.x * ex2_approx((get_mref(g) - cl.y) * kLog2e);
+                    const float F = cl.x == 0.f ? 0.f : cl.x * ex2_approx((mref_cur(g) - cl.y) * kLog2e);
                     const __nv_bfloat16 fh = __float2bfloat16_rn(F);
                     const __nv_bfloat16 fl = __float2bfloat16_rn(F - __bfloat162float(fh));
                     const uint32_t Fh = (uint32_t)__bfloat16_as_ushort(fh) * 0x00010001u;
@@ -339,11 +440,26 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
                     if (lane == 0) mbar_arrive(sfull0 + 8u * (gp & 1u));
                 }
                 if (!have_next) continue;
+                if (EARLY && last) {
+                    // ---- reload of the last group: the e written above, ring -> registers; the slot
+                    // is released behind a proxy fence (the next fill of the slot is an async-proxy
+                    // write over these generic-proxy writes)
+#pragma unroll
+                    for (int kk = 0; kk < kSvStageRounds; ++kk) {
+                        const int k = g * kSvStageRounds + kk;
+                        if (k < NU) lds128(v[k], src + (uint32_t)k * kSvRoundBytes);
+                    }
+                    if (slot_used) {
+                        fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(empty0 + 8u * sl);
+                    }
+                    continue;
+                }
                 // ---- pass 0 of the next row, group g: ring -> registers, target entry masked to -inf
                 // (token_scalars works from lse_rest), packed max; the slot is released after its
                 // last group
                 if (g % kGroupsPerSlot == 0 && slot_used) mbar_wait(full0 + 8u * sl, (uint32_t)(it + 1) & 1u);
-                const uint32_t src = ring + my_off;                  // the two slots are contiguous
 #pragma unroll
                 for (int kk = 0; kk < kSvStageRounds; ++kk) {
                     const int k = g * kSvStageRounds + kk;
@@ -404,33 +520,10 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
                         }
                     }
                 }
-                // fold the group into the thread's state of the row
-                const float M = fmaxf(mrun, m);
-                const float f_old = (mrun == -INFINITY) ? 0.f : ex2_approx((mrun - M) * kLog2e);
-                const float f_new = (m == -INFINITY) ? 0.f : ex2_approx((m - M) * kLog2e);
-                st = st * f_old + ((acc[0].x + acc[0].y) + (acc[1].x + acc[1].y)) * f_new;
-                if (ENT) szt = szt * f_old + (accz.x + accz.y) * f_new;
-                mrun = M;
+                fold(m, (acc[0].x + acc[0].y) + (acc[1].x + acc[1].y), accz.x + accz.y);
                 set_mref(g, m);
             }
-            if (have_next) {
-                // ---- the warp's state, then the exchange: (m_w, s_w, sz_w) of the next row to both
-                // CTAs, data and signal in one st.async each
-                float wm = mrun;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) wm = fmaxf(wm, __shfl_xor_sync(kFull, wm, o));
-                const float sc = (mrun == -INFINITY) ? 0.f : ex2_approx((mrun - wm) * kLog2e);
-                st *= sc;
-                if (ENT) szt *= sc;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-                    st += __shfl_xor_sync(kFull, st, o);
-                    if (ENT) szt += __shfl_xor_sync(kFull, szt, o);
-                }
-                if (lane < 2)
-                    st_async_f32x4(smem_u32(&ctrl->stats[par ^ 1][(int)rank * kSvConsumers + warp]),
-                                   stats_full0 + 8u * (uint32_t)(par ^ 1), (uint32_t)lane, wm, st, szt, 0.f);
-            }
+            if (!EARLY && have_next) send_stats();     // the late schedule: after pass 1 of the last group
             ypos = ynpos;
         }
     }
@@ -465,7 +558,7 @@ bool rows_rfs_supported(int64_t V, int64_t ld, int dtype) {
     return make_sv_plan(V, ld, dtype, p, nu);
 }
 
-template <int NU, bool ENT>
+template <int NU, bool ENT, bool EARLY>
 static cudaError_t launch_sv(const RowArgs& a, SvPlan p, int num_sms, cudaStream_t st) {
     static PerDeviceInt cached;              // co-resident clusters (device query, cached per device)
     const int dev = PerDeviceInt::device();
@@ -482,12 +575,12 @@ static cudaError_t launch_sv(const RowArgs& a, SvPlan p, int num_sms, cudaStream
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     if (max_clusters < 0) {
-        cudaError_t e = cudaFuncSetAttribute(rows_rfs_kernel<NU, ENT>,
+        cudaError_t e = cudaFuncSetAttribute(rows_rfs_kernel<NU, ENT, EARLY>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, kSvSmemBytes);
         if (e != cudaSuccess) return e;
         cfg.gridDim = dim3(2 * num_sms, 1, 1);
         int n = 0;
-        e = cudaOccupancyMaxActiveClusters(&n, rows_rfs_kernel<NU, ENT>, &cfg);
+        e = cudaOccupancyMaxActiveClusters(&n, rows_rfs_kernel<NU, ENT, EARLY>, &cfg);
         if (e != cudaSuccess) return e;
         const int want = num_sms / 2;
         max_clusters = n < 1 ? 1 : (n > want ? want : n);
@@ -497,19 +590,20 @@ static cudaError_t launch_sv(const RowArgs& a, SvPlan p, int num_sms, cudaStream
     if ((int64_t)nc > a.n_tok) nc = (int)a.n_tok;
     p.num_clusters = nc;
     cfg.gridDim = dim3(2 * nc, 1, 1);
-    return cudaLaunchKernelEx(&cfg, rows_rfs_kernel<NU, ENT>, a, p);
+    return cudaLaunchKernelEx(&cfg, rows_rfs_kernel<NU, ENT, EARLY>, a, p);
 }
 
-cudaError_t launch_rows_rfs(const RowArgs& a, int num_sms, cudaStream_t st) {
+template <bool EARLY>
+static cudaError_t launch_rows_rfs_t(const RowArgs& a, int num_sms, cudaStream_t st) {
     if (a.n_tok <= 0) return cudaSuccess;
     SvPlan p;
     int nu = 0;
     if (!make_sv_plan(a.V, a.ld, AWR_DTYPE_BF16, p, nu)) return cudaErrorInvalidValue;
     switch (nu) {
-#define AWR_SV_CASE(N)                                                                  \
-    case N:                                                                             \
-        return a.token_entropy != nullptr ? launch_sv<N, true>(a, p, num_sms, st)       \
-                                          : launch_sv<N, false>(a, p, num_sms, st);
+#define AWR_SV_CASE(N)                                                                       \
+    case N:                                                                                  \
+        return a.token_entropy != nullptr ? launch_sv<N, true, EARLY>(a, p, num_sms, st)     \
+                                          : launch_sv<N, false, EARLY>(a, p, num_sms, st);
         AWR_SV_CASE(3) AWR_SV_CASE(4) AWR_SV_CASE(5) AWR_SV_CASE(6) AWR_SV_CASE(7) AWR_SV_CASE(8)
         AWR_SV_CASE(9) AWR_SV_CASE(10) AWR_SV_CASE(11) AWR_SV_CASE(12) AWR_SV_CASE(13)
         AWR_SV_CASE(14) AWR_SV_CASE(15) AWR_SV_CASE(16) AWR_SV_CASE(17) AWR_SV_CASE(18)
@@ -517,6 +611,12 @@ cudaError_t launch_rows_rfs(const RowArgs& a, int num_sms, cudaStream_t st) {
 #undef AWR_SV_CASE
         default: return cudaErrorInvalidValue;
     }
+}
+
+// early_stats: the schedule (file header); both produce the same values up to fp32 rounding of the
+// last group's sum
+cudaError_t launch_rows_rfs(const RowArgs& a, int num_sms, bool early_stats, cudaStream_t st) {
+    return early_stats ? launch_rows_rfs_t<true>(a, num_sms, st) : launch_rows_rfs_t<false>(a, num_sms, st);
 }
 
 }  // namespace awr

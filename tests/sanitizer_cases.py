@@ -49,7 +49,7 @@ def main():
     big = W.workload(3, n_groups=6, group_size=4, n_tok=300)            # V = 151,936 bf16
     for name, k in (("generic", A.KERNEL_GENERIC), ("cluster", A.KERNEL_CLUSTER),
                     ("cluster_rf", A.KERNEL_CLUSTER_RF), ("cluster_rf4", A.KERNEL_CLUSTER_RF4),
-                    ("cluster_rfs", A.KERNEL_CLUSTER_RFS)):
+                    ("cluster_rfs", A.KERNEL_CLUSTER_RFS), ("cluster_rfs_late", A.KERNEL_CLUSTER_RFS_LATE)):
         print("300 x 151,936 bf16,", name, ":", rows_case(big, k))
     print("300 x 151,936 bf16, cluster_rf + entropy:", rows_case(big, A.KERNEL_CLUSTER_RF, entropy=True))
     for ent in (False, True):

@@ -78,7 +78,7 @@ def test_host_side_status_codes():
     assert f(C.byref(B), C.byref(P), C.byref(Oo), None, 0, None) == _abi.AWR_ERR_DTYPE
     B.logits_dtype = 0
     for bad in (dict(k_norm=0.0), dict(clip_eps=1.0), dict(clip_eps=-0.1), dict(normalizer=3),
-                dict(flags=16), dict(dual_clip_c=float("nan")), dict(kernel=12),
+                dict(flags=16), dict(dual_clip_c=float("nan")), dict(kernel=13),
                 dict(stale_cap=float("nan"))):
         Q = _abi.awr_params(10.0, 0.2, 0.0, 1.0, 0.0, 0, 0, 0)
         for k, v in bad.items():

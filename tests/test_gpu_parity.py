@@ -72,7 +72,8 @@ CLUSTER_SHAPES = [(151_936, 151_936), (40_000, 40_008), (32_768, 32_768), (65_54
                   (131_072, 131_072)]
 
 
-CLUSTER_KERNELS = [A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4, A.KERNEL_CLUSTER_RFS]
+CLUSTER_KERNELS = [A.KERNEL_CLUSTER, A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4, A.KERNEL_CLUSTER_RFS,
+                   A.KERNEL_CLUSTER_RFS_LATE]
 
 
 @pytest.mark.parametrize("kernel", CLUSTER_KERNELS)
@@ -310,7 +311,8 @@ def test_dynamic_sampling_flag():
 
 @pytest.mark.parametrize("flags", [A.FLAG_SUCCESS_FILTER, A.FLAG_COUPLED,
                                    A.FLAG_SUCCESS_FILTER | A.FLAG_COUPLED])
-@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RFS])
+@pytest.mark.parametrize("kernel", [A.KERNEL_GENERIC, A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RFS,
+                                    A.KERNEL_CLUSTER_RFS_LATE])
 def test_baseline_variants(flags, kernel):
     """the paper's two comparison losses by flag - RAFT++ (advantage =
     1[R > 0]; run at group size 1 as in :462 and at 4) and the coupled-ratio
@@ -364,6 +366,8 @@ def test_dual_clip(kernel, norm):
                                             (A.KERNEL_CLUSTER_RF, 40_000, torch.bfloat16),
                                             (A.KERNEL_CLUSTER_RFS, 151_936, torch.bfloat16),
                                             (A.KERNEL_CLUSTER_RFS, 40_000, torch.bfloat16),
+                                            (A.KERNEL_CLUSTER_RFS_LATE, 151_936, torch.bfloat16),
+                                            (A.KERNEL_CLUSTER_RFS_LATE, 40_000, torch.bfloat16),
                                             (A.KERNEL_AUTO, 151_936, torch.bfloat16)])
 @pytest.mark.parametrize("backward", [True, False])
 def test_token_entropy(kernel, V, dtype, backward):
@@ -440,6 +444,23 @@ def test_deterministic():
     b = P.run_gpu(batch)
     for k in a:
         assert torch.equal(a[k], b[k]), k
+
+
+@pytest.mark.parametrize("V,ld", [(151_936, 151_936), (40_000, 40_008), (20_000, 20_000)])
+def test_rfs_schedules_same_bits(V, ld):
+    """AWR_KERNEL_CLUSTER_RFS takes the last register group's (max, sum) from the ring before that
+    group's registers are free and writes exp back in place; AWR_KERNEL_CLUSTER_RFS_LATE does it in
+    registers afterwards.  Same elements, same references, same fold order: every output, the
+    gradient included, must be bit-identical (config-3 laws: clips, zero-advantage rows, masked
+    tokens; NG = 4, 2 and 1 groups per row half)."""
+    w = W.workload(3, n_groups=4, group_size=4, n_tok=700, V=V)
+    batch = W.make_batch(w, seed=77, device=DEV, ld=ld, masked_frac=0.05)
+    outs = []
+    for kernel in (A.KERNEL_CLUSTER_RFS, A.KERNEL_CLUSTER_RFS_LATE):
+        batch["params"]["kernel"] = kernel
+        outs.append(P.run_gpu(batch, dual_clip_c=3.0))
+    for k in outs[0]:
+        assert torch.equal(outs[0][k], outs[1][k]), k
 
 
 # ------------------------------------------------------------------ edge cases
@@ -576,7 +597,8 @@ def test_register_file_kernels_random_shapes(V, ld, n_tok, seed):
     (fewer rows than clusters included), both cluster shapes, entropy on."""
     w = W.workload(3, n_groups=3, group_size=4, n_tok=max(n_tok, 12), V=V)
     batch = W.make_batch(w, seed=seed % 1000, device=DEV, ld=ld, masked_frac=0.05)
-    kernels = [A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4] + ([A.KERNEL_CLUSTER_RFS] if V <= 153_600 else [])
+    kernels = [A.KERNEL_CLUSTER_RF, A.KERNEL_CLUSTER_RF4] + (
+        [A.KERNEL_CLUSTER_RFS, A.KERNEL_CLUSTER_RFS_LATE] if V <= 153_600 else [])
     for kernel in kernels:
         batch["params"]["kernel"] = kernel
         gpu, ora = P.full_check(batch, dual_clip_c=3.0)
@@ -636,7 +658,7 @@ def _zones_intact(buf, pad_e, n, pattern):
 
 @pytest.mark.parametrize("kernel,backward", [(A.KERNEL_GENERIC, True), (A.KERNEL_CLUSTER, True),
                                              (A.KERNEL_CLUSTER_RF, True), (A.KERNEL_CLUSTER_RF4, True),
-                                             (A.KERNEL_CLUSTER_RFS, True),
+                                             (A.KERNEL_CLUSTER_RFS, True), (A.KERNEL_CLUSTER_RFS_LATE, True),
                                              (A.KERNEL_FWD_STREAM, False)])
 @pytest.mark.parametrize("V,ld", [(151_936, 151_936), (40_000, 40_008)])
 def test_red_zones_row_kernels(kernel, backward, V, ld):
