@@ -460,7 +460,10 @@ def test_rfs_schedules_same_bits(V, ld):
         batch["params"]["kernel"] = kernel
         outs.append(P.run_gpu(batch, dual_clip_c=3.0))
     for k in outs[0]:
-        assert torch.equal(outs[0][k], outs[1][k]), k
+        a, b = outs[0][k], outs[1][k]
+        if k == "dlogits":                       # the padding columns >= V are not written by anybody
+            a, b = a[:, :V], b[:, :V]
+        assert torch.equal(a, b), k
 
 
 # ------------------------------------------------------------------ edge cases
