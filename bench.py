@@ -28,6 +28,8 @@ The JSON line:
                 config 2 under 1/k and under 1/|tau_i|, config 3 into a separate gradient buffer and
                 in place, config 4 (fused LM head, tensor roofline), awr_loss_fwd on config 1
   --impl reference   times the oracle alone (this tier's reference arm)
+  --regimes [--kernel rfs|rfs_late]   diagnostic, its own JSON object: per-call kernel times of
+                config 1 against the board's clock state
 """
 from __future__ import annotations
 
@@ -788,8 +790,9 @@ def main(argv=None):
     ap.add_argument("--normalizer", type=int, default=None, choices=[0, 1])
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "cluster", "rf", "rf4", "rfs", "rfs_late"])
     ap.add_argument("--head-kernel", default="auto", choices=["auto", "1cta", "2cta", "stored", "e16", "rowref"],
-                    help="config 4: tcgen05 shape / backward mode (auto = stored: CTA pairs, fp32 "
-                         "logits of one row panel kept for the dS pass; 1cta / 2cta recompute)")
+                    help="config 4: tcgen05 shape / backward mode (auto = rowref: CTA pairs, bf16 exp(z - "
+                         "row reference) of one row panel kept, no dS pass; e16: exp(z - tile max) + an "
+                         "in-place dS pass; stored: fp32 logits panel; 1cta / 2cta recompute)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: --steps")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
