@@ -129,9 +129,9 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
        AWR_KERNEL_CLUSTER_RFS_LATE = 12 /* AWR_KERNEL_CLUSTER_RFS with the row's (max, sum) sent for a3 after
                                     the last register group has been exponentiated instead of before its
                                     gradient is staged: the data warps wait ~2 k clocks per row for a3,
-                                    but 25 % fewer shared-memory sweeps.  Measured (config 1): ~8 % slower
-                                    than CLUSTER_RFS in a cold burst at the boost clock, ~5 % faster at
-                                    power-capped SM clocks (between dense GEMMs) - DESIGN.md section 4 */ };
+                                    but 25 % fewer shared-memory sweeps.  Measured (config 1): 5-8 % slower
+                                    than CLUSTER_RFS in a cold burst at the boost clock, 2-3 % faster at
+                                    1.6-1.8 GHz, level between dense GEMMs - DESIGN.md section 4 */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
        AWR_ERRBIT_TARGET_RANGE = 8u,
        AWR_ERRBIT_HEAD_RANGE = 16u /* AWR_KERNEL_HEAD_2CTA_ROWREF only: exp(z - zref) overflowed in a row */ };

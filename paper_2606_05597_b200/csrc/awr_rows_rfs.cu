@@ -32,10 +32,13 @@
 //     back IN PLACE as bf16) - the statistics are sent, and only then is the previous row's last
 //     group staged (pass 2) and the e reloaded from the ring: the hand-over runs behind that work.
 //     EARLY = false (AWR_KERNEL_CLUSTER_RFS_LATE) keeps pass 2 / pass 0 / pass 1 for the last group
-//     too and sends afterwards.  Measured, config 1, same lease: EARLY 3.78 ms
-//     in the first 20 calls from an idle board (boost clock), 3.90-3.97 ms over the next 80, 4.05-4.15
-//     ms at 1.7 GHz, 5.16-5.35 ms between bursts of dense GEMMs (1.35 GHz); late 3.98-4.06 / 3.71-3.86 /
-//     3.84-3.98 / 4.97-5.05 ms; the predecessor schedule (pass 0 of the next row inside the staging
+//     too and sends afterwards.  The row's last piece then reaches the TMA late, so the service lane
+//     frees the staging buffer of the piece before it as soon as that piece's own store has read it
+//     out (a blocking wait_group.read 0 at a point where nothing else is due) instead of at the next
+//     hand-over.  Measured, config 1, same lease: EARLY 3.79 ms in the first
+//     20 calls from an idle board (boost clock), 3.83-3.93 ms over the next 80, 3.97-4.07 ms at 1.65
+//     GHz, 4.83-4.95 ms between bursts of dense GEMMs (1.35 GHz); late 3.97-4.09 / 3.78-3.91 /
+//     3.91-4.04 / 4.90-4.99 ms; the predecessor schedule (pass 0 of the next row inside the staging
 //     waits, then one MUFU pass per row) 3.69 / 4.12 / 4.30 / 5.45 ms.
 //   * Exchange: every consumer warp sends its (max, sum[, sum e z]) with st.async to BOTH CTAs; the
 //     16 bytes complete a transaction count on the receiver's mbarrier - no cluster barrier, no
