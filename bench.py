@@ -382,7 +382,8 @@ def rows_leg(torch, A, W, dev, cfg, steps, warmup, *, seed=1000, normalizer=None
            "normalizer": "1/k" if params["normalizer"] == A.NORM_CONST_K else "1/|tau_i|",
            "in_place": bool(in_place and backward), "entry": call._name,
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm"], "unit": "GB/s",
-                        "frac": achieved / peaks["hbm"], "traffic": traffic, "traffic_source": capture,
+                        "frac": achieved / peaks["hbm"], "frac_of_8tbs_data_sheet": achieved / 8000.0,
+                        "traffic": traffic, "traffic_source": capture,
                         "kernel": KERNEL_NAMES.get(kern, str(kern)), "kernel_ms": row_ms,
                         "kernel_share_of_step": row_ms / (local_ms / steps),
                         "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peaks["src"]},
