@@ -326,9 +326,13 @@ rows_rfs_kernel(RowArgs a, SvPlan p) {
             // the warp's state of the next row, then the exchange: (m_w, s_w, sz_w) to both CTAs, data
             // and signal in one st.async each
             auto send_stats = [&]() {
-                float wm = mrun;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) wm = fmaxf(wm, __shfl_xor_sync(kFull, wm, o));
+                // max over the warp in ONE instruction (floats order like their bits once the negative
+                // ones are flipped): this chain is on the critical path of the a3 hand-over
+                int mi = __float_as_int(mrun);
+                mi ^= (mi >> 31) & 0x7fffffff;
+                mi = __reduce_max_sync(kFull, mi);
+                mi ^= (mi >> 31) & 0x7fffffff;
+                const float wm = __int_as_float(mi);
                 const float sc = (mrun == -INFINITY) ? 0.f : ex2_approx((mrun - wm) * kLog2e);
                 st *= sc;
                 if (ENT) szt *= sc;
