@@ -466,6 +466,34 @@ def test_rfs_schedules_same_bits(V, ld):
         assert torch.equal(a, b), k
 
 
+@pytest.mark.parametrize("kernel", [A.KERNEL_CLUSTER_RFS, A.KERNEL_CLUSTER_RFS_LATE])
+@pytest.mark.parametrize("V,ld,n_tok", [(151_936, 151_936, 1500), (40_000, 40_008, 37)])
+def test_rfs_soak_bit_identical(V, ld, n_tok, kernel):
+    """300 back-to-back calls of the service-warp kernel (mbarrier hand-overs between 15 data warps,
+    the service warp, the TMA and the peer CTA; ring slots and staging buffers reused every row):
+    every output stays bit-identical to the first call's.  Stands in for racecheck (closed on this
+    pool): a lost hand-over shows as a wrong row or a hang."""
+    w = W.workload(3, n_groups=4, group_size=4, n_tok=n_tok, V=V)
+    batch = W.make_batch(w, seed=5, device=DEV, ld=ld, masked_frac=0.03)
+    call = A.LossCall(batch["logits"], batch["target_ids"], batch["behave_lp"], batch["prox_lp"],
+                      batch["step_off"], batch["traj_off"], batch["group_off"], batch["rewards"],
+                      want=("err_word", "tok_term", "tok_coef", "token_entropy"),
+                      **dict(batch["params"], kernel=kernel, dual_clip_c=3.0))
+    call.run()
+    torch.cuda.synchronize()
+    ref = {k: v.clone() for k, v in call.out.items()}
+    for i in range(300):
+        call.out["dlogits"].fill_(7.0)
+        call.run()
+        if i % 50 == 49:
+            torch.cuda.synchronize()
+            for k, v in ref.items():
+                a, b = call.out[k], v
+                if k == "dlogits":
+                    a, b = a[:, :V], b[:, :V]
+                assert torch.equal(a, b), (k, i)
+
+
 # ------------------------------------------------------------------ edge cases
 def test_empty_batch():
     z = torch.empty(0, 1024, dtype=torch.bfloat16, device=DEV)
