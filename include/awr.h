@@ -123,9 +123,9 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     among the first 256 vocabulary entries: one column tile), so dS =
                                     E f_t with ONE factor per row: the dhidden GEMM scales its output rows
                                     by f_t, the dw_head GEMM reads bf16(f_t hidden_t); no pass over the
-                                    panel is left.  A valid token whose row has a logit more than ~88 nats
-                                    above that reference sets AWR_ERRBIT_HEAD_RANGE and contributes
-                                    nothing (use AWR_KERNEL_HEAD_2CTA_E16 for such logits) */,
+                                    panel is left.  A row with a logit more than ~88 nats above that
+                                    reference (exp overflows; none on ordinary logits) is redone exactly
+                                    from hidden and w_head on the CUDA cores (~2 ms per such row) */,
        AWR_KERNEL_CLUSTER_RFS_LATE = 12 /* AWR_KERNEL_CLUSTER_RFS with the row's (max, sum) sent for a3 after
                                     the last register group has been exponentiated instead of before its
                                     gradient is staged: the data warps wait ~2 k clocks per row for a3,
@@ -133,8 +133,7 @@ enum { AWR_KERNEL_AUTO = 0,     /* pick by shape / dtype */
                                     than CLUSTER_RFS in a cold burst at the boost clock, 2-3 % faster at
                                     1.6-1.8 GHz, level between dense GEMMs - DESIGN.md section 4 */ };
 enum { AWR_ERRBIT_STEP_OFF = 1u, AWR_ERRBIT_TRAJ_OFF = 2u, AWR_ERRBIT_GROUP_OFF = 4u,
-       AWR_ERRBIT_TARGET_RANGE = 8u,
-       AWR_ERRBIT_HEAD_RANGE = 16u /* AWR_KERNEL_HEAD_2CTA_ROWREF only: exp(z - zref) overflowed in a row */ };
+       AWR_ERRBIT_TARGET_RANGE = 8u };
 
 /* One batch of response tokens (:61 "G rollouts per task, |tau_i| steps per rollout,
  * |tau_{i,j}| tokens per step"), as three CSR offset arrays.  Each offset array starts at 0,

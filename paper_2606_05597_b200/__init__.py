@@ -3,7 +3,7 @@ and its gradient over the LM-head vocabulary: hand-written sm_100a CUDA kernels 
 of include/awr.h (libawr.so), plus this thin torch-tensor binding.  No CPU fallback exists."""
 from ._abi import (AwrError, DTYPE_BF16, DTYPE_F32, ERRBIT_GROUP_OFF, ERRBIT_STEP_OFF,
                    ERRBIT_TARGET_RANGE, ERRBIT_TRAJ_OFF, FLAG_SAMPLE_STD, FLAG_SUCCESS_FILTER, FLAG_COUPLED, FLAG_SKIP_UNIFORM, KERNEL_AUTO,
-                   KERNEL_CLUSTER, KERNEL_CLUSTER_RF, KERNEL_CLUSTER_RF4, KERNEL_CLUSTER_RFS, KERNEL_CLUSTER_RFS_LATE, KERNEL_GENERIC, KERNEL_HEAD_1CTA, KERNEL_HEAD_2CTA, KERNEL_HEAD_2CTA_STORED, KERNEL_HEAD_2CTA_E16, KERNEL_HEAD_2CTA_ROWREF, ERRBIT_HEAD_RANGE, KERNEL_FWD_STREAM, NORM_CONST_K, NORM_PER_TRAJ, W_K_BY_V,
+                   KERNEL_CLUSTER, KERNEL_CLUSTER_RF, KERNEL_CLUSTER_RF4, KERNEL_CLUSTER_RFS, KERNEL_CLUSTER_RFS_LATE, KERNEL_GENERIC, KERNEL_HEAD_1CTA, KERNEL_HEAD_2CTA, KERNEL_HEAD_2CTA_STORED, KERNEL_HEAD_2CTA_E16, KERNEL_HEAD_2CTA_ROWREF, KERNEL_FWD_STREAM, NORM_CONST_K, NORM_PER_TRAJ, W_K_BY_V,
                    W_V_BY_K, STATIC_WS_BYTES, lib_path, load)
 from .api import (HEAD_OPTIONAL_OUTPUTS, HeadLossCall, HostHeadLossCall, HostLossCall, LossCall, head_host_workspace_bytes, awr_gemm_bf16,
                   awr_loss_fwd_bwd_fused_head, head_launches_per_call, head_workspace_bytes, OPTIONAL_OUTPUTS, awr_group_advantage, awr_loss_fwd,

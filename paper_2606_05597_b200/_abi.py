@@ -33,7 +33,6 @@ KERNEL_CLUSTER_RFS = 10
 KERNEL_HEAD_2CTA_ROWREF = 11
 KERNEL_CLUSTER_RFS_LATE = 12
 ERRBIT_STEP_OFF, ERRBIT_TRAJ_OFF, ERRBIT_GROUP_OFF, ERRBIT_TARGET_RANGE = 1, 2, 4, 8
-ERRBIT_HEAD_RANGE = 16
 
 _vp = C.c_void_p
 

@@ -9,6 +9,8 @@
 //              the accumulator                                                  (GEMM, kEpiLseRef)
 //     scalars  partials -> lse, l_t, ratio / clip / normalizer (a3), c_t; then f_t = c_t exp(zref_t -
 //              lse), the target entry of E, and Hs = bf16(f_t h_t)                 (one warp per row)
+//     fix-up   rows with a logit > 88 nats above zref_t (none on ordinary logits) redone exactly from
+//              hidden and w_head on the CUDA cores                                  (one CTA per such row)
 //     pass G2  dhidden[panel] = diag(f) (E W_head^T): row scale in the epilogue    (GEMM, kEpiStoreBf16)
 //     pass G3  dw_head += Hs^T E   (fp32 running sum, bf16 at the end)             (GEMM, kEpiAccum)
 //   so dS = diag(f) E is never formed.  E16 mode: E relative to the tile's row max (kEpiLse16, two
@@ -377,8 +379,8 @@ head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a,
                 // The row's exp reference is known before the GEMM (zref: the largest of the row's
                 // first 256 logits), so ONE pass over the accumulator gives both the sum and
                 // E = bf16(exp(z - zref)).  The unrounded e feed the partial; an overflowing e (a logit
-                // 88 nats above the reference) makes the sum +inf, which head_scalars_kernel reports;
-                // the stored E is clamped to a finite value so that a zero row scale still gives zeros.
+                // 88 nats above the reference) makes the sum +inf: head_scalars_kernel marks the row and
+                // head_fix_rows_kernel redoes it; the stored E is clamped to a finite value meanwhile.
                 const int y = row_ok ? g.e.target_ids[row] : -1;
                 const bool want_ent = g.e.partz != nullptr;
                 const bool y_here = (y >= n0) && (y < n0 + kTN) && (y < g.N);
@@ -582,7 +584,8 @@ namespace head {
 // the panel this warp writes f_row (the dhidden GEMM scales its output rows by it), the row of
 // Hs = bf16(f_row H) (the A operand of the dw_head GEMM) and ONE element of E: the target entry,
 // (p_y - 1) exp(lse - zref), so that E f_row = c_t (p_y - 1) there.  A row whose sum overflowed
-// (a logit 88 nats above the reference) sets AWR_ERRBIT_HEAD_RANGE and contributes nothing.
+// (a logit 88 nats above the reference) is marked in `fix` and written as a row that contributes
+// nothing; head_fix_rows_kernel then redoes exactly that row from hidden and w_head.
 struct HeadRefArgs {
     const float* zref;            // [n_tok] or nullptr
     float* row_f;                 // [n_tok]
@@ -591,6 +594,7 @@ struct HeadRefArgs {
     const __nv_bfloat16* hidden;  // [n_tok, K]
     __nv_bfloat16* hs;            // [panel rows, K], row 0 = token row0
     int64_t K;
+    uint8_t* fix;                 // [n_tok] 1 = the row's sum overflowed relative to zref
 };
 
 __global__ void __launch_bounds__(256)
@@ -633,7 +637,6 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
     const TokenScalars ts = token_scalars(h, lse_rest, valid, a.clip_eps, a.stale_cap, a.dual_c);
     if (lane == 0) {
         if (h.y >= a.V) atomicOr(a.err_word, AWR_ERRBIT_TARGET_RANGE);
-        if (overflow) atomicOr(a.err_word, AWR_ERRBIT_HEAD_RANGE);
         store_token_outputs(a, row, h, ts, valid);
         if (a.token_entropy) a.token_entropy[row] = valid ? row_entropy(ts.lse, st.m, sz, ts.lp, h.zy) : 0.f;
         row_lse[row] = ts.lse;
@@ -645,6 +648,7 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
         const float f = ts.coef == 0.f ? 0.f : ts.coef * ex2_approx((zr - ts.lse) * kLog2e);
         if (lane == 0) {
             ref.row_f[row] = f;
+            ref.fix[row] = overflow ? 1 : 0;
             if (f != 0.f) {
                 const float ty = (ts.gy / ts.coef) * ex2_approx((ts.lse - zr) * kLog2e);
                 ref.e[(row - row0) * ref.e_ld + h.y] = __float2bfloat16_rn(fmaxf(ty, -3.0e38f));
@@ -663,6 +667,99 @@ head_scalars_kernel(RowArgs a, const float2* __restrict__ part, int64_t part_ld,
             }
             dst[u] = o;
         }
+    }
+}
+
+// Row-reference mode, the rows head_scalars_kernel marked in `fix` (some logit more than ~88 nats
+// above the row's reference: exp(z - zref) overflowed).  Such a row is redone here from scratch, one
+// CTA per row, on the CUDA cores: logits by plain fp32 dot products of hidden_t with the columns of
+// w_head, an online (max, sum[, sum e z]) over them (target left out), a3, then E relative to the
+// row's TRUE maximum, f_t, Hs and the per-token outputs - everything the forward GEMM and
+// head_scalars_kernel would have written.  Two passes over the dot products (~2 ms per row): the
+// path exists so that the mode is exact for every finite input, not to be fast; on ordinary
+// logits no row is marked and every CTA leaves after one byte load per row.
+struct Triple { float m, s, sz; };
+__device__ __forceinline__ Triple combine3(Triple a, Triple b) {
+    const float M = fmaxf(a.m, b.m);
+    if (M == -INFINITY) return Triple{M, 0.f, 0.f};
+    const float fa = ex2_approx((a.m - M) * kLog2e), fb = ex2_approx((b.m - M) * kLog2e);
+    return Triple{M, a.s * fa + b.s * fb, a.sz * fa + b.sz * fb};
+}
+
+__global__ void __launch_bounds__(512)
+head_fix_rows_kernel(RowArgs a, HeadRefArgs ref, const __nv_bfloat16* __restrict__ w_head, int kv_layout,
+                     float* __restrict__ row_lse, float* __restrict__ row_coef, float* __restrict__ row_gy,
+                     int64_t row0, int64_t row1) {
+    __shared__ Triple wstate[16];
+    __shared__ float sh[6];                       // zy, ref, f, target entry of E, -, -
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t V = a.V, K = ref.K;
+    for (int64_t row = row0 + blockIdx.x; row < row1; row += gridDim.x) {
+        if (!ref.fix[row]) continue;              // the same byte for the whole CTA
+        const int y = a.target_ids[row];          // valid: only valid rows are marked
+        const __nv_bfloat16* hr = ref.hidden + row * K;
+        auto logit = [&](int64_t v) {
+            float acc = 0.f;
+            if (kv_layout) {
+                const __nv_bfloat16* wc = w_head + v;
+                for (int64_t k = 0; k < K; ++k)
+                    acc = fmaf(__bfloat162float(hr[k]), __bfloat162float(wc[k * V]), acc);
+            } else {
+                const __nv_bfloat16* wr = w_head + v * K;
+                for (int64_t k = 0; k < K; ++k)
+                    acc = fmaf(__bfloat162float(hr[k]), __bfloat162float(wr[k]), acc);
+            }
+            return acc;
+        };
+        // ---- pass 1: online (max, sum, sum e z) of the row without its target; the target's logit
+        Triple t{-INFINITY, 0.f, 0.f};
+        for (int64_t v = tid; v < V; v += blockDim.x) {
+            const float z = logit(v);
+            if (v == y) { sh[0] = z; continue; }
+            t = combine3(t, Triple{z, 1.f, fmaxf(z, kZFloor)});
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+            t = combine3(t, Triple{__shfl_xor_sync(kFull, t.m, o), __shfl_xor_sync(kFull, t.s, o),
+                                   __shfl_xor_sync(kFull, t.sz, o)});
+        if (lane == 0) wstate[warp] = t;
+        __syncthreads();
+        if (tid == 0) {
+            Triple r = wstate[0];
+            for (int i = 1; i < (int)(blockDim.x >> 5); ++i) r = combine3(r, wstate[i]);
+            RowHeader h;
+            h.y = y;
+            const int traj = a.tok_traj[row];
+            h.q = a.prox_lp[row];
+            h.b = a.behave_lp[row];
+            h.A = traj >= 0 ? a.adv[traj] : 0.f;
+            h.scale = traj >= 0 ? a.traj_scale[traj] : 0.f;
+            h.zy = sh[0];
+            const float lse_rest = r.m + logf(r.s);                   // -inf when nothing but the target
+            const TokenScalars ts = token_scalars(h, lse_rest, true, a.clip_eps, a.stale_cap, a.dual_c);
+            store_token_outputs(a, row, h, ts, true);
+            if (a.token_entropy) a.token_entropy[row] = row_entropy(ts.lse, r.m, r.sz, ts.lp, h.zy);
+            row_lse[row] = ts.lse;
+            row_coef[row] = ts.coef;
+            row_gy[row] = ts.gy;
+            const float zr = fmaxf(r.m, h.zy);                        // every e <= 1 relative to it
+            const float f = ts.coef == 0.f ? 0.f : ts.coef * ex2_approx((zr - ts.lse) * kLog2e);
+            sh[1] = zr;
+            sh[2] = f;
+            sh[3] = f != 0.f ? (ts.gy / ts.coef) * ex2_approx((ts.lse - zr) * kLog2e) : 0.f;
+            ref.row_f[row] = f;
+            ref.fix[row] = 0;
+        }
+        __syncthreads();
+        // ---- pass 2: E relative to the row's maximum, the target entry, Hs
+        const float nref = -sh[1] * kLog2e, f = sh[2], ty = sh[3];
+        __nv_bfloat16* er = ref.e + (row - row0) * ref.e_ld;
+        for (int64_t v = tid; v < V; v += blockDim.x)
+            er[v] = __float2bfloat16_rn(v == y ? ty : ex2_approx(fmaf(logit(v), kLog2e, nref)));
+        __nv_bfloat16* hsr = ref.hs + (row - row0) * K;
+        for (int64_t k = tid; k < K; k += blockDim.x)
+            hsr[k] = __float2bfloat16_rn(f * __bfloat162float(hr[k]));
+        __syncthreads();                                              // sh / wstate are reused by the next row
     }
 }
 
@@ -964,6 +1061,7 @@ struct HeadWs {
     float* zpanel;           // stored-logits mode: fp32 [panel_rows, z_ld]
     float* zpanel2;          // second buffer: the forward of panel p + 1 runs beside the dS pass of p
     float *zref, *row_f;     // row-reference mode: exp reference and dS scale of every row
+    uint8_t* fix;            // row-reference mode: rows to be redone by head_fix_rows_kernel
     __nv_bfloat16* hs;       // row-reference mode: bf16(f_row H) of the panel [panel_rows, K]
     int64_t part_ld, ds_ld, z_ld, panel_rows;
     int n_vtiles, n_panels;
@@ -1002,6 +1100,7 @@ static HeadWs head_carve(void* base, int64_t n_tok, int64_t V, int64_t K, int ct
     const bool rowref = mode == kHeadRowRef;
     w.zref = (float*)take(rowref ? (size_t)n_pad * 4 : 0);
     w.row_f = (float*)take(rowref ? (size_t)n_pad * 4 : 0);
+    w.fix = (uint8_t*)take(rowref ? (size_t)n_pad : 0);
     w.hs = (__nv_bfloat16*)take(rowref ? (size_t)w.panel_rows * K * 2 : 0);
     w.total = off;
     return w;
@@ -1061,11 +1160,17 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
         const int warps = 8;
         const unsigned blocks = (unsigned)((rows + warps - 1) / warps);
         HeadRefArgs ra = {};
-        if (rowref) ra = HeadRefArgs{w.zref, w.row_f, w.ds, w.ds_ld, H, w.hs, c.K};
+        if (rowref) ra = HeadRefArgs{w.zref, w.row_f, w.ds, w.ds_ld, H, w.hs, c.K, w.fix};
         head_scalars_kernel<<<blocks, warps * 32, 0, st>>>(*c.rows, w.part, w.part_ld, w.n_vtiles,
                                                            c.rows->token_entropy ? w.partz : nullptr,
                                                            w.zy, w.row_lse, w.row_coef, w.row_gy,
                                                            r0, r0 + rows, ra);
+        err = cudaGetLastError();
+        if (err != cudaSuccess || !rowref) return err;
+        // rows whose sum overflowed relative to their reference (none on ordinary logits): redone exactly
+        const unsigned fblocks = (unsigned)(rows < 2 * (int64_t)num_sms ? rows : 2 * (int64_t)num_sms);
+        head_fix_rows_kernel<<<fblocks, 512, 0, st>>>(*c.rows, ra, reinterpret_cast<const __nv_bfloat16*>(c.w_head),
+                                                      kv ? 1 : 0, w.row_lse, w.row_coef, w.row_gy, r0, r0 + rows);
         return cudaGetLastError();
     };
     if (c.mode == kHeadRecompute) {
@@ -1168,8 +1273,8 @@ cudaError_t launch_head(const HeadCall& c, int num_sms, cudaStream_t st) {
 int head_launches(int64_t n_tok, int64_t V, int64_t K, int ctas, int mode) {
     const HeadWs w = head_carve(nullptr, n_tok, V, K, ctas == 1 ? 1 : 2, mode);
     // recompute: F, scalars, then (dS GEMM, dH, dW) per panel; stored / E16: (F, scalars, dS pass, dH, dW) per panel
-    // row reference: (reference tile, F, scalars, dH, dW) per panel
-    if (mode == kHeadRowRef) return 5 * w.n_panels;
+    // row reference: (reference tile, F, scalars, fix-up of overflowed rows, dH, dW) per panel
+    if (mode == kHeadRowRef) return 6 * w.n_panels;
     return mode != kHeadRecompute ? 5 * w.n_panels : 2 + 3 * w.n_panels;
 }
 

@@ -143,7 +143,8 @@ def test_head_several_panels(norm, kernel, n_tok, panels):
     ora = _oracle_head(batch, normalizer=norm)
     _check_head(gpu, ora, A.W_K_BY_V)
     per_call = 5 * panels if kernel in HEAD_PANEL_KERNELS else 2 + 3 * panels
-    # row reference: (reference tile, F, scalars, dhidden, dw_head) per panel - also 5
+    if kernel == A.KERNEL_HEAD_2CTA_ROWREF:
+        per_call = 6 * panels          # (reference tile, F, scalars, fix-up, dhidden, dw_head) per panel
     assert A.head_launches_per_call(n_tok, 512, 64, kernel) == 3 + per_call
     assert A.head_launches_per_call(n_tok, 512, 64) == A.head_launches_per_call(
         n_tok, 512, 64, A.KERNEL_HEAD_2CTA_ROWREF)          # AUTO resolves to the row-reference mode
@@ -193,39 +194,49 @@ def test_head_rowref_peaked_and_unlikely_targets(loud_id):
         _check_head(gpu, ora, A.W_K_BY_V)
 
 
-def test_head_rowref_overflow_is_reported():
-    """A row with a logit more than ~88 nats above its reference (the largest of its first 256 logits)
-    cannot be represented relative to it: AWR_ERRBIT_HEAD_RANGE is set, the token contributes
-    nothing (zero term, zero dhidden row, token_lp 0 like a masked token) and every other row is
-    what the oracle gives with that token masked."""
+@pytest.mark.parametrize("w_layout", [A.W_K_BY_V, A.W_V_BY_K])
+def test_head_rowref_overflow_rows_are_redone(w_layout):
+    """Rows with a logit more than ~88 nats above their reference (the largest of their first 256
+    logits) cannot be represented relative to it: exp overflows, head_scalars_kernel marks the row and
+    head_fix_rows_kernel redoes it from hidden and w_head.  Two such rows (one with the loud token as
+    its target, one with an ordinary target 140 nats below it), a masked row with the same logits,
+    entropy on: every output meets the oracle at the usual bars, nothing is flagged."""
     n_tok, K, V = 300, 64, 1000
     batch = _head_batch(n_tok, K, V, seed=62)
     hid = batch["hidden"].float().clone()
     w = batch["w_head"].float().clone()
-    bad = 17
-    y = int(batch["target_ids"][bad])
-    other = 500 if y != 500 else 501                          # beyond the reference tile
-    w[:, other] = hid[bad] / hid[bad].norm() * 3.0
-    hid[bad] *= 6.0                                           # |h| ~ 48: z[bad, other] ~ 144, the rest ~ N(0, 1)
+    ids = batch["target_ids"].clone()
+    loud = 500                                                # beyond the reference tile
+    bad = [17, 130, 201]
+    d = hid[bad].mean(0)
+    w[:, loud] = d / d.norm() * 3.0
+    for r in bad:
+        hid[r] = 6.0 * (0.2 * hid[r] + d / d.norm() * 8.0)    # z[r, loud] ~ 144, the rest ~ N(0, 1)
+    ids[17] = 3 if int(ids[17]) == loud else ids[17]
+    ids[130] = loud
+    ids[201] = -1
     batch["hidden"] = hid.to(torch.bfloat16)
     batch["w_head"] = w.to(torch.bfloat16)
+    batch["target_ids"] = ids
     z = batch["hidden"].float() @ batch["w_head"].float()
-    assert float(z[bad, other] - z[bad, :256].max()) > 100.0
-    gpu = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA_ROWREF)
-    assert int(gpu["err_word"][0]) == A.ERRBIT_HEAD_RANGE
-    assert float(gpu["token_lp"][bad]) == 0.0 and float(gpu["tok_term"][bad]) == 0.0
-    assert not gpu["dhidden"][bad].any()
+    for r in bad:
+        assert float(z[r, loud] - z[r, :256].max()) > 100.0
+    lp = torch.log_softmax(z.double(), -1).gather(1, ids.clamp(min=0).long()[:, None])[:, 0].float()
+    batch["prox_lp"] = lp + 0.01 * torch.randn_like(lp)       # ratios near 1 also for the -140 nat token
+    batch["behave_lp"] = batch["prox_lp"] + 0.01 * torch.randn_like(lp)
+    params = dict(batch["params"], kernel=A.KERNEL_HEAD_2CTA_ROWREF)
+    wh = batch["w_head"] if w_layout == A.W_K_BY_V else batch["w_head"].t().contiguous()
+    gpu = A.awr_loss_fwd_bwd_fused_head(batch["hidden"], wh, batch["target_ids"], batch["behave_lp"],
+                                        batch["prox_lp"], batch["step_off"], batch["traj_off"],
+                                        batch["group_off"], batch["rewards"], w_layout=w_layout,
+                                        want=A.api.HEAD_OPTIONAL_OUTPUTS + ("token_entropy",), **params)
+    torch.cuda.synchronize()
+    ora = _oracle_head(batch, want_entropy=True)
+    assert ora["token_lp"][17] < -100.0 and ora["token_lp"][130] > -1e-6
+    _check_head(gpu, ora, w_layout)
+    H = gpu["token_entropy"].cpu().numpy().astype(np.float64)
+    assert np.abs(H - ora["token_entropy"]).max() <= 1e-4
     assert torch.isfinite(gpu["dhidden"].float()).all() and torch.isfinite(gpu["dw_head"].float()).all()
-    masked = dict(batch)
-    masked["target_ids"] = batch["target_ids"].clone()
-    masked["target_ids"][bad] = -1
-    ora = _oracle_head(masked)
-    gpu["err_word"].zero_()
-    _check_head(gpu, ora, A.W_K_BY_V)
-    # the other modes take the same row in their stride
-    e16 = _run_head(batch, kernel=A.KERNEL_HEAD_2CTA_E16)
-    assert int(e16["err_word"][0]) == 0
-    _check_head(e16, _oracle_head(batch), A.W_K_BY_V)
 
 
 def test_head_shapes_agree_bitwise_on_integers():
