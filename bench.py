@@ -433,6 +433,8 @@ def head_leg(torch, A, W, dev, steps, warmup, *, seed=1000, head_kernel="auto", 
            "workspace_bytes": int(call.ws_bytes),
            "roofline": {"bound": "tensor", "achieved": achieved, "peak": peaks["tensor"],
                         "unit": "TFLOP/s", "frac": achieved / peaks["tensor"], "traffic": None,
+                        "traffic_source": "null: tensor-bound leg of several kernels; dram bytes per kernel "
+                                          "of one panel are in profiles/r2_head.md",
                         "kernel": "head_gemm_kernel<epi, %s> (%s), whole step" % (
                             "1" if head_kernel == "1cta" else "2",
                             "4 GEMMs, logits recomputed" if exe_ratio != 1.0 else
